@@ -1,0 +1,180 @@
+"""CPU oracle for the oblate-transit model of arXiv:2410.05408 -- TEST INFRASTRUCTURE ONLY.
+
+A thin numpy/ctypes front end over ``gl_oracle.c`` (plain C, fp64; see that file's
+header for the passages it follows and for what pins it).  Nothing in the product
+package ``paper_2410_05408_b200`` imports this module, and this module imports
+nothing from it.  Allowed callers: ``tests/``, ``__graft_entry__.smoke()`` and
+``bench.py``'s ``cpu_baseline`` / ``--impl reference`` legs.
+
+PARITY UNPINNED (no external pin exists; self-consistency pins only): e>0
+orbits, the supersampling convention, chi^2.
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+import subprocess
+from pathlib import Path
+
+import numpy as np
+
+_HERE = Path(__file__).resolve().parent
+_SRC = _HERE / "gl_oracle.c"
+_LIB = _HERE / "libgl_oracle.so"
+
+_dp = ctypes.POINTER(ctypes.c_double)
+_lib = None
+
+
+def build(force: bool = False) -> Path:
+    """Compile gl_oracle.c with gcc (-O2, OpenMP) into oracle/libgl_oracle.so."""
+    if force or not _LIB.exists() or _LIB.stat().st_mtime < _SRC.stat().st_mtime:
+        tmp = _LIB.with_suffix(f".so.tmp{os.getpid()}")
+        cmd = ["gcc", "-O2", "-std=c11", "-fPIC", "-shared", "-fopenmp", "-fno-fast-math",
+               "-ffp-contract=off", "-o", str(tmp), str(_SRC), "-lm"]
+        subprocess.run(cmd, check=True)
+        os.replace(tmp, _LIB)
+    return _LIB
+
+
+def _load():
+    global _lib
+    if _lib is None:
+        build()
+        lib = ctypes.CDLL(str(_LIB))
+        d, i, l = ctypes.c_double, ctypes.c_int, ctypes.c_long
+        lib.gl_oracle_rotation.argtypes = [d, d, d, _dp]
+        lib.gl_oracle_outline.argtypes = [d, d, d, d, d, d, _dp]
+        lib.gl_oracle_outline_locked.argtypes = [d, d, d, d, d, d, d, d, _dp]
+        lib.gl_oracle_leggauss.argtypes = [i, _dp, _dp]
+        lib.gl_oracle_areas.argtypes = [d, d, d, d, d, _dp]
+        lib.gl_oracle_areas.restype = i
+        lib.gl_oracle_areas_snap_simpson.argtypes = [d, d, d, d, d, l, _dp]
+        lib.gl_oracle_flux_outline.argtypes = [d, d, d, d, d, d, d]
+        lib.gl_oracle_flux_outline.restype = d
+        lib.gl_oracle_kepler.argtypes = [d, d]
+        lib.gl_oracle_kepler.restype = d
+        lib.gl_oracle_position.argtypes = [_dp, d, _dp, _dp]
+        lib.gl_oracle_position.restype = i
+        lib.gl_oracle_params_valid.argtypes = [_dp]
+        lib.gl_oracle_params_valid.restype = i
+        lib.gl_oracle_flux_time.argtypes = [_dp, d, d, i]
+        lib.gl_oracle_flux_time.restype = d
+        lib.gl_oracle_lightcurve.argtypes = [_dp, i, _dp, i, d, i, _dp, i]
+        lib.gl_oracle_lightcurve.restype = i
+        lib.gl_oracle_loglike.argtypes = [_dp, i, _dp, i, d, i, _dp, _dp, _dp, _dp, i]
+        lib.gl_oracle_loglike.restype = i
+        lib.gl_oracle_flux_geometry.argtypes = [_dp, l, _dp, i]
+        lib.gl_oracle_flux_geometry.restype = i
+        _lib = lib
+    return _lib
+
+
+def _c(a):
+    a = np.ascontiguousarray(a, dtype=np.float64)
+    return a, a.ctypes.data_as(_dp)
+
+
+def rotation(zeta, eta, xi):
+    """R(zeta,eta,xi) = Rx Ry Rz as a 3x3 array (eq. 6)."""
+    out = np.zeros(9)
+    _load().gl_oracle_rotation(zeta, eta, xi, out.ctypes.data_as(_dp))
+    return out.reshape(3, 3)
+
+
+def outline(a, b, c, zeta, eta, xi):
+    """(dx, dy1, dy2) of eqs. 11-13."""
+    out = np.zeros(3)
+    _load().gl_oracle_outline(a, b, c, zeta, eta, xi, out.ctypes.data_as(_dp))
+    return out
+
+
+def outline_locked(a, b, c, zeta, eta, xi, alpha, beta):
+    """(dx, dy1, dy2) of eqs. B14-B16."""
+    out = np.zeros(3)
+    _load().gl_oracle_outline_locked(a, b, c, zeta, eta, xi, alpha, beta,
+                                     out.ctypes.data_as(_dp))
+    return out
+
+
+def leggauss(n):
+    x, w = np.zeros(n), np.zeros(n)
+    _load().gl_oracle_leggauss(n, x.ctypes.data_as(_dp), w.ctypes.data_as(_dp))
+    return x, w
+
+
+def areas(x0, y0, dx, dy1, dy2):
+    """(A_flat, A_lin, A_quad), n_crossings (or -1 when the overlap is empty)."""
+    A = np.zeros(3)
+    n = _load().gl_oracle_areas(x0, y0, dx, dy1, dy2, A.ctypes.data_as(_dp))
+    return A, n
+
+
+def areas_snap_simpson(x0, y0, dx, dy1, dy2, N):
+    """The paper's literal snap + Simpson algorithm with N intervals."""
+    A = np.zeros(3)
+    _load().gl_oracle_areas_snap_simpson(x0, y0, dx, dy1, dy2, int(N), A.ctypes.data_as(_dp))
+    return A
+
+
+def flux_outline(x0, y0, dx, dy1, dy2, u1, u2):
+    return _load().gl_oracle_flux_outline(x0, y0, dx, dy1, dy2, u1, u2)
+
+
+def kepler(M, e):
+    return _load().gl_oracle_kepler(M, e)
+
+
+def position(params12, t):
+    """(x0, y0, in_front) of the planet centre at time t."""
+    p, pp = _c(params12)
+    x, y = ctypes.c_double(), ctypes.c_double()
+    front = _load().gl_oracle_position(pp, float(t), ctypes.byref(x), ctypes.byref(y))
+    return x.value, y.value, bool(front)
+
+
+def params_valid(params12):
+    p, pp = _c(params12)
+    return bool(_load().gl_oracle_params_valid(pp))
+
+
+def flux_time(params12, t, t_exp=0.0, n_ss=1):
+    p, pp = _c(params12)
+    return _load().gl_oracle_flux_time(pp, float(t), float(t_exp), int(n_ss))
+
+
+def lightcurve(params, times, t_exp=0.0, n_ss=1, nthreads=0):
+    """flux[B,T] (fp64).  ``nthreads`` <= 0 uses every host core."""
+    p, pp = _c(np.atleast_2d(params))
+    t, tp = _c(times)
+    flux = np.empty((p.shape[0], t.shape[0]))
+    _load().gl_oracle_lightcurve(pp, p.shape[0], tp, t.shape[0], float(t_exp), int(n_ss),
+                                 flux.ctypes.data_as(_dp), int(nthreads))
+    return flux
+
+
+def loglike(params, times, t_exp, n_ss, obs, sigma, nthreads=0, return_threads=False):
+    """(chi2[B], flux[B,T]) in fp64."""
+    p, pp = _c(np.atleast_2d(params))
+    t, tp = _c(times)
+    o, op = _c(obs)
+    s, sp = _c(sigma)
+    flux = np.empty((p.shape[0], t.shape[0]))
+    chi2 = np.empty(p.shape[0])
+    used = _load().gl_oracle_loglike(pp, p.shape[0], tp, t.shape[0], float(t_exp), int(n_ss),
+                                     op, sp, chi2.ctypes.data_as(_dp),
+                                     flux.ctypes.data_as(_dp), int(nthreads))
+    if return_threads:
+        return chi2, flux, used
+    return chi2, flux
+
+
+def flux_geometry(geom, nthreads=0, return_threads=False):
+    """flux[N] for rows (d, Rp, f_proj, PA, u1, u2) (config 5)."""
+    g, gp = _c(np.atleast_2d(geom))
+    out = np.empty(g.shape[0])
+    used = _load().gl_oracle_flux_geometry(gp, g.shape[0], out.ctypes.data_as(_dp),
+                                           int(nthreads))
+    if return_threads:
+        return out, used
+    return out
