@@ -1,0 +1,111 @@
+/* greenlantern_b200.h -- C ABI of the B200 (sm_100a) oblate-planet transit library.
+ *
+ * The model is the one of arXiv:2410.05408 (Price et al., the `greenlantern` code); citations
+ * are PAPER.md:<line> (+ equation) of the paper text and DESIGN.md "Readings" (R<n>) where the
+ * paper is silent.  The library holds hand-written CUDA only; there is no CPU fallback.
+ *
+ * Conventions common to every entry point
+ *   - Unless a parameter is marked HOST, every pointer is a CUDA DEVICE pointer owned by the
+ *     caller.  The library never frees, retains or reallocates it.
+ *   - Work is enqueued on `stream` (a cudaStream_t passed as void*; NULL = the legacy default
+ *     stream) and the call returns WITHOUT synchronising.  Buffers must stay alive until the
+ *     stream has passed the work.
+ *   - No hidden device allocation, no global mutable state: calls are re-entrant and may be
+ *     issued concurrently on different streams.
+ *   - Return value: GL_OK or a negative gl_status.  Argument errors (GL_EINVAL) enqueue nothing.
+ *     B == 0, T == 0 or N == 0 is GL_OK and enqueues nothing.
+ *   - Parameters, times, observations and sigmas cross the boundary as fp64 whatever the compute
+ *     dtype: an fp32 time stamp at |t| ~ 40 d is coarser than the whole flux error budget
+ *     (DESIGN.md "Precision plan").
+ *
+ * Parameter row, GL_NPARAMS = 12 doubles (north_star of BASELINE.json; R4-R7):
+ *    0 t0      time of inferior conjunction (same unit as `times`)
+ *    1 P       orbital period
+ *    2 a/R*    semi-major axis in stellar radii
+ *    3 b       signed sky-plane x-offset of the planet centre at t0, in stellar radii
+ *              (x0(t0) = b, eq. 9 with d sin(beta) = b)
+ *    4 e       eccentricity, 0 <= e < 1          5 omega   argument of periastron [rad]
+ *    6 Rp_eq   equatorial radius / R*, 0 < Rp_eq < 0.5
+ *    7 f       flattening (R_eq - R_pol)/R_eq, 0 <= f < 1        (eq. 1)
+ *    8 xi      sky-projected obliquity [rad]: rotation about z' in eq. 6
+ *    9 eta     tilt of the spin axis out of the sky plane [rad]: rotation about y' in eq. 6
+ *   10 u1, 11 u2   quadratic limb darkening I = 1 - u1(1-mu) - u2(1-mu)^2
+ *
+ * What a flux value is (SURVEY.md 8(c); PAPER.md:127-135 eqs. 21-23, :145):
+ *    F_inst = 1 - [c0 A_flat + c1 A_lin + c2 A_quad] / [pi (1 - u1/3 - u2/6)],
+ *    A_flat, A_lin, A_quad = integrals of 1, sqrt(1-r^2), r^2 over (projected outline) n (unit
+ *    disc), c0 = 1-u1-2u2, c1 = u1+2u2, c2 = u2; F_inst = 1 when the overlap is empty or the
+ *    planet is behind the star.  F(t_i) = mean of F_inst over n_ss sub-exposures at
+ *    t_i + ((j+1/2)/n_ss - 1/2) t_exp, j = 0..n_ss-1 (midpoint rule, R18).
+ *
+ * Per-walker invalid parameters do not fail a call: that walker's flux row is NaN and its
+ * chi^2 is +inf.  Invalid = any non-finite entry, P <= 0, e outside [0,1), Rp_eq outside
+ * (0,0.5), f outside [0,1), a/R* (1-e) <= 1, |b|(1+e sin omega) > a/R* (1-e^2),
+ * 1 - u1/3 - u2/6 <= 0.
+ */
+#ifndef GREENLANTERN_B200_H
+#define GREENLANTERN_B200_H
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define GL_NPARAMS 12
+#define GL_NGEOM 6
+
+typedef enum { GL_F32 = 0, GL_F64 = 1 } gl_dtype; /* arithmetic AND output precision */
+
+typedef enum {
+    GL_OK = 0,
+    GL_EINVAL = -1,       /* null pointer, negative size, n_ss < 1, unknown dtype, t_exp not finite */
+    GL_ECUDA = -2,        /* a CUDA runtime call or a launch failed; see gl_last_cuda_error() */
+    GL_EUNSUPPORTED = -3  /* size outside what one launch can index (B*T or N >= 2^40)         */
+} gl_status;
+
+/* gl_lightcurve: flux_out[b*T + i] = F_b(times[i]).
+ *   params  [B, GL_NPARAMS] row-major fp64 (device)      times [T] fp64 (device)
+ *   t_exp   exposure length (HOST scalar, same unit as times; >= 0)   n_ss >= 1 sub-exposures
+ *   flux_out [B, T] row-major, float (GL_F32) or double (GL_F64) (device), fully overwritten.
+ * Steps: Kepler + sky position (eqs. 9-10, R7), outline (PAPER.md:89-96
+ * eqs. 11-13), outline/limb crossings (R3), boundary integrals (eqs. 21-23),
+ * exposure mean -- one fused kernel, nothing per-sub-sample is stored. */
+int gl_lightcurve(const double* params, int B, const double* times, int T, double t_exp, int n_ss,
+                  void* flux_out, gl_dtype dtype, void* stream);
+
+/* gl_loglike: chi2_out[b] = sum_i ((obs[i] - F_b(times[i])) / sigma[i])^2   (R19).
+ *   obs, sigma [T] fp64 (device), sigma > 0 (a non-positive or non-finite sigma makes every
+ *   chi^2 +inf).  chi2_out [B] float/double per dtype, fully overwritten.
+ *   flux_out_or_null: optional [B, T] output as in gl_lightcurve; NULL => the model flux never
+ *   leaves registers.  The residual sum is accumulated in fp64 in both dtypes. */
+int gl_loglike(const double* params, int B, const double* times, int T, double t_exp, int n_ss,
+               const double* obs, const double* sigma, void* chi2_out, void* flux_out_or_null,
+               gl_dtype dtype, void* stream);
+
+/* gl_flux_geometry: steps "crossings + boundary integrals" alone, for N bare geometries.
+ *   geom [N, GL_NGEOM] row-major fp64 (device): (d, Rp, f_proj, PA, u1, u2) -- planet centre at
+ *   (d, 0), d >= 0; projected semi-major axis Rp (0 < Rp < 0.5) at position angle PA [rad],
+ *   counter-clockwise from the star-centre -> planet-centre direction; semi-minor Rp (1-f_proj),
+ *   0 <= f_proj < 1.  flux_out [N] float/double.  An invalid row gives NaN. */
+int gl_flux_geometry(const double* geom, long long N, void* flux_out, gl_dtype dtype, void* stream);
+
+/* HOST-buffer convenience wrappers (used for the end-to-end numbers of bench.py): every pointer
+ * below is a HOST pointer; the call allocates device scratch, copies in, runs the kernel above,
+ * copies out and synchronises before it returns.  Same semantics and status codes otherwise. */
+int gl_lightcurve_host(const double* params, int B, const double* times, int T, double t_exp,
+                       int n_ss, void* flux_out, gl_dtype dtype);
+int gl_loglike_host(const double* params, int B, const double* times, int T, double t_exp, int n_ss,
+                    const double* obs, const double* sigma, void* chi2_out, void* flux_out_or_null,
+                    gl_dtype dtype);
+int gl_flux_geometry_host(const double* geom, long long N, void* flux_out, gl_dtype dtype);
+
+/* Number of kernel launches the calling thread's entry points have enqueued so far (HOST). */
+long long gl_launch_count(void);
+
+const char* gl_strerror(int code);          /* static string, never NULL           */
+const char* gl_last_cuda_error(void);       /* text of the last GL_ECUDA, per thread */
+int gl_version(void);                       /* major*10000 + minor*100 + patch       */
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* GREENLANTERN_B200_H */
