@@ -1,0 +1,189 @@
+"""Thin ctypes binding over the C ABI of include/greenlantern_b200.h.
+
+Argument marshalling only: every step of the path runs inside the CUDA library.  torch is used
+for device memory and streams.  There is NO CPU fallback: if the shared library is missing or a
+tensor is not on a CUDA device, the call raises.
+"""
+from __future__ import annotations
+
+import ctypes
+from pathlib import Path
+
+import numpy as np
+
+GL_F32, GL_F64 = 0, 1
+GL_NPARAMS, GL_NGEOM = 12, 6
+_LIBPATH = Path(__file__).resolve().parent / "csrc" / "libgreenlantern_b200.so"
+_lib = None
+
+EXPORTS = ("gl_lightcurve", "gl_loglike", "gl_flux_geometry", "gl_lightcurve_host",
+           "gl_loglike_host", "gl_flux_geometry_host", "gl_launch_count", "gl_strerror",
+           "gl_last_cuda_error", "gl_version")
+
+
+class GreenlanternError(RuntimeError):
+    pass
+
+
+def load_library():
+    """dlopen csrc/libgreenlantern_b200.so (built by paper_2410_05408_b200.build)."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    if not _LIBPATH.exists():
+        raise GreenlanternError(
+            f"{_LIBPATH} is missing: run `python -m paper_2410_05408_b200.build` (needs nvcc). "
+            "There is no CPU fallback.")
+    lib = ctypes.CDLL(str(_LIBPATH))
+    vp, i, d, ll = ctypes.c_void_p, ctypes.c_int, ctypes.c_double, ctypes.c_longlong
+    lib.gl_lightcurve.argtypes = [vp, i, vp, i, d, i, vp, i, vp]
+    lib.gl_loglike.argtypes = [vp, i, vp, i, d, i, vp, vp, vp, vp, i, vp]
+    lib.gl_flux_geometry.argtypes = [vp, ll, vp, i, vp]
+    lib.gl_lightcurve_host.argtypes = [vp, i, vp, i, d, i, vp, i]
+    lib.gl_loglike_host.argtypes = [vp, i, vp, i, d, i, vp, vp, vp, vp, i]
+    lib.gl_flux_geometry_host.argtypes = [vp, ll, vp, i]
+    for name in ("gl_lightcurve", "gl_loglike", "gl_flux_geometry", "gl_lightcurve_host",
+                 "gl_loglike_host", "gl_flux_geometry_host", "gl_version"):
+        getattr(lib, name).restype = i
+    lib.gl_launch_count.restype = ll
+    lib.gl_strerror.argtypes = [i]
+    lib.gl_strerror.restype = ctypes.c_char_p
+    lib.gl_last_cuda_error.restype = ctypes.c_char_p
+    _lib = lib
+    return lib
+
+
+def _check(rc):
+    if rc != 0:
+        lib = load_library()
+        msg = lib.gl_strerror(rc).decode()
+        if rc == -2:
+            msg += ": " + lib.gl_last_cuda_error().decode()
+        raise GreenlanternError(f"greenlantern_b200 status {rc}: {msg}")
+
+
+def _torch():
+    import torch
+    return torch
+
+
+def _dev_f64(x, shape_tail=None):
+    torch = _torch()
+    if not isinstance(x, torch.Tensor) or not x.is_cuda:
+        raise GreenlanternError("expected a CUDA torch.Tensor (no CPU fallback exists)")
+    if x.dtype != torch.float64 or not x.is_contiguous():
+        raise GreenlanternError("inputs must be contiguous float64 tensors")
+    if shape_tail is not None and (x.dim() != 2 or x.shape[1] != shape_tail):
+        raise GreenlanternError(f"expected shape [*, {shape_tail}]")
+    return x
+
+
+def _tdtype(dtype):
+    torch = _torch()
+    if dtype in (GL_F32, "f32", "float32", torch.float32):
+        return GL_F32, torch.float32
+    if dtype in (GL_F64, "f64", "float64", torch.float64):
+        return GL_F64, torch.float64
+    raise GreenlanternError(f"unknown dtype {dtype!r}")
+
+
+def _stream(x):
+    return ctypes.c_void_p(_torch().cuda.current_stream(x.device).cuda_stream)
+
+
+def gl_lightcurve(params, times, t_exp=0.0, n_ss=1, dtype="f32", out=None):
+    """flux[B, T] for params[B, 12] and times[T] (device tensors, fp64)."""
+    torch = _torch()
+    lib = load_library()
+    params, times = _dev_f64(params, GL_NPARAMS), _dev_f64(times)
+    code, td = _tdtype(dtype)
+    B, T = params.shape[0], times.shape[0]
+    if out is None:
+        out = torch.empty((B, T), dtype=td, device=params.device)
+    with torch.cuda.device(params.device):
+        _check(lib.gl_lightcurve(params.data_ptr(), B, times.data_ptr(), T, float(t_exp),
+                                 int(n_ss), out.data_ptr(), code, _stream(params)))
+    return out
+
+
+def gl_loglike(params, times, t_exp, n_ss, obs, sigma, dtype="f32", want_flux=False):
+    """chi2[B] (and flux[B, T] when want_flux) -- one fused launch."""
+    torch = _torch()
+    lib = load_library()
+    params, times = _dev_f64(params, GL_NPARAMS), _dev_f64(times)
+    obs, sigma = _dev_f64(obs), _dev_f64(sigma)
+    code, td = _tdtype(dtype)
+    B, T = params.shape[0], times.shape[0]
+    if obs.shape[0] != T or sigma.shape[0] != T:
+        raise GreenlanternError("obs and sigma must have the length of times")
+    chi2 = torch.empty((B,), dtype=td, device=params.device)
+    flux = torch.empty((B, T), dtype=td, device=params.device) if want_flux else None
+    with torch.cuda.device(params.device):
+        _check(lib.gl_loglike(params.data_ptr(), B, times.data_ptr(), T, float(t_exp), int(n_ss),
+                              obs.data_ptr(), sigma.data_ptr(), chi2.data_ptr(),
+                              flux.data_ptr() if want_flux else None, code, _stream(params)))
+    return (chi2, flux) if want_flux else chi2
+
+
+def gl_flux_geometry(geom, dtype="f32"):
+    """flux[N] for rows (d, Rp, f_proj, PA, u1, u2) (device tensor, fp64)."""
+    torch = _torch()
+    lib = load_library()
+    geom = _dev_f64(geom, GL_NGEOM)
+    code, td = _tdtype(dtype)
+    out = torch.empty((geom.shape[0],), dtype=td, device=geom.device)
+    with torch.cuda.device(geom.device):
+        _check(lib.gl_flux_geometry(geom.data_ptr(), geom.shape[0], out.data_ptr(), code,
+                                    _stream(geom)))
+    return out
+
+
+def _host_f64(x):
+    return np.ascontiguousarray(x, dtype=np.float64)
+
+
+def gl_loglike_host(params, times, t_exp, n_ss, obs, sigma, dtype="f32", want_flux=False):
+    """HOST numpy in, HOST numpy out; the library does the copies (end-to-end path)."""
+    lib = load_library()
+    params, times, obs, sigma = map(_host_f64, (np.atleast_2d(params), times, obs, sigma))
+    code = GL_F64 if dtype in (GL_F64, "f64", "float64") else GL_F32
+    nd = np.float64 if code == GL_F64 else np.float32
+    B, T = params.shape[0], times.shape[0]
+    chi2 = np.empty(B, dtype=nd)
+    flux = np.empty((B, T), dtype=nd) if want_flux else None
+    _check(lib.gl_loglike_host(params.ctypes.data, B, times.ctypes.data, T, float(t_exp),
+                               int(n_ss), obs.ctypes.data, sigma.ctypes.data, chi2.ctypes.data,
+                               flux.ctypes.data if want_flux else None, code))
+    return (chi2, flux) if want_flux else chi2
+
+
+def gl_lightcurve_host(params, times, t_exp=0.0, n_ss=1, dtype="f32"):
+    lib = load_library()
+    params, times = _host_f64(np.atleast_2d(params)), _host_f64(times)
+    code = GL_F64 if dtype in (GL_F64, "f64", "float64") else GL_F32
+    flux = np.empty((params.shape[0], times.shape[0]),
+                    dtype=np.float64 if code == GL_F64 else np.float32)
+    _check(lib.gl_lightcurve_host(params.ctypes.data, params.shape[0], times.ctypes.data,
+                                  times.shape[0], float(t_exp), int(n_ss), flux.ctypes.data, code))
+    return flux
+
+
+def gl_flux_geometry_host(geom, dtype="f32"):
+    lib = load_library()
+    geom = _host_f64(np.atleast_2d(geom))
+    code = GL_F64 if dtype in (GL_F64, "f64", "float64") else GL_F32
+    out = np.empty(geom.shape[0], dtype=np.float64 if code == GL_F64 else np.float32)
+    _check(lib.gl_flux_geometry_host(geom.ctypes.data, geom.shape[0], out.ctypes.data, code))
+    return out
+
+
+def gl_launch_count():
+    return int(load_library().gl_launch_count())
+
+
+def gl_version():
+    return int(load_library().gl_version())
+
+
+def gl_strerror(code):
+    return load_library().gl_strerror(int(code)).decode()

@@ -1,0 +1,677 @@
+// greenlantern_b200.cu -- kernels and C ABI of the B200 oblate-transit library (sm_100a).
+//
+// One fused kernel does the whole hot path of DESIGN.md section 1 for a batch of walkers:
+//   a0 per-walker prelude (fp64)            -> shared memory
+//   a1 Kepler + sky position per sub-sample  (phase in fp64, then the compute type)
+//   a2 projected-outline geometry            (in the prelude: constant over a transit)
+//   a3 outline/limb crossings, a4 boundary integrals   (gl_core.cuh)
+//   a5 exposure mean, residual^2, deterministic block + cluster reduction of chi^2
+// Work layout: one thread-block CLUSTER per walker (1..8 CTAs, DSMEM reduction, no atomics, no
+// scratch in HBM); each CTA classifies tiles of exposure times against the walker's transit
+// window, compacts the in-window ones into shared memory and spreads their (time, sub-exposure)
+// pairs over its threads, so the lanes of a warp all do in-transit work.
+#include <cooperative_groups.h>
+#include <cuda_runtime.h>
+#include <math.h>
+#include <stdint.h>
+#include <stdio.h>
+
+#include <mutex>
+
+#include "../../include/greenlantern_b200.h"
+#include "gl_core.cuh"
+#include "gl_tables.h"
+
+namespace cg = cooperative_groups;
+
+namespace {
+
+constexpr int NQ32 = 16;   // Gauss-Legendre points per outline arc, fp32 production path
+constexpr int NQ64 = 48;   // ... fp64 validation path
+constexpr int NT = 256;    // threads per CTA
+constexpr int TILE = 1024; // exposure times classified per tile
+constexpr int MAXCLUSTER = 8;
+
+__constant__ float c_phi32[NQ32 / 2], c_om32[NQ32 / 2];
+__constant__ double c_phi64[NQ64 / 2], c_om64[NQ64 / 2];
+
+template <typename T> struct Quad;
+template <> struct Quad<float> {
+    static constexpr int N = NQ32;
+    static __device__ __forceinline__ const float* phi() { return c_phi32; }
+    static __device__ __forceinline__ const float* om() { return c_om32; }
+};
+template <> struct Quad<double> {
+    static constexpr int N = NQ64;
+    static __device__ __forceinline__ const double* phi() { return c_phi64; }
+    static __device__ __forceinline__ const double* om() { return c_om64; }
+};
+
+constexpr double kPi = 3.14159265358979323846;
+constexpr double kTwoPi = 6.28318530717958647692;
+
+// ------------------------------------------------------------------------------------------
+// a0 + a2: everything that is constant for one walker.
+// ------------------------------------------------------------------------------------------
+struct Walker {
+    // orbit (fp64: phases and Kepler's equation are always double)
+    double t0, inv_P, aR, e, omega, cosi, Mc, sq1pe, sq1me, half_win_phase, vmax;
+    // projected outline: semi-axes and the rotation into the kernel frame
+    double a, b, cpsi, spsi;
+    // limb darkening, already divided by the disc-integrated intensity
+    double k0, k1, k2;
+    int valid;
+};
+
+// Semi-axes (a >= b) and major-axis angle psi of the sky-projected outline of an ellipsoid with
+// semi-axes (sa, sb, sc) along x', y', z' rotated by R = Rx(zeta) Ry(eta) Rz(xi)
+// (eqs. 3-6).  The outline x = dx cos th, y = dy1 cos th + dy2 sin th of
+// PAPER.md:89-96 (eqs. 11-13) is the image of the unit circle under the lower-Cholesky factor of
+//   C = [[Cxx, Cxy], [Cxy, Cyy]],  Cxx = dx^2 = sa^2 r1^2 + sb^2 r4^2 + sc^2 r7^2   (eq. 11)
+//   Cxy = dx dy1 = sa^2 r1 r2 + sb^2 r4 r5 + sc^2 r7 r8                               (eq. 12)
+//   det C = (dx dy2)^2 = sa^2 sb^2 r9^2 + sa^2 sc^2 r6^2 + sb^2 sc^2 r3^2             (eq. 13)
+// so its principal axes are the eigenvectors of C: a^2 = larger eigenvalue, b = sqrt(det C)/a.
+__device__ void outline_axes(double sa, double sb, double sc, double zeta, double eta, double xi,
+                             double* a, double* b, double* cpsi, double* spsi) {
+    double sz, cz, se, ce, sx, cx;
+    sincos(zeta, &sz, &cz);
+    sincos(eta, &se, &ce);
+    sincos(xi, &sx, &cx);
+    // rows of Rx(zeta) Ry(eta) Rz(xi)
+    const double r1 = ce * cx, r2 = -ce * sx, r3 = se;
+    const double r4 = cz * sx + sz * se * cx, r5 = cz * cx - sz * se * sx, r6 = -sz * ce;
+    const double r7 = sz * sx - cz * se * cx, r8 = sz * cx + cz * se * sx, r9 = cz * ce;
+    const double A2 = sa * sa, B2 = sb * sb, C2 = sc * sc;
+    const double Cxx = A2 * r1 * r1 + B2 * r4 * r4 + C2 * r7 * r7;
+    const double Cxy = A2 * r1 * r2 + B2 * r4 * r5 + C2 * r7 * r8;
+    const double Cyy = A2 * r2 * r2 + B2 * r5 * r5 + C2 * r8 * r8;
+    const double det = A2 * B2 * r9 * r9 + A2 * C2 * r6 * r6 + B2 * C2 * r3 * r3;
+    const double hd = 0.5 * (Cxx - Cyy);
+    const double rad = sqrt(hd * hd + Cxy * Cxy);
+    const double lam = 0.5 * (Cxx + Cyy) + rad;
+    *a = sqrt(lam);
+    *b = sqrt(det) / *a;
+    double psi = (rad > 0.0) ? 0.5 * atan2(Cxy, hd) : 0.0;
+    sincos(psi, spsi, cpsi);
+}
+
+__device__ void walker_prelude(const double* __restrict__ p, double t_exp, Walker* w) {
+    const double t0 = p[0], P = p[1], aR = p[2], b = p[3], e = p[4], om = p[5];
+    const double Rp = p[6], f = p[7], xi = p[8], eta = p[9], u1 = p[10], u2 = p[11];
+    bool ok = true;
+    for (int k = 0; k < GL_NPARAMS; ++k) ok = ok && isfinite(p[k]);
+    const double norm = 1.0 - u1 / 3.0 - u2 / 6.0;
+    ok = ok && (P > 0.0) && (e >= 0.0) && (e < 1.0) && (Rp > 0.0) && (Rp < 0.5) && (f >= 0.0) &&
+         (f < 1.0) && (aR * (1.0 - e) > 1.0) && (norm > 0.0) &&
+         (fabs(b) * (1.0 + e * sin(om)) <= aR * (1.0 - e * e));
+    w->valid = ok ? 1 : 0;
+    if (!ok) return;
+    w->t0 = t0;
+    w->inv_P = 1.0 / P;
+    w->aR = aR;
+    w->e = e;
+    w->omega = om;
+    // R7: conjunction at true anomaly pi/2 - omega; cos i from the impact parameter
+    const double nuc = 0.5 * kPi - om;
+    const double s1 = sqrt(1.0 + e), s2 = sqrt(1.0 - e);
+    const double Ec = 2.0 * atan2(s2 * sin(0.5 * nuc), s1 * cos(0.5 * nuc));
+    w->Mc = Ec - e * sin(Ec);
+    w->sq1pe = s1;
+    w->sq1me = s2;
+    w->cosi = (b / aR) * (1.0 + e * sin(om)) / (1.0 - e * e);
+    // oblate spheroid: polar semi-axis Rp (1-f) along x', equatorial Rp; zeta = 0 (R4, R5)
+    outline_axes(Rp * (1.0 - f), Rp, Rp, 0.0, eta, xi, &w->a, &w->b, &w->cpsi, &w->spsi);
+    const double pn = kPi * norm;
+    w->k0 = (1.0 - u1 - 2.0 * u2) / pn;
+    w->k1 = (u1 + 2.0 * u2) / pn;
+    w->k2 = u2 / pn;
+    // transit window.  e = 0: the centre is within 1 + a of the star centre iff
+    //   sin^2(phi) < [((1+a)/aR)^2 - cos^2 i] / sin^2 i  and cos(phi) > 0;
+    // stored as a half-width in orbital phase, widened by half an exposure.
+    const double reach = (1.0 + w->a) * (1.0 + 1e-12);
+    double hw = -1.0;   // < 0: never in transit
+    if (e == 0.0) {
+        const double ci2 = w->cosi * w->cosi;
+        const double S2 = ((reach / aR) * (reach / aR) - ci2) / (1.0 - ci2);
+        if (S2 > 0.0) hw = (S2 >= 1.0) ? 0.25 : asin(sqrt(S2)) / kTwoPi;
+        if (hw >= 0.0) hw += 0.5 * t_exp * w->inv_P + 1e-13;
+    }
+    w->half_win_phase = hw;
+    // largest sky-plane speed (periastron), in stellar radii per time unit: bounds how far the
+    // centre moves within half an exposure (window test of eccentric orbits)
+    w->vmax = kTwoPi * w->inv_P * aR * s1 / s2;
+}
+
+// ------------------------------------------------------------------------------------------
+// a1: sky-plane position of the planet centre at time t, in the kernel frame.
+//   e = 0: eqs. 9-10 with alpha = 2 pi (t - t0)/P, d = a/R*, sin(beta) = cos i.
+//   e > 0: Kepler's equation in fp64 (R7).  Returns false when the planet is behind the star.
+// The orbital phase is always formed and reduced in fp64.
+// ------------------------------------------------------------------------------------------
+__device__ __forceinline__ double reduced_phase(const Walker& w, double t) {
+    const double ph = (t - w.t0) * w.inv_P;
+    return ph - rint(ph);
+}
+
+__device__ double kepler_E(double M, double e) {
+    // Newton from E = M + e sin M, safeguarded by the bracket [M - e, M + e]
+    double lo = M - e, hi = M + e;
+    double E = fmin(fmax(M + e * sin(M), lo), hi);
+    for (int it = 0; it < 64; ++it) {
+        double s, c;
+        sincos(E, &s, &c);
+        const double f = E - e * s - M;
+        if (f > 0.0) hi = E; else lo = E;
+        double En = E - f / (1.0 - e * c);
+        if (!(En > lo && En < hi)) En = 0.5 * (lo + hi);
+        const double d = En - E;
+        E = En;
+        if (fabs(d) <= 2e-16 * fmax(1.0, fabs(E))) break;
+    }
+    return E;
+}
+
+// fp64 position in the SKY frame (x0 along the projected orbit normal, y0 along the chord).
+__device__ bool sky_position_f64(const Walker& w, double ph, double* x0, double* y0) {
+    if (w.e == 0.0) {
+        double s, c;
+        sincospi(2.0 * ph, &s, &c);
+        *x0 = w.aR * c * w.cosi;
+        *y0 = w.aR * s;
+        return c > 0.0;
+    }
+    const double M = w.Mc + kTwoPi * ph;
+    const double E = kepler_E(M, w.e);
+    double sh, ch, sE, cE;
+    sincos(0.5 * E, &sh, &ch);
+    sincos(E, &sE, &cE);
+    const double nu = 2.0 * atan2(w.sq1pe * sh, w.sq1me * ch);
+    const double r = w.aR * (1.0 - w.e * cE);
+    double sp, cp;
+    sincos(nu + w.omega - 0.5 * kPi, &sp, &cp);
+    *x0 = r * cp * w.cosi;
+    *y0 = r * sp;
+    return cp > 0.0;
+}
+
+// Per-walker constants narrowed to the compute type once per thread.
+template <typename T> struct WalkerT {
+    T aR, cosi, a, b, cpsi, spsi, k0, k1, k2;
+    bool circular;
+};
+template <typename T> __device__ __forceinline__ WalkerT<T> narrow(const Walker& w) {
+    WalkerT<T> v;
+    v.aR = T(w.aR);
+    v.cosi = T(w.cosi);
+    v.a = T(w.a);
+    v.b = T(w.b);
+    v.cpsi = T(w.cpsi);
+    v.spsi = T(w.spsi);
+    v.k0 = T(w.k0);
+    v.k1 = T(w.k1);
+    v.k2 = T(w.k2);
+    v.circular = (w.e == 0.0);
+    return v;
+}
+
+// Blocked fraction delta = 1 - F_inst at reduced phase ph (a1 + a3 + a4).
+template <typename T>
+__device__ __forceinline__ T blocked_fraction(const Walker& w, const WalkerT<T>& v, double ph) {
+    T x0, y0;
+    if (v.circular) {
+        // phi = 2 pi ph, |ph| <= 1/2; narrowed AFTER the fp64 phase reduction
+        T s, c;
+        glc::gsincos(T(kTwoPi * ph), &s, &c);
+        if (!(c > T(0))) return T(0);
+        x0 = v.aR * c * v.cosi;
+        y0 = v.aR * s;
+    } else {
+        double X, Y;
+        if (!sky_position_f64(w, ph, &X, &Y)) return T(0);
+        x0 = T(X);
+        y0 = T(Y);
+    }
+    const T xc = v.cpsi * x0 + v.spsi * y0, yc = v.cpsi * y0 - v.spsi * x0;
+    T A[3];
+    if (!glc::overlap_areas<T, Quad<T>::N>(xc, yc, v.a, v.b, Quad<T>::phi(), Quad<T>::om(), A))
+        return T(0);
+    return v.k0 * A[0] + v.k1 * A[1] + v.k2 * A[2];
+}
+
+// ------------------------------------------------------------------------------------------
+// Deterministic sum of one double per thread over the CTA (fixed shuffle tree, fixed warp order).
+// ------------------------------------------------------------------------------------------
+__device__ __forceinline__ double block_sum(double v, double* warp_scratch) {
+#pragma unroll
+    for (int off = 16; off > 0; off >>= 1) v += __shfl_down_sync(0xffffffffu, v, off);
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    __syncthreads();
+    if (lane == 0) warp_scratch[warp] = v;
+    __syncthreads();
+    double tot = 0.0;
+    if (threadIdx.x == 0)
+        for (int k = 0; k < NT / 32; ++k) tot += warp_scratch[k];
+    return tot;   // valid in thread 0
+}
+
+// ------------------------------------------------------------------------------------------
+// The fused kernel.  grid = (cluster size C, walkers in flight); cluster = (C, 1, 1).
+//   flux  : [B, T] of T-typed values or nullptr          chi2 : [B] or nullptr
+//   obs, sigma : [T] fp64 or nullptr (only read when chi2 != nullptr)
+// ------------------------------------------------------------------------------------------
+template <typename T>
+__global__ void __launch_bounds__(NT)
+transit_kernel(const double* __restrict__ params, int B, const double* __restrict__ times, int nT,
+               double t_exp, int n_ss, const double* __restrict__ obs,
+               const double* __restrict__ sigma, T* __restrict__ flux, T* __restrict__ chi2) {
+    cg::cluster_group cluster = cg::this_cluster();
+    const int crank = (int)cluster.block_rank(), csize = (int)cluster.num_blocks();
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+
+    __shared__ Walker sw;
+    __shared__ int s_list[TILE];
+    __shared__ T s_buf[NT];
+    __shared__ int s_wcount[NT / 32];
+    __shared__ int s_nlist;
+    __shared__ double s_red[NT / 32];
+    __shared__ double s_partial;   // this CTA's chi^2 partial, read by cluster rank 0 via DSMEM
+
+    const double inv_ss = 1.0 / (double)n_ss;
+    const int ntiles = (nT + TILE - 1) / TILE;
+    const bool want_chi2 = (chi2 != nullptr);
+
+    for (int wk = blockIdx.y; wk < B; wk += gridDim.y) {
+        __syncthreads();
+        if (tid == 0) walker_prelude(params + (size_t)wk * GL_NPARAMS, t_exp, &sw);
+        __syncthreads();
+        const bool valid = sw.valid != 0;
+        double acc = 0.0;   // this thread's chi^2 terms
+        T* frow = flux ? flux + (size_t)wk * nT : nullptr;
+
+        if (!valid) {
+            if (frow)
+                for (int i = crank * NT + tid; i < nT; i += csize * NT) frow[i] = T(NAN);
+            acc = (double)INFINITY;
+        } else {
+            const WalkerT<T> v = narrow<T>(sw);
+            const bool circ = v.circular;
+            const double hwin = sw.half_win_phase;
+            const double reach = (1.0 + sw.a) * (1.0 + 1e-12) + 0.5 * t_exp * sw.vmax;
+            for (int tile = crank; tile < ntiles; tile += csize) {
+                const int i0 = tile * TILE;
+                if (tid == 0) s_nlist = 0;
+                __syncthreads();
+                // ---- classify TILE exposure times, compact the in-window ones (stable order)
+                for (int r = 0; r < TILE / NT; ++r) {
+                    const int i = i0 + r * NT + tid;
+                    bool inwin = false;
+                    if (i < nT) {
+                        const double ph = reduced_phase(sw, times[i]);
+                        if (circ) {
+                            inwin = fabs(ph) < hwin;
+                        } else {
+                            double X, Y;
+                            sky_position_f64(sw, ph, &X, &Y);
+                            inwin = X * X + Y * Y < reach * reach;
+                        }
+                        if (!inwin) {
+                            if (frow) frow[i] = T(1);
+                            if (want_chi2) {
+                                const double sg = sigma[i];
+                                const double rr = (obs[i] - 1.0) / sg;
+                                acc += (sg > 0.0 && isfinite(sg)) ? rr * rr : (double)INFINITY;
+                            }
+                        }
+                    }
+                    const unsigned bal = __ballot_sync(0xffffffffu, inwin);
+                    if (lane == 0) s_wcount[warp] = __popc(bal);
+                    __syncthreads();
+                    int base = s_nlist;
+                    for (int k = 0; k < warp; ++k) base += s_wcount[k];
+                    if (inwin) s_list[base + __popc(bal & ((1u << lane) - 1u))] = i;
+                    __syncthreads();
+                    if (tid == 0) {
+                        int tot = s_nlist;
+                        for (int k = 0; k < NT / 32; ++k) tot += s_wcount[k];
+                        s_nlist = tot;
+                    }
+                    __syncthreads();
+                }
+                const int nlist = s_nlist;
+                // ---- evaluate the (time, sub-exposure) pairs of the in-window list
+                if (n_ss <= NT) {
+                    const int per = NT / n_ss;   // exposure times per batch
+                    for (int l0 = 0; l0 < nlist; l0 += per) {
+                        const int nl = min(per, nlist - l0);
+                        if (tid < nl * n_ss) {
+                            const int l = tid / n_ss, j = tid - l * n_ss;
+                            const double t = times[s_list[l0 + l]] +
+                                             (((double)j + 0.5) * inv_ss - 0.5) * t_exp;
+                            s_buf[tid] = blocked_fraction<T>(sw, v, reduced_phase(sw, t));
+                        }
+                        __syncthreads();
+                        if (tid < nl) {
+                            T sum = T(0);
+                            for (int j = 0; j < n_ss; ++j) sum += s_buf[tid * n_ss + j];
+                            const T dbar = sum * T(inv_ss);
+                            const int i = s_list[l0 + tid];
+                            if (frow) frow[i] = T(1) - dbar;
+                            if (want_chi2) {
+                                const double sg = sigma[i];
+                                const double rr = ((obs[i] - 1.0) + (double)dbar) / sg;
+                                acc += (sg > 0.0 && isfinite(sg)) ? rr * rr : (double)INFINITY;
+                            }
+                        }
+                        __syncthreads();
+                    }
+                } else {
+                    // more sub-exposures than threads: one exposure time per thread, serial in j
+                    for (int l = tid; l < nlist; l += NT) {
+                        const int i = s_list[l];
+                        T sum = T(0);
+                        for (int j = 0; j < n_ss; ++j) {
+                            const double t = times[i] + (((double)j + 0.5) * inv_ss - 0.5) * t_exp;
+                            sum += blocked_fraction<T>(sw, v, reduced_phase(sw, t));
+                        }
+                        const T dbar = sum * T(inv_ss);
+                        if (frow) frow[i] = T(1) - dbar;
+                        if (want_chi2) {
+                            const double sg = sigma[i];
+                            const double rr = ((obs[i] - 1.0) + (double)dbar) / sg;
+                            acc += (sg > 0.0 && isfinite(sg)) ? rr * rr : (double)INFINITY;
+                        }
+                    }
+                }
+                __syncthreads();
+            }
+        }
+        // ---- chi^2: CTA sum, then cluster rank 0 adds the partials in rank order over DSMEM
+        if (want_chi2) {
+            const double tot = block_sum(acc, s_red);
+            if (tid == 0) s_partial = tot;
+            cluster.sync();
+            if (crank == 0 && tid == 0) {
+                double c2 = 0.0;
+                for (int r = 0; r < csize; ++r) c2 += *cluster.map_shared_rank(&s_partial, r);
+                chi2[wk] = valid ? T(c2) : T(INFINITY);
+            }
+            cluster.sync();   // keep every CTA's shared memory alive until rank 0 has read it
+        }
+    }
+}
+
+// ------------------------------------------------------------------------------------------
+// Steps a3 + a4 alone, one bare geometry per thread (config 5 of BASELINE.json).
+// row = (d, Rp, f_proj, PA, u1, u2): planet centre at (d, 0), major axis at angle PA from +x, so
+// in the kernel frame the centre is (d cos PA, -d sin PA).
+// ------------------------------------------------------------------------------------------
+template <typename T>
+__global__ void __launch_bounds__(NT)
+geometry_kernel(const double* __restrict__ geom, long long N, T* __restrict__ out) {
+    const long long k = (long long)blockIdx.x * NT + threadIdx.x;
+    if (k >= N) return;
+    const double* g = geom + k * GL_NGEOM;
+    const double d = g[0], Rp = g[1], fp = g[2], pa = g[3], u1 = g[4], u2 = g[5];
+    const double norm = 1.0 - u1 / 3.0 - u2 / 6.0;
+    bool ok = isfinite(d) && isfinite(Rp) && isfinite(fp) && isfinite(pa) && isfinite(u1) &&
+              isfinite(u2) && (d >= 0.0) && (Rp > 0.0) && (Rp < 0.5) && (fp >= 0.0) && (fp < 1.0) &&
+              (norm > 0.0);
+    if (!ok) {
+        out[k] = T(NAN);
+        return;
+    }
+    T s, c;
+    glc::gsincos(T(pa), &s, &c);
+    const T a = T(Rp), b = T(Rp * (1.0 - fp));
+    T A[3];
+    T delta = T(0);
+    if (glc::overlap_areas<T, Quad<T>::N>(T(d) * c, -T(d) * s, a, b, Quad<T>::phi(), Quad<T>::om(),
+                                          A)) {
+        const double pn = kPi * norm;
+        delta = T((1.0 - u1 - 2.0 * u2) / pn) * A[0] + T((u1 + 2.0 * u2) / pn) * A[1] +
+                T(u2 / pn) * A[2];
+    }
+    out[k] = T(1) - delta;
+}
+
+}  // namespace
+
+// ==========================================================================================
+// Host side: table upload, launch configuration, C ABI.
+// ==========================================================================================
+namespace {
+
+thread_local long long tl_launches = 0;
+thread_local char tl_cuda_err[256] = "";
+
+int cuda_fail(cudaError_t e, const char* where) {
+    snprintf(tl_cuda_err, sizeof(tl_cuda_err), "%s: %s", where, cudaGetErrorString(e));
+    return GL_ECUDA;
+}
+
+// Quadrature tables go to constant memory once per device (immutable afterwards).
+int ensure_tables() {
+    static std::mutex mu;
+    static unsigned long long done_mask = 0;   // devices 0..63
+    int dev = 0;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) return cuda_fail(e, "cudaGetDevice");
+    std::lock_guard<std::mutex> lock(mu);
+    if (dev < 64 && (done_mask >> dev) & 1ull) return GL_OK;
+    float p32[NQ32 / 2], o32[NQ32 / 2];
+    double p64[NQ64 / 2], o64[NQ64 / 2];
+    glt::smoothed_gauss_legendre<float>(NQ32, p32, o32);
+    glt::smoothed_gauss_legendre<double>(NQ64, p64, o64);
+    if ((e = cudaMemcpyToSymbol(c_phi32, p32, sizeof(p32))) != cudaSuccess ||
+        (e = cudaMemcpyToSymbol(c_om32, o32, sizeof(o32))) != cudaSuccess ||
+        (e = cudaMemcpyToSymbol(c_phi64, p64, sizeof(p64))) != cudaSuccess ||
+        (e = cudaMemcpyToSymbol(c_om64, o64, sizeof(o64))) != cudaSuccess)
+        return cuda_fail(e, "cudaMemcpyToSymbol");
+    if (dev < 64) done_mask |= 1ull << dev;
+    return GL_OK;
+}
+
+// Cluster size: enough CTAs per walker that the batch fills the GPU, at most one tile each.
+int pick_cluster(int B, int nT) {
+    const int ntiles = (nT + TILE - 1) / TILE;
+    int c = 1;
+    while (c < MAXCLUSTER && c * 2 <= ntiles && (long long)B * c < 4LL * 148) c *= 2;
+    return c;
+}
+
+template <typename T>
+int launch_transit(const double* params, int B, const double* times, int nT, double t_exp, int n_ss,
+                   const double* obs, const double* sigma, void* flux, void* chi2,
+                   cudaStream_t st) {
+    const int C = pick_cluster(B, nT);
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = dim3((unsigned)C, (unsigned)(B < 65535 ? B : 65535), 1);
+    cfg.blockDim = dim3(NT, 1, 1);
+    cfg.dynamicSmemBytes = 0;
+    cfg.stream = st;
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeClusterDimension;
+    attr[0].val.clusterDim.x = (unsigned)C;
+    attr[0].val.clusterDim.y = 1;
+    attr[0].val.clusterDim.z = 1;
+    cfg.attrs = attr;
+    cfg.numAttrs = 1;
+    cudaError_t e = cudaLaunchKernelEx(&cfg, transit_kernel<T>, params, B, times, nT, t_exp, n_ss,
+                                       obs, sigma, (T*)flux, (T*)chi2);
+    if (e != cudaSuccess) return cuda_fail(e, "transit_kernel launch");
+    ++tl_launches;
+    return GL_OK;
+}
+
+int run_transit(const double* params, int B, const double* times, int nT, double t_exp, int n_ss,
+                const double* obs, const double* sigma, void* flux, void* chi2, gl_dtype dtype,
+                void* stream, bool need_flux, bool need_chi2) {
+    if (B < 0 || nT < 0 || n_ss < 1 || !(t_exp >= 0.0) || !isfinite(t_exp)) return GL_EINVAL;
+    if (dtype != GL_F32 && dtype != GL_F64) return GL_EINVAL;
+    if (B == 0) return GL_OK;
+    if (nT == 0 && !need_chi2) return GL_OK;
+    if (!params || (nT > 0 && !times)) return GL_EINVAL;
+    if (need_flux && nT > 0 && !flux) return GL_EINVAL;
+    if (need_chi2 && (!chi2 || (nT > 0 && (!obs || !sigma)))) return GL_EINVAL;
+    if ((long long)B * (long long)nT >= (1LL << 40)) return GL_EUNSUPPORTED;
+    int rc = ensure_tables();
+    if (rc != GL_OK) return rc;
+    cudaStream_t st = (cudaStream_t)stream;
+    return dtype == GL_F32
+               ? launch_transit<float>(params, B, times, nT, t_exp, n_ss, obs, sigma, flux, chi2, st)
+               : launch_transit<double>(params, B, times, nT, t_exp, n_ss, obs, sigma, flux, chi2,
+                                        st);
+}
+
+}  // namespace
+
+extern "C" {
+
+int gl_lightcurve(const double* params, int B, const double* times, int T, double t_exp, int n_ss,
+                  void* flux_out, gl_dtype dtype, void* stream) {
+    return run_transit(params, B, times, T, t_exp, n_ss, nullptr, nullptr, flux_out, nullptr, dtype,
+                       stream, true, false);
+}
+
+int gl_loglike(const double* params, int B, const double* times, int T, double t_exp, int n_ss,
+               const double* obs, const double* sigma, void* chi2_out, void* flux_out_or_null,
+               gl_dtype dtype, void* stream) {
+    return run_transit(params, B, times, T, t_exp, n_ss, obs, sigma, flux_out_or_null, chi2_out,
+                       dtype, stream, false, true);
+}
+
+int gl_flux_geometry(const double* geom, long long N, void* flux_out, gl_dtype dtype,
+                     void* stream) {
+    if (N < 0 || (dtype != GL_F32 && dtype != GL_F64)) return GL_EINVAL;
+    if (N == 0) return GL_OK;
+    if (!geom || !flux_out) return GL_EINVAL;
+    if (N >= (1LL << 40)) return GL_EUNSUPPORTED;
+    int rc = ensure_tables();
+    if (rc != GL_OK) return rc;
+    const unsigned blocks = (unsigned)((N + NT - 1) / NT);
+    cudaStream_t st = (cudaStream_t)stream;
+    if (dtype == GL_F32)
+        geometry_kernel<float><<<blocks, NT, 0, st>>>(geom, N, (float*)flux_out);
+    else
+        geometry_kernel<double><<<blocks, NT, 0, st>>>(geom, N, (double*)flux_out);
+    cudaError_t e = cudaGetLastError();
+    if (e != cudaSuccess) return cuda_fail(e, "geometry_kernel launch");
+    ++tl_launches;
+    return GL_OK;
+}
+
+long long gl_launch_count(void) { return tl_launches; }
+const char* gl_last_cuda_error(void) { return tl_cuda_err; }
+int gl_version(void) { return 100; }
+
+const char* gl_strerror(int code) {
+    switch (code) {
+        case GL_OK: return "ok";
+        case GL_EINVAL: return "invalid argument";
+        case GL_ECUDA: return "CUDA error (see gl_last_cuda_error)";
+        case GL_EUNSUPPORTED: return "size not supported";
+        default: return "unknown status";
+    }
+}
+
+}  // extern "C"
+
+// ------------------------------------------------------------------------------------------
+// HOST-buffer wrappers: stream-ordered scratch from the device's default memory pool, copies in,
+// the kernel above, copies out, one synchronise.
+// ------------------------------------------------------------------------------------------
+namespace {
+
+struct HostCall {
+    cudaStream_t st = nullptr;
+    void* bufs[8];
+    int nbufs = 0;
+    cudaError_t err = cudaSuccess;
+    HostCall() { err = cudaStreamCreateWithFlags(&st, cudaStreamNonBlocking); }
+    void* alloc(size_t bytes) {
+        void* p = nullptr;
+        if (err != cudaSuccess) return nullptr;
+        err = cudaMallocAsync(&p, bytes ? bytes : 1, st);
+        if (err == cudaSuccess) bufs[nbufs++] = p;
+        return p;
+    }
+    void* upload(const void* host, size_t bytes) {
+        void* p = alloc(bytes);
+        if (p && bytes) err = cudaMemcpyAsync(p, host, bytes, cudaMemcpyHostToDevice, st);
+        return p;
+    }
+    void download(void* host, const void* dev, size_t bytes) {
+        if (err == cudaSuccess && bytes)
+            err = cudaMemcpyAsync(host, dev, bytes, cudaMemcpyDeviceToHost, st);
+    }
+    int finish(int rc) {
+        for (int i = 0; i < nbufs; ++i) cudaFreeAsync(bufs[i], st);
+        cudaError_t e2 = st ? cudaStreamSynchronize(st) : cudaSuccess;
+        if (st) cudaStreamDestroy(st);
+        if (rc != GL_OK) return rc;
+        if (err != cudaSuccess) return cuda_fail(err, "host wrapper");
+        if (e2 != cudaSuccess) return cuda_fail(e2, "host wrapper sync");
+        return GL_OK;
+    }
+};
+
+size_t elem(gl_dtype d) { return d == GL_F64 ? 8 : 4; }
+
+}  // namespace
+
+extern "C" {
+
+int gl_loglike_host(const double* params, int B, const double* times, int T, double t_exp, int n_ss,
+                    const double* obs, const double* sigma, void* chi2_out, void* flux_out_or_null,
+                    gl_dtype dtype) {
+    if (B < 0 || T < 0 || (dtype != GL_F32 && dtype != GL_F64)) return GL_EINVAL;
+    if (B == 0) return GL_OK;
+    if (!params || !chi2_out || (T > 0 && (!times || !obs || !sigma))) return GL_EINVAL;
+    HostCall h;
+    void* dp = h.upload(params, sizeof(double) * GL_NPARAMS * (size_t)B);
+    void* dt = h.upload(times, sizeof(double) * (size_t)T);
+    void* dob = h.upload(obs, sizeof(double) * (size_t)T);
+    void* dsg = h.upload(sigma, sizeof(double) * (size_t)T);
+    void* dc = h.alloc(elem(dtype) * (size_t)B);
+    void* df = flux_out_or_null ? h.alloc(elem(dtype) * (size_t)B * (size_t)T) : nullptr;
+    int rc = GL_OK;
+    if (h.err == cudaSuccess)
+        rc = gl_loglike((const double*)dp, B, (const double*)dt, T, t_exp, n_ss, (const double*)dob,
+                        (const double*)dsg, dc, df, dtype, h.st);
+    if (rc == GL_OK) {
+        h.download(chi2_out, dc, elem(dtype) * (size_t)B);
+        if (df) h.download(flux_out_or_null, df, elem(dtype) * (size_t)B * (size_t)T);
+    }
+    return h.finish(rc);
+}
+
+int gl_lightcurve_host(const double* params, int B, const double* times, int T, double t_exp,
+                       int n_ss, void* flux_out, gl_dtype dtype) {
+    if (B < 0 || T < 0 || (dtype != GL_F32 && dtype != GL_F64)) return GL_EINVAL;
+    if (B == 0 || T == 0) return GL_OK;
+    if (!params || !times || !flux_out) return GL_EINVAL;
+    HostCall h;
+    void* dp = h.upload(params, sizeof(double) * GL_NPARAMS * (size_t)B);
+    void* dt = h.upload(times, sizeof(double) * (size_t)T);
+    void* df = h.alloc(elem(dtype) * (size_t)B * (size_t)T);
+    int rc = GL_OK;
+    if (h.err == cudaSuccess)
+        rc = gl_lightcurve((const double*)dp, B, (const double*)dt, T, t_exp, n_ss, df, dtype, h.st);
+    if (rc == GL_OK) h.download(flux_out, df, elem(dtype) * (size_t)B * (size_t)T);
+    return h.finish(rc);
+}
+
+int gl_flux_geometry_host(const double* geom, long long N, void* flux_out, gl_dtype dtype) {
+    if (N < 0 || (dtype != GL_F32 && dtype != GL_F64)) return GL_EINVAL;
+    if (N == 0) return GL_OK;
+    if (!geom || !flux_out) return GL_EINVAL;
+    HostCall h;
+    void* dg = h.upload(geom, sizeof(double) * GL_NGEOM * (size_t)N);
+    void* df = h.alloc(elem(dtype) * (size_t)N);
+    int rc = GL_OK;
+    if (h.err == cudaSuccess) rc = gl_flux_geometry((const double*)dg, N, df, dtype, h.st);
+    if (rc == GL_OK) h.download(flux_out, df, elem(dtype) * (size_t)N);
+    return h.finish(rc);
+}
+
+}  // extern "C"

@@ -1,0 +1,179 @@
+"""GPU parity: the CUDA path (through the C ABI) against the CPU oracle, element by element.
+
+Tolerances are BASELINE.json's north_star: |dflux| <= 5e-7 (fp32), <= 1e-11 (fp64); chi^2 within
+1e-4 relative (fp32).  fp64 chi^2: 1e-9 relative (sum of ~1e4 terms each good to ~1e-11/sigma).
+"""
+import numpy as np
+import pytest
+
+import oracle as orc
+from paper_2410_05408_b200 import workloads as wl
+
+pytestmark = pytest.mark.gpu
+
+FTOL = {"f32": 5e-7, "f64": 1e-11}
+CTOL = {"f32": 1e-4, "f64": 1e-9}
+
+
+@pytest.fixture(scope="module")
+def gl():
+    import torch
+    assert torch.cuda.is_available()
+    import paper_2410_05408_b200 as g
+    g.load_library()
+    return g
+
+
+def dev(x):
+    import torch
+    return torch.as_tensor(np.ascontiguousarray(x, dtype=np.float64), device="cuda:0")
+
+
+def host(t):
+    return t.double().cpu().numpy()
+
+
+@pytest.mark.parametrize("dtype", ["f32", "f64"])
+def test_config1_single_uniform(gl, dtype):
+    w = wl.config1()
+    ref = orc.lightcurve(w.params, w.times, w.t_exp, w.n_ss)
+    out = host(gl.gl_lightcurve(dev(w.params), dev(w.times), w.t_exp, w.n_ss, dtype=dtype))
+    assert out.shape == ref.shape
+    assert np.abs(out - ref).max() <= FTOL[dtype]
+    assert np.all(out[ref == 1.0] == 1.0)          # out of transit is exactly 1
+    # mid-transit depth: SURVEY.md 8(c) pin P2
+    assert abs((1.0 - out.min()) - 0.007413896863355) <= FTOL[dtype]
+
+
+@pytest.mark.parametrize("dtype", ["f32", "f64"])
+def test_config2_k2_single(gl, dtype):
+    w = wl.config2()
+    chi_ref, ref = orc.loglike(w.params, w.times, w.t_exp, w.n_ss, w.obs, w.sigma)
+    chi, out = gl.gl_loglike(dev(w.params), dev(w.times), w.t_exp, w.n_ss, dev(w.obs),
+                             dev(w.sigma), dtype=dtype, want_flux=True)
+    assert np.abs(host(out) - ref).max() <= FTOL[dtype]
+    assert np.abs(host(chi) / chi_ref - 1.0).max() <= CTOL[dtype]
+    # chi^2-only mode (flux never leaves registers) gives the identical number
+    chi_only = gl.gl_loglike(dev(w.params), dev(w.times), w.t_exp, w.n_ss, dev(w.obs),
+                             dev(w.sigma), dtype=dtype)
+    assert np.array_equal(host(chi_only), host(chi))
+    # gl_lightcurve agrees with gl_loglike's flux bit for bit
+    lc = gl.gl_lightcurve(dev(w.params), dev(w.times), w.t_exp, w.n_ss, dtype=dtype)
+    assert np.array_equal(host(lc), host(out))
+
+
+@pytest.mark.parametrize("dtype", ["f32", "f64"])
+def test_config3_mcmc_batch_full(gl, dtype):
+    """Full size of the headline workload (B=256, T=3900, S=15): the oracle does it in seconds."""
+    w = wl.config3()
+    chi_ref, ref = orc.loglike(w.params, w.times, w.t_exp, w.n_ss, w.obs, w.sigma)
+    chi, out = gl.gl_loglike(dev(w.params), dev(w.times), w.t_exp, w.n_ss, dev(w.obs),
+                             dev(w.sigma), dtype=dtype, want_flux=True)
+    err = np.abs(host(out) - ref)
+    assert err.max() <= FTOL[dtype], (err.max(), np.unravel_index(err.argmax(), err.shape))
+    assert np.abs(host(chi) / chi_ref - 1.0).max() <= CTOL[dtype]
+
+
+@pytest.mark.parametrize("dtype", ["f32", "f64"])
+def test_config4_jwst_sampled(gl, dtype):
+    """Full-size launch (B=128, T=20000, S=3); the oracle checks 8 whole walkers (chi^2 needs full
+    rows) plus 64 times of every other walker."""
+    w = wl.config4()
+    chi, out = gl.gl_loglike(dev(w.params), dev(w.times), w.t_exp, w.n_ss, dev(w.obs),
+                             dev(w.sigma), dtype=dtype, want_flux=True)
+    out, chi = host(out), host(chi)
+    rows = np.arange(0, 128, 16)
+    chi_ref, ref = orc.loglike(w.params[rows], w.times, w.t_exp, w.n_ss, w.obs, w.sigma)
+    assert np.abs(out[rows] - ref).max() <= FTOL[dtype]
+    assert np.abs(chi[rows] / chi_ref - 1.0).max() <= CTOL[dtype]
+    rng = np.random.default_rng(7)
+    cols = np.sort(rng.choice(w.T, 64, replace=False))
+    ref2 = orc.lightcurve(w.params, w.times[cols], w.t_exp, w.n_ss)
+    assert np.abs(out[:, cols] - ref2).max() <= FTOL[dtype]
+    assert np.all(np.isfinite(out)) and out.max() <= 1.0 + 1e-6
+
+
+@pytest.mark.parametrize("dtype", ["f32", "f64"])
+def test_config5_edge_geometries(gl, dtype):
+    """200k rows with the same forced-class mix as the 1e6-row config (10 % forced)."""
+    geom, cls = wl.config5(N=200_000)
+    ref = orc.flux_geometry(geom)
+    out = host(gl.gl_flux_geometry(dev(geom), dtype=dtype))
+    err = np.abs(out - ref)
+    for c in range(5):
+        assert err[cls == c].max() <= FTOL[dtype], (c, err[cls == c].max())
+    assert np.all(out[ref == 1.0] >= 1.0 - FTOL[dtype])
+
+
+def test_config5_full_size_sampled(gl):
+    """The 1e6-row launch bench.py uses; the oracle checks a 40k sample plus all forced rows of
+    class (iv) (four crossings)."""
+    geom, cls = wl.config5()
+    out32 = host(gl.gl_flux_geometry(dev(geom), dtype="f32"))
+    out64 = host(gl.gl_flux_geometry(dev(geom), dtype="f64"))
+    rng = np.random.default_rng(11)
+    idx = np.unique(np.concatenate([rng.choice(geom.shape[0], 40_000, replace=False),
+                                    np.flatnonzero(cls == 4)]))
+    ref = orc.flux_geometry(geom[idx])
+    assert np.abs(out32[idx] - ref).max() <= 5e-7
+    assert np.abs(out64[idx] - ref).max() <= 1e-11
+    assert np.abs(out32 - out64).max() <= 5e-7      # property that holds at any size
+
+
+@pytest.mark.parametrize("dtype", ["f32", "f64"])
+def test_edge_cases(gl, dtype):
+    import torch
+    w = wl.config2()
+    p = np.repeat(w.params, 6, axis=0)
+    p[1, 6] = 0.6            # Rp >= 0.5: invalid
+    p[2, 7] = np.nan         # non-finite
+    p[3, 4] = 0.3            # eccentric orbit
+    p[3, 5] = 1.1
+    p[4, 3] = 1.03           # grazing: |b| > 1 - Rp
+    p[5, 7] = 0.0            # sphere
+    t = w.times[1900:2003]   # ragged: not a multiple of anything
+    chi_ref, ref = orc.loglike(p, t, w.t_exp, w.n_ss, w.obs[1900:2003], w.sigma[1900:2003])
+    chi, out = gl.gl_loglike(dev(p), dev(t), w.t_exp, w.n_ss, dev(w.obs[1900:2003]),
+                             dev(w.sigma[1900:2003]), dtype=dtype, want_flux=True)
+    out, chi = host(out), host(chi)
+    assert np.all(np.isnan(out[1])) and np.all(np.isnan(out[2]))
+    assert np.isinf(chi[1]) and np.isinf(chi[2]) and np.isinf(chi_ref[1])
+    good = [0, 3, 4, 5]
+    assert np.abs(out[good] - ref[good]).max() <= FTOL[dtype]
+    assert np.abs(chi[good] / chi_ref[good] - 1.0).max() <= CTOL[dtype]
+    # empty inputs are a no-op
+    e = gl.gl_lightcurve(dev(np.zeros((0, 12))), dev(t), 0.0, 1, dtype=dtype)
+    assert e.shape == (0, t.shape[0])
+    e = gl.gl_lightcurve(dev(p), dev(np.zeros(0)), 0.0, 1, dtype=dtype)
+    assert e.shape == (6, 0)
+    assert gl.gl_flux_geometry(dev(np.zeros((0, 6))), dtype=dtype).shape == (0,)
+    # unsorted, repeated times and many orbits away from t0: same values as sorted
+    perm = np.random.default_rng(3).permutation(t.shape[0])
+    tt = t[perm] + 542.0 * 7
+    o2 = host(gl.gl_lightcurve(dev(p[good]), dev(tt), w.t_exp, w.n_ss, dtype=dtype))
+    r2 = orc.lightcurve(p[good], tt, w.t_exp, w.n_ss)
+    assert np.abs(o2 - r2).max() <= FTOL[dtype]
+    # more sub-exposures than threads in a CTA (serial fallback), and n_ss = 1 with t_exp = 0
+    o3 = host(gl.gl_lightcurve(dev(p[:1]), dev(t[40:60]), w.t_exp, 300, dtype=dtype))
+    r3 = orc.lightcurve(p[:1], t[40:60], w.t_exp, 300)
+    assert np.abs(o3 - r3).max() <= FTOL[dtype]
+    with pytest.raises(gl.GreenlanternError):
+        gl.gl_lightcurve(dev(p), dev(t), 0.0, 0, dtype=dtype)
+    with pytest.raises(gl.GreenlanternError):
+        gl.gl_lightcurve(torch.zeros(1, 12, dtype=torch.float64), dev(t), 0.0, 1, dtype=dtype)
+
+
+def test_host_wrappers_match_device_path(gl):
+    w = wl.config3(B=16)
+    chi_d, flux_d = gl.gl_loglike(dev(w.params), dev(w.times), w.t_exp, w.n_ss, dev(w.obs),
+                                  dev(w.sigma), dtype="f32", want_flux=True)
+    chi_h, flux_h = gl.gl_loglike_host(w.params, w.times, w.t_exp, w.n_ss, w.obs, w.sigma,
+                                       dtype="f32", want_flux=True)
+    assert np.array_equal(host(chi_d), chi_h.astype(np.float64))
+    assert np.array_equal(host(flux_d), flux_h.astype(np.float64))
+    lc = gl.gl_lightcurve_host(w.params, w.times, w.t_exp, w.n_ss, dtype="f64")
+    assert np.abs(lc - host(flux_d)).max() <= 5e-7
+    geom, _ = wl.config5(N=10_000)
+    assert np.array_equal(gl.gl_flux_geometry_host(geom, "f32").astype(np.float64),
+                          host(gl.gl_flux_geometry(dev(geom), "f32")))
+    assert gl.gl_launch_count() > 0
