@@ -1,0 +1,298 @@
+// gl_fast32.cuh -- fp32 PRODUCTION arithmetic of steps a3 + a4: the same three area
+// integrals as gl_core.cuh, arranged for throughput on the sm_100a FP32 and MUFU pipes.
+//
+// What is different from the generic (validation) code in gl_core.cuh, and why it is allowed:
+//  * The result wanted is the BLOCKED FRACTION delta = 1 - F <= ~0.06, to 5e-7 absolute, i.e. to
+//    1e-5 relative at best: MUFU approximations (sin/cos/rcp/sqrt .approx, ~2^-21 absolute) are far
+//    inside the budget as long as no step cancels (every term below is O(a) or smaller).
+//  * A crossing angle that is wrong by eps moves the three areas by O(eps^2): all three 1-forms
+//    (eqs. 21-23, D3) are multiples of x dy - y dx, which vanishes on the radial
+//    segment that joins a slightly-off crossing point to the limb, so only the sliver between the
+//    two curves (width ~ |g'| eps, length eps) is mis-counted (R12).  Crossings are therefore
+//    solved to 5e-5 rad, not to an ulp.
+//  * An outline that lies wholly inside the disc is a closed, periodic contour: the N-point
+//    trapezoid rule at FIXED angles 2 pi k/N converges geometrically and needs no trigonometry at
+//    run time (cos/sin of the nodes are constants).  Measured on 4e5 config-5 geometries in fp64
+//    (DESIGN.md 5.6): N = 16 is good to 2e-8 in flux once the gap to the limb is >= 0.01, N = 32 to
+//    1.7e-8 for every gap down to tangency.
+//  * Only the rare geometries whose star centre may lie inside the outline's evolute (a second
+//    pair of critical points, up to four crossings) go through gl_core.cuh's bracketed search.
+#pragma once
+#include "gl_core.cuh"
+
+namespace glf {
+
+#ifdef __CUDACC__
+#define GLF_DEV __device__ __forceinline__
+#define GLF_CONST __constant__
+#else   // host build: only for checking the arithmetic on a CPU (exact math in place of MUFU)
+#define GLF_DEV inline
+#define GLF_CONST static
+#endif
+
+// cos, sin of 2 pi k / 32, k = 0..15 (the other half is the mirror image); filled at library load.
+GLF_CONST float c_trap_cos[16], c_trap_sin[16];
+// smoothed Gauss-Legendre table of the generic path (gl_tables.h), fp32 copy: 8 positive nodes.
+GLF_CONST float c_gl_phi[8], c_gl_om[8];
+
+constexpr float kPiF = 3.14159265358979323846f;
+constexpr float kTwoPiF = 6.28318530717958647692f;
+
+#ifdef __CUDACC__
+GLF_DEV float mufu_rcp(float x) {
+    float r;
+    asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(x));
+    return r;
+}
+GLF_DEV float mufu_sqrt(float x) {
+    float r;
+    asm("sqrt.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(x));
+    return r;
+}
+GLF_DEV float mufu_rsqrt(float x) {
+    float r;
+    asm("rsqrt.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(x));
+    return r;
+}
+GLF_DEV float mufu_sin(float x) {
+    float r;
+    asm("sin.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(x));
+    return r;
+}
+GLF_DEV float mufu_cos(float x) {
+    float r;
+    asm("cos.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(x));
+    return r;
+}
+GLF_DEV float fast_div(float x, float y) { return __fdividef(x, y); }
+#else
+GLF_DEV float mufu_rcp(float x) { return 1.f / x; }
+GLF_DEV float mufu_sqrt(float x) { return sqrtf(x); }
+GLF_DEV float mufu_rsqrt(float x) { return 1.f / sqrtf(x); }
+#ifdef GLF_HOST_NOISE   // the harness models the 2^-21 absolute error of MUFU.SIN/COS
+GLF_DEV float mufu_sin(float x) { return sinf(x) + nz(); }
+GLF_DEV float mufu_cos(float x) { return cosf(x) + nz(); }
+#else
+GLF_DEV float mufu_sin(float x) { return sinf(x); }
+GLF_DEV float mufu_cos(float x) { return cosf(x); }
+#endif
+GLF_DEV float fast_div(float x, float y) { return x / y; }
+#endif
+// sin, cos of an angle in [-pi, 3 pi]: folded into [-pi, pi], where the MUFU error is 2^-21.
+GLF_DEV void mufu_sincos(float t, float* s, float* c) {
+    const float tr = (t > kPiF) ? t - kTwoPiF : t;
+    *s = mufu_sin(tr);
+    *c = mufu_cos(tr);
+}
+
+// W(s) f for the two mirror nodes of a pair, sharing ONE reciprocal:
+//   W = 1 + m^2/(1+m), m = sqrt(max(1 - r^2, 0))   (eq. 22 in the form of R9, R11)
+GLF_DEV float pair_term(float m2p, float fp, float m2q, float fq) {
+    m2p = fmaxf(m2p, 0.f);
+    m2q = fmaxf(m2q, 0.f);
+    const float dp = 1.f + mufu_sqrt(m2p), dq = 1.f + mufu_sqrt(m2q);
+    const float r = mufu_rcp(dp * dq);             // 1/dp = dq r, 1/dq = dp r
+    const float Wp = fmaf(m2p, dq * r, 1.f), Wq = fmaf(m2q, dp * r, 1.f);
+    return fmaf(Wp, fp, Wq * fq);
+}
+
+// Integral over the WHOLE outline of W(r^2) (2 f_flat) dt by the N-point trapezoid rule, N = 16 or
+// 32.  2 f_flat = ab + u cos t + v sin t with u = b xc, v = a yc (gl_core.cuh).  Nodes k and k+N/2
+// are mirror images, so each table entry serves two nodes.
+template <int N>
+GLF_DEV float whole_outline_lin(float xc, float yc, float a, float b, float ab,
+                                                   float u, float v) {
+    constexpr int STRIDE = 32 / N;
+    float acc = 0.f;
+#pragma unroll
+    for (int k = 0; k < N / 2; ++k) {
+        const float c = c_trap_cos[k * STRIDE], s = c_trap_sin[k * STRIDE];
+        const float p = a * c, q = b * s;
+        const float xp = xc + p, yp = yc + q, xq = xc - p, yq = yc - q;
+        const float m2p = fmaf(-xp, xp, fmaf(-yp, yp, 1.f));
+        const float m2q = fmaf(-xq, xq, fmaf(-yq, yq, 1.f));
+        const float w = fmaf(u, c, v * s);
+        acc += pair_term(m2p, ab + w, m2q, ab - w);
+    }
+    return acc * (kTwoPiF / float(N));
+}
+
+// The outline in the kernel frame, re-parametrised by tau = t - t_far (t_far = the outline point
+// farthest from the star centre, given by its cosine/sine cf, sf).
+struct Arc {
+    float xc, yc, a, b, cf, sf;
+};
+GLF_DEV void abs_trig(const Arc& o, float tau, float* s, float* c) {
+    float st, ct;
+    mufu_sincos(tau, &st, &ct);
+    *c = o.cf * ct - o.sf * st;
+    *s = o.sf * ct + o.cf * st;
+}
+// g = x^2 + y^2 - 1 and g'/2 at tau; also returns the absolute sine/cosine.
+GLF_DEV void eval_g(const Arc& o, float tau, float* g, float* h, float* s,
+                                       float* c) {
+    abs_trig(o, tau, s, c);
+    const float x = fmaf(o.a, *c, o.xc), y = fmaf(o.b, *s, o.yc);
+    *g = fmaf(x, x, fmaf(y, y, -1.f));
+    *h = o.b * *c * y - o.a * *s * x;
+}
+
+// Crossing of g on [lo, hi] (one sign change): Newton from `t`, bisection whenever the step leaves
+// the bracket.  Stops BEFORE applying a step shorter than 5e-5 rad, or when |g| is at the fp32
+// rounding level of x^2 + y^2 - 1 (near-tangent crossings, where Newton would only chase noise),
+// or at the iteration cap -- always WITHOUT moving, so that (s, c) belong to the angle returned
+// (a mismatch would open a gap between the outline arc and the limb arc).
+GLF_DEV float crossing(const Arc& o, float lo, float hi, float t, bool rising, float* s, float* c) {
+    t = fminf(fmaxf(t, lo), hi);
+    for (int it = 0;; ++it) {
+        float g, h;
+        eval_g(o, t, &g, &h, s, c);
+        if ((g > 0.f) == rising) hi = t; else lo = t;
+        float tn = t - fast_div(g, h + h);
+        if (!(tn > lo && tn < hi)) tn = 0.5f * (lo + hi);
+        if (fabsf(tn - t) < 5e-5f || fabsf(g) < 1.5e-7f || it == 23) break;
+        t = tn;
+    }
+    return t;
+}
+
+// acos for a FIRST GUESS only (error < 0.02 rad): sqrt(2(1-r)) series, mirrored for r < 0.
+GLF_DEV float rough_acos(float r) {
+    const float q = 1.f - fabsf(r);
+    const float u = mufu_sqrt(q + q) * fmaf(q, fmaf(q, 0.01875f, 0.0833333f), 1.f);
+    return r < 0.f ? kPiF - u : u;
+}
+
+// Critical point of g near the unit vector (c, s): Newton on h = g'/2 by small rotations, kept
+// inside the quadrant with sign pattern (sx, sy).  SGN = +1: the maximum (h' < 0 there; where the
+// curvature has the wrong sign the step is a fixed 0.5 rad uphill), SGN = -1: the minimum.
+// Stops after a step shorter than 1e-3 rad (the error left is ~ that step squared).
+template <int SGN>
+GLF_DEV void critical_point(float xc, float yc, float a, float b, float* c,
+                                               float* s, float sx, float sy) {
+    for (int it = 0; it < 12; ++it) {
+        const float x = fmaf(a, *c, xc), y = fmaf(b, *s, yc);
+        const float bc = b * *c, as = a * *s;
+        const float h = bc * y - as * x;
+        const float hp = fmaf(bc, bc, as * as) - fmaf(b * *s, y, a * *c * x);
+        float d = (float(SGN) * hp < 0.f) ? -fast_div(h, hp) : copysignf(0.5f, float(SGN) * h);
+        d = fminf(fmaxf(d, -0.5f), 0.5f);
+        // rotate (c, s) by d: sin d, cos d to O(d^7), then renormalise
+        const float d2 = d * d;
+        const float sd = d * fmaf(d2, fmaf(d2, 1.f / 120.f, -1.f / 6.f), 1.f);
+        const float cd = fmaf(d2, fmaf(d2, fmaf(d2, -1.f / 720.f, 1.f / 24.f), -0.5f), 1.f);
+        float cn = *c * cd - *s * sd, sn = *s * cd + *c * sd;
+        cn = sx * fmaxf(sx * cn, 0.f);
+        sn = sy * fmaxf(sy * sn, 0.f);
+        const float rn = mufu_rsqrt(fmaf(cn, cn, sn * sn));
+        *c = cn * rn;
+        *s = sn * rn;
+        if (fabsf(d) < 1e-3f) break;
+    }
+}
+
+// Blocked fraction delta = k0 A_flat + k1 A_lin + k2 A_quad for an outline with centre (xc, yc) in
+// the kernel frame (any signs), semi-axes a >= b > 0, a < 1/2.  k0, k1, k2 = c0, c1, c2 of R8 divided
+// by pi (1 - u1/3 - u2/6).  Returns 0 when the overlap is empty.
+GLF_DEV float blocked_f32(float xc_in, float yc_in, float a, float b, float k0,
+                                             float k1, float k2) {
+    const float xc = fabsf(xc_in), yc = fabsf(yc_in);   // mirror images have the same areas
+    const float r0sq = fmaf(xc, xc, yc * yc);
+    const float reach = 1.f + a;
+    if (r0sq >= reach * reach) return 0.f;
+    const float ab = a * b, u = b * xc, v = a * yc;
+    const float e2 = (a - b) * (a + b);
+    // whole-outline closed forms: A_flat = pi a b, A_quad = pi a b (r0^2 + (a^2 + b^2)/4)
+    const float in_flat = kPiF * ab;
+    const float in_quad = in_flat * fmaf(0.25f, fmaf(a, a, b * b), r0sq);
+    const float r0 = r0sq * mufu_rsqrt(fmaxf(r0sq, 1e-30f));
+    if (r0 + a <= 0.99f) {
+        // well inside the limb (gap >= 0.01): 16 fixed nodes
+        const float lin = whole_outline_lin<16>(xc, yc, a, b, ab, u, v);
+        return fmaf(k0, in_flat, fmaf(k1 * (1.f / 3.f), lin, k2 * in_quad));
+    }
+    const float Aa = a * xc, Bb = b * yc;
+    if (Aa < e2 && Bb < e2) {
+        // the star centre may lie inside the evolute (up to four crossings): bracketed search
+        float A[3];
+        if (!glc::overlap_areas<float, 16>(xc, yc, a, b, c_gl_phi, c_gl_om, A)) return 0.f;
+        return fmaf(k0, A[0], fmaf(k1, A[1], k2 * A[2]));
+    }
+    // farthest outline point from the star centre: the only maximum of g (first quadrant)
+    float cf, sf;
+    {
+        const float rn = mufu_rsqrt(fmaf(Aa, Aa, Bb * Bb));   // Aa, Bb not both 0 here (r0 > 0.49)
+        cf = Aa * rn;
+        sf = Bb * rn;
+        critical_point<1>(xc, yc, a, b, &cf, &sf, 1.f, 1.f);
+    }
+    const float xf = fmaf(a, cf, xc), yf = fmaf(b, sf, yc);
+    const float gfar = fmaf(xf, xf, fmaf(yf, yf, -1.f));
+    if (gfar <= 0.f) {
+        // wholly inside, close to the limb
+        const float lin = (gfar < -0.04f) ? whole_outline_lin<16>(xc, yc, a, b, ab, u, v)
+                                          : whole_outline_lin<32>(xc, yc, a, b, ab, u, v);
+        return fmaf(k0, in_flat, fmaf(k1 * (1.f / 3.f), lin, k2 * in_quad));
+    }
+    // the outline crosses the limb twice (or misses the disc).  tau = t - t_far in [0, 2 pi).
+    Arc o = {xc, yc, a, b, cf, sf};
+    float tsplit = kPiF;
+    const float xo = fmaf(-a, cf, xc), yo = fmaf(-b, sf, yc);   // the point opposite t_far
+    float gsplit = fmaf(xo, xo, fmaf(yo, yo, -1.f));
+    if (gsplit >= 0.f) {
+        // mostly outside: find the nearest outline point (third quadrant) and its tau
+        float cn = -cf, sn = -sf;
+        critical_point<-1>(xc, yc, a, b, &cn, &sn, -1.f, -1.f);
+        const float xn = fmaf(a, cn, xc), yn = fmaf(b, sn, yc);
+        gsplit = fmaf(xn, xn, fmaf(yn, yn, -1.f));
+        if (gsplit >= 0.f) return 0.f;
+        float dtau = atan2f(cf * sn - sf * cn, cf * cn + sf * sn);   // in (-pi, pi]
+        tsplit = dtau < 0.f ? dtau + kTwoPiF : dtau;
+    }
+    // half-cosine model of g between its maximum and the split point (exact for a circle)
+    const float mid = 0.5f * (gfar + gsplit), amp = 0.5f * (gfar - gsplit);
+    const float uu = rough_acos(fminf(fmaxf(-fast_div(mid, amp), -1.f), 1.f)) * (1.f / kPiF);
+    float s1, c1, s2, c2;
+    const float t1 = crossing(o, 0.f, tsplit, uu * tsplit, false, &s1, &c1);
+    const float t2 = crossing(o, tsplit, kTwoPiF, kTwoPiF - uu * (kTwoPiF - tsplit), true, &s2, &c2);
+    // ---- outline arc [t1, t2] (inside the disc): flat and quad in closed form
+    glc::Outline<float> oo = {xc, yc, a, b, e2};
+    const glc::ArcCoef<float> k = glc::arc_coefficients(oo);
+    const float dt = t2 - t1;
+    float f1, q1, f2, q2;
+    glc::arc_primitive(k, s1, c1, &f1, &q1);
+    glc::arc_primitive(k, s2, c2, &f2, &q2);
+    float Aflat = 0.5f * fmaf(k.ab, dt, f2 - f1);
+    float Aquad = 0.25f * fmaf(k.k0, dt, q2 - q1);
+    // ---- f_lin: 16-point Gauss-Legendre in z, t = tm + hw (3z - z^3)/2
+    const float hw = 0.5f * dt;
+    float sm, cm;
+    abs_trig(o, t1 + hw, &sm, &cm);
+    float acc = 0.f;
+#pragma unroll
+    for (int i = 0; i < 8; ++i) {
+        float sd, cd;
+        const float dd = hw * c_gl_phi[i];   // in [0, pi]
+        sd = mufu_sin(dd);
+        cd = mufu_cos(dd);
+        const float cp = cm * cd - sm * sd, sp = sm * cd + cm * sd;
+        const float cq = cm * cd + sm * sd, sq = sm * cd - cm * sd;
+        const float xp = fmaf(a, cp, xc), yp = fmaf(b, sp, yc);
+        const float xq = fmaf(a, cq, xc), yq = fmaf(b, sq, yc);
+        const float m2p = fmaf(-xp, xp, fmaf(-yp, yp, 1.f));
+        const float m2q = fmaf(-xq, xq, fmaf(-yq, yq, 1.f));
+        const float fp = fmaf(u, cp, fmaf(v, sp, ab)), fq = fmaf(u, cq, fmaf(v, sq, ab));
+        acc = fmaf(c_gl_om[i], pair_term(m2p, fp, m2q, fq), acc);
+    }
+    float Alin = (1.f / 3.f) * hw * acc;
+    // ---- limb arc from the exit point (t2) counter-clockwise back to the entry point (t1)
+    const float xa = fmaf(a, c2, xc), ya = fmaf(b, s2, yc);
+    const float xb = fmaf(a, c1, xc), yb = fmaf(b, s1, yc);
+    const float dl = atan2f(xa * yb - ya * xb, xa * xb + ya * yb);
+    Aflat = fmaf(0.5f, dl, Aflat);
+    Alin = fmaf(1.f / 3.f, dl, Alin);
+    Aquad = fmaf(0.25f, dl, Aquad);
+    return fmaf(k0, Aflat, fmaf(k1, Alin, k2 * Aquad));
+}
+
+}  // namespace glf

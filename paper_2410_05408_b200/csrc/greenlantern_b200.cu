@@ -20,6 +20,7 @@
 
 #include "../../include/greenlantern_b200.h"
 #include "gl_core.cuh"
+#include "gl_fast32.cuh"
 #include "gl_tables.h"
 
 namespace cg = cooperative_groups;
@@ -32,20 +33,7 @@ constexpr int NT = 256;    // threads per CTA
 constexpr int TILE = 1024; // exposure times classified per tile
 constexpr int MAXCLUSTER = 8;
 
-__constant__ float c_phi32[NQ32 / 2], c_om32[NQ32 / 2];
 __constant__ double c_phi64[NQ64 / 2], c_om64[NQ64 / 2];
-
-template <typename T> struct Quad;
-template <> struct Quad<float> {
-    static constexpr int N = NQ32;
-    static __device__ __forceinline__ const float* phi() { return c_phi32; }
-    static __device__ __forceinline__ const float* om() { return c_om32; }
-};
-template <> struct Quad<double> {
-    static constexpr int N = NQ64;
-    static __device__ __forceinline__ const double* phi() { return c_phi64; }
-    static __device__ __forceinline__ const double* om() { return c_om64; }
-};
 
 constexpr double kPi = 3.14159265358979323846;
 constexpr double kTwoPi = 6.28318530717958647692;
@@ -214,6 +202,21 @@ template <typename T> __device__ __forceinline__ WalkerT<T> narrow(const Walker&
     return v;
 }
 
+// a3 + a4 for an outline centred at (xc, yc) in the kernel frame: fp64 = generic bracketed search +
+// 48-point rule (validation), fp32 = gl_fast32.cuh (production).
+template <typename T> __device__ __forceinline__ T blocked_at(T xc, T yc, T a, T b, T k0, T k1, T k2);
+template <> __device__ __forceinline__ double blocked_at<double>(double xc, double yc, double a,
+                                                                 double b, double k0, double k1,
+                                                                 double k2) {
+    double A[3];
+    if (!glc::overlap_areas<double, NQ64>(xc, yc, a, b, c_phi64, c_om64, A)) return 0.0;
+    return k0 * A[0] + k1 * A[1] + k2 * A[2];
+}
+template <> __device__ __forceinline__ float blocked_at<float>(float xc, float yc, float a, float b,
+                                                               float k0, float k1, float k2) {
+    return glf::blocked_f32(xc, yc, a, b, k0, k1, k2);
+}
+
 // Blocked fraction delta = 1 - F_inst at reduced phase ph (a1 + a3 + a4).
 template <typename T>
 __device__ __forceinline__ T blocked_fraction(const Walker& w, const WalkerT<T>& v, double ph) {
@@ -232,10 +235,7 @@ __device__ __forceinline__ T blocked_fraction(const Walker& w, const WalkerT<T>&
         y0 = T(Y);
     }
     const T xc = v.cpsi * x0 + v.spsi * y0, yc = v.cpsi * y0 - v.spsi * x0;
-    T A[3];
-    if (!glc::overlap_areas<T, Quad<T>::N>(xc, yc, v.a, v.b, Quad<T>::phi(), Quad<T>::om(), A))
-        return T(0);
-    return v.k0 * A[0] + v.k1 * A[1] + v.k2 * A[2];
+    return blocked_at<T>(xc, yc, v.a, v.b, v.k0, v.k1, v.k2);
 }
 
 // ------------------------------------------------------------------------------------------
@@ -258,6 +258,12 @@ __device__ __forceinline__ double block_sum(double v, double* warp_scratch) {
 // The fused kernel.  grid = (cluster size C, walkers in flight); cluster = (C, 1, 1).
 //   flux  : [B, T] of T-typed values or nullptr          chi2 : [B] or nullptr
 //   obs, sigma : [T] fp64 or nullptr (only read when chi2 != nullptr)
+// Per walker the exposure times are taken in rounds of C * TILE: CTA r classifies tile r of the
+// round against the transit window (out-of-window times are finished on the spot), compacts the
+// in-window indices into its own shared list, and after ONE cluster barrier every CTA takes an
+// equal share of the round's whole in-window list, reading the other CTAs' lists over DSMEM.
+// A K2-shaped series (1 % in transit, all of it inside one tile) is thereby spread over the whole
+// cluster.  Lists are double-buffered, so one barrier per round is enough.
 // ------------------------------------------------------------------------------------------
 template <typename T>
 __global__ void __launch_bounds__(NT)
@@ -269,16 +275,20 @@ transit_kernel(const double* __restrict__ params, int B, const double* __restric
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
 
     __shared__ Walker sw;
-    __shared__ int s_list[TILE];
+    __shared__ int s_list[2][TILE];   // in-window time indices of this CTA's tile (double-buffered)
+    __shared__ int s_nlist[2];
+    __shared__ int s_pre[MAXCLUSTER + 1];   // prefix of the cluster's list lengths, this round
+    __shared__ int s_idx[NT];         // time index of each slot of the current batch
     __shared__ T s_buf[NT];
     __shared__ int s_wcount[NT / 32];
-    __shared__ int s_nlist;
     __shared__ double s_red[NT / 32];
     __shared__ double s_partial;   // this CTA's chi^2 partial, read by cluster rank 0 via DSMEM
 
     const double inv_ss = 1.0 / (double)n_ss;
-    const int ntiles = (nT + TILE - 1) / TILE;
+    const int round_span = csize * TILE;
+    const int nrounds = (nT + round_span - 1) / round_span;
     const bool want_chi2 = (chi2 != nullptr);
+    int buf = 0;
 
     for (int wk = blockIdx.y; wk < B; wk += gridDim.y) {
         __syncthreads();
@@ -297,9 +307,9 @@ transit_kernel(const double* __restrict__ params, int B, const double* __restric
             const bool circ = v.circular;
             const double hwin = sw.half_win_phase;
             const double reach = (1.0 + sw.a) * (1.0 + 1e-12) + 0.5 * t_exp * sw.vmax;
-            for (int tile = crank; tile < ntiles; tile += csize) {
-                const int i0 = tile * TILE;
-                if (tid == 0) s_nlist = 0;
+            for (int round = 0; round < nrounds; ++round, buf ^= 1) {
+                const int i0 = (round * csize + crank) * TILE;
+                if (tid == 0) s_nlist[buf] = 0;
                 __syncthreads();
                 // ---- classify TILE exposure times, compact the in-window ones (stable order)
                 for (int r = 0; r < TILE / NT; ++r) {
@@ -326,26 +336,48 @@ transit_kernel(const double* __restrict__ params, int B, const double* __restric
                     const unsigned bal = __ballot_sync(0xffffffffu, inwin);
                     if (lane == 0) s_wcount[warp] = __popc(bal);
                     __syncthreads();
-                    int base = s_nlist;
+                    int base = s_nlist[buf];
                     for (int k = 0; k < warp; ++k) base += s_wcount[k];
-                    if (inwin) s_list[base + __popc(bal & ((1u << lane) - 1u))] = i;
+                    if (inwin) s_list[buf][base + __popc(bal & ((1u << lane) - 1u))] = i;
                     __syncthreads();
                     if (tid == 0) {
-                        int tot = s_nlist;
+                        int tot = s_nlist[buf];
                         for (int k = 0; k < NT / 32; ++k) tot += s_wcount[k];
-                        s_nlist = tot;
+                        s_nlist[buf] = tot;
                     }
                     __syncthreads();
                 }
-                const int nlist = s_nlist;
-                // ---- evaluate the (time, sub-exposure) pairs of the in-window list
+                // ---- share the round's list over the cluster
+                cluster.sync();
+                if (tid < csize) s_wcount[tid] = *cluster.map_shared_rank(&s_nlist[buf], tid);
+                __syncthreads();
+                if (tid == 0) {
+                    int run = 0;
+                    for (int r = 0; r < csize; ++r) {
+                        s_pre[r] = run;
+                        run += s_wcount[r];
+                    }
+                    s_pre[csize] = run;
+                }
+                __syncthreads();
+                const int M = s_pre[csize];
+                const int m0 = (int)(((long long)M * crank) / csize);
+                const int m1 = (int)(((long long)M * (crank + 1)) / csize);
+                auto fetch = [&](int p) {
+                    int r = 0;
+                    while (r + 1 < csize && p >= s_pre[r + 1]) ++r;
+                    return *cluster.map_shared_rank(&s_list[buf][p - s_pre[r]], r);
+                };
+                // ---- evaluate the (time, sub-exposure) pairs of this CTA's share
                 if (n_ss <= NT) {
                     const int per = NT / n_ss;   // exposure times per batch
-                    for (int l0 = 0; l0 < nlist; l0 += per) {
-                        const int nl = min(per, nlist - l0);
+                    for (int l0 = m0; l0 < m1; l0 += per) {
+                        const int nl = min(per, m1 - l0);
+                        if (tid < nl) s_idx[tid] = fetch(l0 + tid);
+                        __syncthreads();
                         if (tid < nl * n_ss) {
                             const int l = tid / n_ss, j = tid - l * n_ss;
-                            const double t = times[s_list[l0 + l]] +
+                            const double t = times[s_idx[l]] +
                                              (((double)j + 0.5) * inv_ss - 0.5) * t_exp;
                             s_buf[tid] = blocked_fraction<T>(sw, v, reduced_phase(sw, t));
                         }
@@ -354,7 +386,7 @@ transit_kernel(const double* __restrict__ params, int B, const double* __restric
                             T sum = T(0);
                             for (int j = 0; j < n_ss; ++j) sum += s_buf[tid * n_ss + j];
                             const T dbar = sum * T(inv_ss);
-                            const int i = s_list[l0 + tid];
+                            const int i = s_idx[tid];
                             if (frow) frow[i] = T(1) - dbar;
                             if (want_chi2) {
                                 const double sg = sigma[i];
@@ -362,12 +394,11 @@ transit_kernel(const double* __restrict__ params, int B, const double* __restric
                                 acc += (sg > 0.0 && isfinite(sg)) ? rr * rr : (double)INFINITY;
                             }
                         }
-                        __syncthreads();
                     }
                 } else {
                     // more sub-exposures than threads: one exposure time per thread, serial in j
-                    for (int l = tid; l < nlist; l += NT) {
-                        const int i = s_list[l];
+                    for (int l = m0 + tid; l < m1; l += NT) {
+                        const int i = fetch(l);
                         T sum = T(0);
                         for (int j = 0; j < n_ss; ++j) {
                             const double t = times[i] + (((double)j + 0.5) * inv_ss - 0.5) * t_exp;
@@ -398,6 +429,7 @@ transit_kernel(const double* __restrict__ params, int B, const double* __restric
             cluster.sync();   // keep every CTA's shared memory alive until rank 0 has read it
         }
     }
+    cluster.sync();   // no CTA may exit while a neighbour can still read its lists
 }
 
 // ------------------------------------------------------------------------------------------
@@ -423,14 +455,9 @@ geometry_kernel(const double* __restrict__ geom, long long N, T* __restrict__ ou
     T s, c;
     glc::gsincos(T(pa), &s, &c);
     const T a = T(Rp), b = T(Rp * (1.0 - fp));
-    T A[3];
-    T delta = T(0);
-    if (glc::overlap_areas<T, Quad<T>::N>(T(d) * c, -T(d) * s, a, b, Quad<T>::phi(), Quad<T>::om(),
-                                          A)) {
-        const double pn = kPi * norm;
-        delta = T((1.0 - u1 - 2.0 * u2) / pn) * A[0] + T((u1 + 2.0 * u2) / pn) * A[1] +
-                T(u2 / pn) * A[2];
-    }
+    const double pn = kPi * norm;
+    const T delta = blocked_at<T>(T(d) * c, -T(d) * s, a, b, T((1.0 - u1 - 2.0 * u2) / pn),
+                                  T((u1 + 2.0 * u2) / pn), T(u2 / pn));
     out[k] = T(1) - delta;
 }
 
@@ -462,8 +489,17 @@ int ensure_tables() {
     double p64[NQ64 / 2], o64[NQ64 / 2];
     glt::smoothed_gauss_legendre<float>(NQ32, p32, o32);
     glt::smoothed_gauss_legendre<double>(NQ64, p64, o64);
-    if ((e = cudaMemcpyToSymbol(c_phi32, p32, sizeof(p32))) != cudaSuccess ||
-        (e = cudaMemcpyToSymbol(c_om32, o32, sizeof(o32))) != cudaSuccess ||
+    float tc[16], ts[16];
+    for (int k = 0; k < 16; ++k) {
+        tc[k] = (float)cosl(3.141592653589793238462643383279502884L * k / 16.0L);
+        ts[k] = (float)sinl(3.141592653589793238462643383279502884L * k / 16.0L);
+    }
+    tc[8] = 0.f;   // exact zeros at the axes
+    ts[0] = 0.f;
+    if ((e = cudaMemcpyToSymbol(glf::c_gl_phi, p32, sizeof(p32))) != cudaSuccess ||
+        (e = cudaMemcpyToSymbol(glf::c_gl_om, o32, sizeof(o32))) != cudaSuccess ||
+        (e = cudaMemcpyToSymbol(glf::c_trap_cos, tc, sizeof(tc))) != cudaSuccess ||
+        (e = cudaMemcpyToSymbol(glf::c_trap_sin, ts, sizeof(ts))) != cudaSuccess ||
         (e = cudaMemcpyToSymbol(c_phi64, p64, sizeof(p64))) != cudaSuccess ||
         (e = cudaMemcpyToSymbol(c_om64, o64, sizeof(o64))) != cudaSuccess)
         return cuda_fail(e, "cudaMemcpyToSymbol");
