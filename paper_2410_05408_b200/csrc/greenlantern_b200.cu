@@ -265,29 +265,37 @@ __device__ __forceinline__ double block_sum(double v, double* warp_scratch) {
 // A K2-shaped series (1 % in transit, all of it inside one tile) is thereby spread over the whole
 // cluster.  Lists are double-buffered, so one barrier per round is enough.
 // ------------------------------------------------------------------------------------------
+// Residual^2 of one exposure against the data (R19); a bad sigma poisons the walker's chi^2.
+__device__ __forceinline__ double residual_sq(double obs_m1, double delta, double sg) {
+    const double rr = (obs_m1 + delta) / sg;
+    return (sg > 0.0 && isfinite(sg)) ? rr * rr : (double)INFINITY;
+}
+
 template <typename T>
-__global__ void __launch_bounds__(NT)
+__global__ void __launch_bounds__(NT, sizeof(T) == 4 ? 4 : 1)
 transit_kernel(const double* __restrict__ params, int B, const double* __restrict__ times, int nT,
                double t_exp, int n_ss, const double* __restrict__ obs,
                const double* __restrict__ sigma, T* __restrict__ flux, T* __restrict__ chi2) {
     cg::cluster_group cluster = cg::this_cluster();
     const int crank = (int)cluster.block_rank(), csize = (int)cluster.num_blocks();
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    constexpr int NW = NT / 32, NSUB = TILE / NT;
 
     __shared__ Walker sw;
     __shared__ int s_list[2][TILE];   // in-window time indices of this CTA's tile (double-buffered)
     __shared__ int s_nlist[2];
-    __shared__ int s_pre[MAXCLUSTER + 1];   // prefix of the cluster's list lengths, this round
-    __shared__ int s_idx[NT];         // time index of each slot of the current batch
-    __shared__ T s_buf[NT];
-    __shared__ int s_wcount[NT / 32];
-    __shared__ double s_red[NT / 32];
+    __shared__ int s_cnt[NSUB * NW];  // in-window count per (sub-chunk, warp) of the tile
+    __shared__ int s_rcnt[MAXCLUSTER];   // list lengths of the cluster's CTAs, this round
+    __shared__ double s_red[NW];
     __shared__ double s_partial;   // this CTA's chi^2 partial, read by cluster rank 0 via DSMEM
 
     const double inv_ss = 1.0 / (double)n_ss;
     const int round_span = csize * TILE;
     const int nrounds = (nT + round_span - 1) / round_span;
     const bool want_chi2 = (chi2 != nullptr);
+    // lane -> (exposure slot l, sub-exposure j) when a warp holds G = 32 / n_ss whole exposures
+    const int G = n_ss <= 32 ? 32 / n_ss : 0;
+    const int my_l = G ? lane / n_ss : 0, my_j = G ? lane - my_l * n_ss : lane;
     int buf = 0;
 
     for (int wk = blockIdx.y; wk < B; wk += gridDim.y) {
@@ -309,10 +317,10 @@ transit_kernel(const double* __restrict__ params, int B, const double* __restric
             const double reach = (1.0 + sw.a) * (1.0 + 1e-12) + 0.5 * t_exp * sw.vmax;
             for (int round = 0; round < nrounds; ++round, buf ^= 1) {
                 const int i0 = (round * csize + crank) * TILE;
-                if (tid == 0) s_nlist[buf] = 0;
-                __syncthreads();
-                // ---- classify TILE exposure times, compact the in-window ones (stable order)
-                for (int r = 0; r < TILE / NT; ++r) {
+                // ---- classify TILE exposure times against the transit window
+                unsigned bal[NSUB];
+#pragma unroll
+                for (int r = 0; r < NSUB; ++r) {
                     const int i = i0 + r * NT + tid;
                     bool inwin = false;
                     if (i < nT) {
@@ -326,94 +334,91 @@ transit_kernel(const double* __restrict__ params, int B, const double* __restric
                         }
                         if (!inwin) {
                             if (frow) frow[i] = T(1);
-                            if (want_chi2) {
-                                const double sg = sigma[i];
-                                const double rr = (obs[i] - 1.0) / sg;
-                                acc += (sg > 0.0 && isfinite(sg)) ? rr * rr : (double)INFINITY;
-                            }
+                            if (want_chi2) acc += residual_sq(obs[i] - 1.0, 0.0, sigma[i]);
                         }
                     }
-                    const unsigned bal = __ballot_sync(0xffffffffu, inwin);
-                    if (lane == 0) s_wcount[warp] = __popc(bal);
-                    __syncthreads();
-                    int base = s_nlist[buf];
-                    for (int k = 0; k < warp; ++k) base += s_wcount[k];
-                    if (inwin) s_list[buf][base + __popc(bal & ((1u << lane) - 1u))] = i;
-                    __syncthreads();
-                    if (tid == 0) {
-                        int tot = s_nlist[buf];
-                        for (int k = 0; k < NT / 32; ++k) tot += s_wcount[k];
-                        s_nlist[buf] = tot;
+                    bal[r] = __ballot_sync(0xffffffffu, inwin);
+                    if (lane == 0) s_cnt[r * NW + warp] = __popc(bal[r]);
+                }
+                __syncthreads();
+                // ---- compact the in-window indices into this CTA's list, in index order
+                {
+                    int run = 0, base[NSUB];
+#pragma unroll
+                    for (int q = 0; q < NSUB * NW; ++q) {
+                        if ((q % NW) == warp) base[q / NW] = run;
+                        run += s_cnt[q];
                     }
-                    __syncthreads();
+#pragma unroll
+                    for (int r = 0; r < NSUB; ++r)
+                        if ((bal[r] >> lane) & 1u)
+                            s_list[buf][base[r] + __popc(bal[r] & ((1u << lane) - 1u))] =
+                                i0 + r * NT + tid;
+                    if (tid == 0) s_nlist[buf] = run;
                 }
                 // ---- share the round's list over the cluster
                 cluster.sync();
-                if (tid < csize) s_wcount[tid] = *cluster.map_shared_rank(&s_nlist[buf], tid);
+                if (tid < csize) s_rcnt[tid] = *cluster.map_shared_rank(&s_nlist[buf], tid);
                 __syncthreads();
-                if (tid == 0) {
-                    int run = 0;
-                    for (int r = 0; r < csize; ++r) {
-                        s_pre[r] = run;
-                        run += s_wcount[r];
-                    }
-                    s_pre[csize] = run;
-                }
-                __syncthreads();
-                const int M = s_pre[csize];
+                int pre[MAXCLUSTER + 1];
+                pre[0] = 0;
+#pragma unroll
+                for (int r = 0; r < MAXCLUSTER; ++r) pre[r + 1] = pre[r] + (r < csize ? s_rcnt[r] : 0);
+                const int M = pre[MAXCLUSTER];
                 const int m0 = (int)(((long long)M * crank) / csize);
                 const int m1 = (int)(((long long)M * (crank + 1)) / csize);
-                auto fetch = [&](int p) {
-                    int r = 0;
-                    while (r + 1 < csize && p >= s_pre[r + 1]) ++r;
-                    return *cluster.map_shared_rank(&s_list[buf][p - s_pre[r]], r);
-                };
-                // ---- evaluate the (time, sub-exposure) pairs of this CTA's share
-                if (n_ss <= NT) {
-                    const int per = NT / n_ss;   // exposure times per batch
-                    for (int l0 = m0; l0 < m1; l0 += per) {
-                        const int nl = min(per, m1 - l0);
-                        if (tid < nl) s_idx[tid] = fetch(l0 + tid);
-                        __syncthreads();
-                        if (tid < nl * n_ss) {
-                            const int l = tid / n_ss, j = tid - l * n_ss;
-                            const double t = times[s_idx[l]] +
-                                             (((double)j + 0.5) * inv_ss - 0.5) * t_exp;
-                            s_buf[tid] = blocked_fraction<T>(sw, v, reduced_phase(sw, t));
+                auto fetch = [&](int p) {   // p-th entry of the cluster-wide list
+                    int r = 0, off = 0;
+#pragma unroll
+                    for (int q = 1; q < MAXCLUSTER; ++q)
+                        if (q < csize && p >= pre[q]) {
+                            r = q;
+                            off = pre[q];
                         }
-                        __syncthreads();
-                        if (tid < nl) {
-                            T sum = T(0);
-                            for (int j = 0; j < n_ss; ++j) sum += s_buf[tid * n_ss + j];
+                    return *cluster.map_shared_rank(&s_list[buf][p - off], r);
+                };
+                // ---- evaluate this CTA's share, each warp on its own (no block barriers)
+                if (G) {
+                    // a warp takes G whole exposures at a time: lane = (exposure slot, sub-exposure)
+                    for (int p0 = m0 + warp * G; p0 < m1; p0 += NW * G) {
+                        const int p = p0 + my_l;
+                        const bool active = (my_l < G) && (p < m1);
+                        int i = 0;
+                        T delta = T(0);
+                        if (active) {
+                            i = fetch(p);
+                            const double t = times[i] + (((double)my_j + 0.5) * inv_ss - 0.5) * t_exp;
+                            delta = blocked_fraction<T>(sw, v, reduced_phase(sw, t));
+                        }
+                        T sum = T(0);   // exposure mean in sub-exposure order (R18)
+                        for (int jj = 0; jj < n_ss; ++jj)
+                            sum += __shfl_sync(0xffffffffu, delta, (lane + jj) & 31);
+                        if (active && my_j == 0) {
                             const T dbar = sum * T(inv_ss);
-                            const int i = s_idx[tid];
                             if (frow) frow[i] = T(1) - dbar;
-                            if (want_chi2) {
-                                const double sg = sigma[i];
-                                const double rr = ((obs[i] - 1.0) + (double)dbar) / sg;
-                                acc += (sg > 0.0 && isfinite(sg)) ? rr * rr : (double)INFINITY;
-                            }
+                            if (want_chi2) acc += residual_sq(obs[i] - 1.0, (double)dbar, sigma[i]);
                         }
                     }
                 } else {
-                    // more sub-exposures than threads: one exposure time per thread, serial in j
-                    for (int l = m0 + tid; l < m1; l += NT) {
-                        const int i = fetch(l);
+                    // more sub-exposures than lanes: one exposure per warp, lanes stride over j
+                    for (int p = m0 + warp; p < m1; p += NW) {
+                        const int i = fetch(p);
+                        const double tc = times[i];
                         T sum = T(0);
-                        for (int j = 0; j < n_ss; ++j) {
-                            const double t = times[i] + (((double)j + 0.5) * inv_ss - 0.5) * t_exp;
+                        for (int j = lane; j < n_ss; j += 32) {
+                            const double t = tc + (((double)j + 0.5) * inv_ss - 0.5) * t_exp;
                             sum += blocked_fraction<T>(sw, v, reduced_phase(sw, t));
                         }
-                        const T dbar = sum * T(inv_ss);
-                        if (frow) frow[i] = T(1) - dbar;
-                        if (want_chi2) {
-                            const double sg = sigma[i];
-                            const double rr = ((obs[i] - 1.0) + (double)dbar) / sg;
-                            acc += (sg > 0.0 && isfinite(sg)) ? rr * rr : (double)INFINITY;
+#pragma unroll
+                        for (int off = 16; off > 0; off >>= 1)
+                            sum += __shfl_xor_sync(0xffffffffu, sum, off);
+                        if (lane == 0) {
+                            const T dbar = sum * T(inv_ss);
+                            if (frow) frow[i] = T(1) - dbar;
+                            if (want_chi2) acc += residual_sq(obs[i] - 1.0, (double)dbar, sigma[i]);
                         }
                     }
                 }
-                __syncthreads();
             }
         }
         // ---- chi^2: CTA sum, then cluster rank 0 adds the partials in rank order over DSMEM
