@@ -39,6 +39,8 @@ GL_DEV float gabs(float x) { return fabsf(x); }
 GL_DEV double gabs(double x) { return fabs(x); }
 GL_DEV float gatan2(float y, float x) { return atan2f(y, x); }
 GL_DEV double gatan2(double y, double x) { return atan2(y, x); }
+GL_DEV float gasin(float x) { return asinf(x); }
+GL_DEV double gasin(double x) { return asin(x); }
 GL_DEV float gacos(float x) { return acosf(x); }
 GL_DEV double gacos(double x) { return acos(x); }
 GL_DEV float gcbrt(float x) { return cbrtf(x); }

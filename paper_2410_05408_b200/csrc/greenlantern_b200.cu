@@ -29,8 +29,8 @@ namespace {
 
 constexpr int NQ32 = 16;   // Gauss-Legendre points per outline arc, fp32 production path
 constexpr int NQ64 = 48;   // ... fp64 validation path
-constexpr int NT = 256;    // threads per CTA
-constexpr int TILE = 1024; // exposure times classified per tile
+constexpr int NT = 128;    // threads per CTA
+constexpr int TILE = 512;  // exposure times classified per tile
 constexpr int MAXCLUSTER = 8;
 
 __constant__ double c_phi64[NQ64 / 2], c_om64[NQ64 / 2];
@@ -43,7 +43,7 @@ constexpr double kTwoPi = 6.28318530717958647692;
 // ------------------------------------------------------------------------------------------
 struct Walker {
     // orbit (fp64: phases and Kepler's equation are always double)
-    double t0, inv_P, aR, e, omega, cosi, Mc, sq1pe, sq1me, half_win_phase, vmax;
+    double t0, inv_P, aR, e, omega, cosi, Mc, sq1pe, sq1me, half_win_phase, vmax, reach;
     // projected outline: semi-axes and the rotation into the kernel frame
     double a, b, cpsi, spsi;
     // limb darkening, already divided by the disc-integrated intensity
@@ -59,75 +59,109 @@ struct Walker {
 //   Cxy = dx dy1 = sa^2 r1 r2 + sb^2 r4 r5 + sc^2 r7 r8                               (eq. 12)
 //   det C = (dx dy2)^2 = sa^2 sb^2 r9^2 + sa^2 sc^2 r6^2 + sb^2 sc^2 r3^2             (eq. 13)
 // so its principal axes are the eigenvectors of C: a^2 = larger eigenvalue, b = sqrt(det C)/a.
-__device__ void outline_axes(double sa, double sb, double sc, double zeta, double eta, double xi,
-                             double* a, double* b, double* cpsi, double* spsi) {
-    double sz, cz, se, ce, sx, cx;
-    sincos(zeta, &sz, &cz);
-    sincos(eta, &se, &ce);
-    sincos(xi, &sx, &cx);
+// R = double for the validation path; float for the production path, whose per-walker constants
+// are narrowed to fp32 anyway (relative 1e-7 on a, b, psi: < 1e-8 in flux).
+template <typename R>
+__device__ void outline_axes(R sa, R sb, R sc, R zeta, R eta, R xi, R* a, R* b, R* cpsi, R* spsi) {
+    R sz, cz, se, ce, sx, cx;
+    glc::gsincos(zeta, &sz, &cz);
+    glc::gsincos(eta, &se, &ce);
+    glc::gsincos(xi, &sx, &cx);
     // rows of Rx(zeta) Ry(eta) Rz(xi)
-    const double r1 = ce * cx, r2 = -ce * sx, r3 = se;
-    const double r4 = cz * sx + sz * se * cx, r5 = cz * cx - sz * se * sx, r6 = -sz * ce;
-    const double r7 = sz * sx - cz * se * cx, r8 = sz * cx + cz * se * sx, r9 = cz * ce;
-    const double A2 = sa * sa, B2 = sb * sb, C2 = sc * sc;
-    const double Cxx = A2 * r1 * r1 + B2 * r4 * r4 + C2 * r7 * r7;
-    const double Cxy = A2 * r1 * r2 + B2 * r4 * r5 + C2 * r7 * r8;
-    const double Cyy = A2 * r2 * r2 + B2 * r5 * r5 + C2 * r8 * r8;
-    const double det = A2 * B2 * r9 * r9 + A2 * C2 * r6 * r6 + B2 * C2 * r3 * r3;
-    const double hd = 0.5 * (Cxx - Cyy);
-    const double rad = sqrt(hd * hd + Cxy * Cxy);
-    const double lam = 0.5 * (Cxx + Cyy) + rad;
-    *a = sqrt(lam);
-    *b = sqrt(det) / *a;
-    double psi = (rad > 0.0) ? 0.5 * atan2(Cxy, hd) : 0.0;
-    sincos(psi, spsi, cpsi);
+    const R r1 = ce * cx, r2 = -ce * sx, r3 = se;
+    const R r4 = cz * sx + sz * se * cx, r5 = cz * cx - sz * se * sx, r6 = -sz * ce;
+    const R r7 = sz * sx - cz * se * cx, r8 = sz * cx + cz * se * sx, r9 = cz * ce;
+    const R A2 = sa * sa, B2 = sb * sb, C2 = sc * sc;
+    const R Cxx = A2 * r1 * r1 + B2 * r4 * r4 + C2 * r7 * r7;
+    const R Cxy = A2 * r1 * r2 + B2 * r4 * r5 + C2 * r7 * r8;
+    const R Cyy = A2 * r2 * r2 + B2 * r5 * r5 + C2 * r8 * r8;
+    const R det = A2 * B2 * r9 * r9 + A2 * C2 * r6 * r6 + B2 * C2 * r3 * r3;
+    const R hd = R(0.5) * (Cxx - Cyy);
+    const R rad = glc::gsqrt(hd * hd + Cxy * Cxy);
+    const R lam = R(0.5) * (Cxx + Cyy) + rad;
+    *a = glc::gsqrt(lam);
+    *b = glc::gsqrt(det) / *a;
+    const R psi = (rad > R(0)) ? R(0.5) * glc::gatan2(Cxy, hd) : R(0);
+    glc::gsincos(psi, spsi, cpsi);
 }
 
-__device__ void walker_prelude(const double* __restrict__ p, double t_exp, Walker* w) {
-    const double t0 = p[0], P = p[1], aR = p[2], b = p[3], e = p[4], om = p[5];
-    const double Rp = p[6], f = p[7], xi = p[8], eta = p[9], u1 = p[10], u2 = p[11];
+__device__ __forceinline__ bool walker_valid(const double* __restrict__ p) {
+    const double P = p[1], aR = p[2], b = p[3], e = p[4], om = p[5];
+    const double Rp = p[6], f = p[7], u1 = p[10], u2 = p[11];
     bool ok = true;
     for (int k = 0; k < GL_NPARAMS; ++k) ok = ok && isfinite(p[k]);
     const double norm = 1.0 - u1 / 3.0 - u2 / 6.0;
     ok = ok && (P > 0.0) && (e >= 0.0) && (e < 1.0) && (Rp > 0.0) && (Rp < 0.5) && (f >= 0.0) &&
-         (f < 1.0) && (aR * (1.0 - e) > 1.0) && (norm > 0.0) &&
-         (fabs(b) * (1.0 + e * sin(om)) <= aR * (1.0 - e * e));
+         (f < 1.0) && (aR * (1.0 - e) > 1.0) && (norm > 0.0);
+    if (ok) ok = (e == 0.0) ? (fabs(b) <= aR) : (fabs(b) * (1.0 + e * sin(om)) <= aR * (1.0 - e * e));
+    return ok;
+}
+
+// The prelude is split in two independent halves so that two warps can run them side by side:
+// ORBIT (validity, phase constants, cos i, transit window, Kepler constants) and SHAPE (projected
+// outline, limb-darkening constants).  R as in outline_axes.
+template <typename R>
+__device__ void walker_prelude_orbit(const double* __restrict__ p, double t_exp, Walker* w) {
+    const bool ok = walker_valid(p);
     w->valid = ok ? 1 : 0;
     if (!ok) return;
+    const double t0 = p[0], P = p[1], aR = p[2], b = p[3], e = p[4], om = p[5], Rp = p[6];
     w->t0 = t0;
     w->inv_P = 1.0 / P;
     w->aR = aR;
     w->e = e;
     w->omega = om;
-    // R7: conjunction at true anomaly pi/2 - omega; cos i from the impact parameter
-    const double nuc = 0.5 * kPi - om;
-    const double s1 = sqrt(1.0 + e), s2 = sqrt(1.0 - e);
-    const double Ec = 2.0 * atan2(s2 * sin(0.5 * nuc), s1 * cos(0.5 * nuc));
-    w->Mc = Ec - e * sin(Ec);
-    w->sq1pe = s1;
-    w->sq1me = s2;
-    w->cosi = (b / aR) * (1.0 + e * sin(om)) / (1.0 - e * e);
-    // oblate spheroid: polar semi-axis Rp (1-f) along x', equatorial Rp; zeta = 0 (R4, R5)
-    outline_axes(Rp * (1.0 - f), Rp, Rp, 0.0, eta, xi, &w->a, &w->b, &w->cpsi, &w->spsi);
-    const double pn = kPi * norm;
-    w->k0 = (1.0 - u1 - 2.0 * u2) / pn;
-    w->k1 = (u1 + 2.0 * u2) / pn;
-    w->k2 = u2 / pn;
-    // transit window.  e = 0: the centre is within 1 + a of the star centre iff
-    //   sin^2(phi) < [((1+a)/aR)^2 - cos^2 i] / sin^2 i  and cos(phi) > 0;
-    // stored as a half-width in orbital phase, widened by half an exposure.
-    const double reach = (1.0 + w->a) * (1.0 + 1e-12);
+    // the projected semi-major axis of an oblate spheroid is its equatorial radius: the window
+    // does not have to wait for the SHAPE half
+    const bool lowp = sizeof(R) == 4;
+    const double reach = (1.0 + Rp) * (lowp ? 1.0 + 1e-5 : 1.0 + 1e-12);
     double hw = -1.0;   // < 0: never in transit
     if (e == 0.0) {
-        const double ci2 = w->cosi * w->cosi;
-        const double S2 = ((reach / aR) * (reach / aR) - ci2) / (1.0 - ci2);
-        if (S2 > 0.0) hw = (S2 >= 1.0) ? 0.25 : asin(sqrt(S2)) / kTwoPi;
-        if (hw >= 0.0) hw += 0.5 * t_exp * w->inv_P + 1e-13;
+        // PAPER.md:85-87 eqs. 9-10: the centre is within `reach` of the star centre iff
+        //   sin^2(phi) < [(reach/aR)^2 - cos^2 i] / sin^2 i  and cos(phi) > 0;
+        // stored as a half-width in orbital phase, widened by half an exposure.
+        w->cosi = b / aR;
+        w->Mc = 0.0;
+        w->sq1pe = w->sq1me = 1.0;
+        const R ci2 = R(w->cosi) * R(w->cosi), q = R(reach) / R(aR);
+        const R S2 = (q * q - ci2) / (R(1) - ci2);
+        if (S2 > R(0))
+            hw = (S2 >= R(1)) ? 0.25
+                              : (double)(glc::gasin(glc::gsqrt(S2)) * R(0.15915494309189535)) *
+                                    (lowp ? 1.0 + 1e-5 : 1.0);
+        if (hw >= 0.0) hw += 0.5 * t_exp * w->inv_P + (lowp ? 1e-9 : 1e-13);
+        w->vmax = kTwoPi * w->inv_P * aR;
+    } else {
+        // R7: conjunction at true anomaly pi/2 - omega; cos i from the impact parameter
+        const double nuc = 0.5 * kPi - om;
+        const double s1 = sqrt(1.0 + e), s2 = sqrt(1.0 - e);
+        const double Ec = 2.0 * atan2(s2 * sin(0.5 * nuc), s1 * cos(0.5 * nuc));
+        w->Mc = Ec - e * sin(Ec);
+        w->sq1pe = s1;
+        w->sq1me = s2;
+        w->cosi = (b / aR) * (1.0 + e * sin(om)) / (1.0 - e * e);
+        // largest sky-plane speed (periastron), in stellar radii per time unit: bounds how far
+        // the centre moves within half an exposure (window test of eccentric orbits)
+        w->vmax = kTwoPi * w->inv_P * aR * s1 / s2;
     }
     w->half_win_phase = hw;
-    // largest sky-plane speed (periastron), in stellar radii per time unit: bounds how far the
-    // centre moves within half an exposure (window test of eccentric orbits)
-    w->vmax = kTwoPi * w->inv_P * aR * s1 / s2;
+    w->reach = reach;
+}
+
+template <typename R>
+__device__ void walker_prelude_shape(const double* __restrict__ p, Walker* w) {
+    const double Rp = p[6], f = p[7], xi = p[8], eta = p[9], u1 = p[10], u2 = p[11];
+    // oblate spheroid: polar semi-axis Rp (1-f) along x', equatorial Rp; zeta = 0 (R4, R5)
+    R a, b, cpsi, spsi;
+    outline_axes<R>(R(Rp * (1.0 - f)), R(Rp), R(Rp), R(0), R(eta), R(xi), &a, &b, &cpsi, &spsi);
+    w->a = a;
+    w->b = b;
+    w->cpsi = cpsi;
+    w->spsi = spsi;
+    const R pn = R(kPi * (1.0 - u1 / 3.0 - u2 / 6.0));
+    w->k0 = R(1.0 - u1 - 2.0 * u2) / pn;
+    w->k1 = R(u1 + 2.0 * u2) / pn;
+    w->k2 = R(u2) / pn;
 }
 
 // ------------------------------------------------------------------------------------------
@@ -266,13 +300,27 @@ __device__ __forceinline__ double block_sum(double v, double* warp_scratch) {
 // cluster.  Lists are double-buffered, so one barrier per round is enough.
 // ------------------------------------------------------------------------------------------
 // Residual^2 of one exposure against the data (R19); a bad sigma poisons the walker's chi^2.
+// fp64 path: IEEE division.  fp32 path: 1/sigma from the MUFU reciprocal of float(sigma) refined by
+// two Newton steps in fp64 (2^-22 -> 2^-44 -> 2^-88 relative), 4 DFMA instead of a ~30-instruction
+// division; sigmas outside the comfortable float range take the division.
+template <typename T>
 __device__ __forceinline__ double residual_sq(double obs_m1, double delta, double sg) {
+    if (sizeof(T) == 4) {
+        const float sf = (float)sg;
+        if (sf > 1e-30f && sf < 1e30f) {
+            double r = (double)glf::mufu_rcp(sf);
+            r = fma(r, fma(-sg, r, 1.0), r);
+            r = fma(r, fma(-sg, r, 1.0), r);
+            const double rr = (obs_m1 + delta) * r;
+            return rr * rr;
+        }
+    }
     const double rr = (obs_m1 + delta) / sg;
     return (sg > 0.0 && isfinite(sg)) ? rr * rr : (double)INFINITY;
 }
 
 template <typename T>
-__global__ void __launch_bounds__(NT, sizeof(T) == 4 ? 4 : 1)
+__global__ void __launch_bounds__(NT, sizeof(T) == 4 ? 8 : 2)
 transit_kernel(const double* __restrict__ params, int B, const double* __restrict__ times, int nT,
                double t_exp, int n_ss, const double* __restrict__ obs,
                const double* __restrict__ sigma, T* __restrict__ flux, T* __restrict__ chi2) {
@@ -287,7 +335,8 @@ transit_kernel(const double* __restrict__ params, int B, const double* __restric
     __shared__ int s_cnt[NSUB * NW];  // in-window count per (sub-chunk, warp) of the tile
     __shared__ int s_rcnt[MAXCLUSTER];   // list lengths of the cluster's CTAs, this round
     __shared__ double s_red[NW];
-    __shared__ double s_partial;   // this CTA's chi^2 partial, read by cluster rank 0 via DSMEM
+    __shared__ double s_partial[2];   // this CTA's chi^2 partial (per walker parity), read by
+                                      // cluster rank 0 via DSMEM
 
     const double inv_ss = 1.0 / (double)n_ss;
     const int round_span = csize * TILE;
@@ -296,11 +345,12 @@ transit_kernel(const double* __restrict__ params, int B, const double* __restric
     // lane -> (exposure slot l, sub-exposure j) when a warp holds G = 32 / n_ss whole exposures
     const int G = n_ss <= 32 ? 32 / n_ss : 0;
     const int my_l = G ? lane / n_ss : 0, my_j = G ? lane - my_l * n_ss : lane;
-    int buf = 0;
+    int buf = 0, wpar = 0;
 
     for (int wk = blockIdx.y; wk < B; wk += gridDim.y) {
         __syncthreads();
-        if (tid == 0) walker_prelude(params + (size_t)wk * GL_NPARAMS, t_exp, &sw);
+        if (tid == 0) walker_prelude_orbit<T>(params + (size_t)wk * GL_NPARAMS, t_exp, &sw);
+        if (tid == 32) walker_prelude_shape<T>(params + (size_t)wk * GL_NPARAMS, &sw);
         __syncthreads();
         const bool valid = sw.valid != 0;
         double acc = 0.0;   // this thread's chi^2 terms
@@ -314,7 +364,7 @@ transit_kernel(const double* __restrict__ params, int B, const double* __restric
             const WalkerT<T> v = narrow<T>(sw);
             const bool circ = v.circular;
             const double hwin = sw.half_win_phase;
-            const double reach = (1.0 + sw.a) * (1.0 + 1e-12) + 0.5 * t_exp * sw.vmax;
+            const double reach = sw.reach + 0.5 * t_exp * sw.vmax;
             for (int round = 0; round < nrounds; ++round, buf ^= 1) {
                 const int i0 = (round * csize + crank) * TILE;
                 // ---- classify TILE exposure times against the transit window
@@ -334,7 +384,7 @@ transit_kernel(const double* __restrict__ params, int B, const double* __restric
                         }
                         if (!inwin) {
                             if (frow) frow[i] = T(1);
-                            if (want_chi2) acc += residual_sq(obs[i] - 1.0, 0.0, sigma[i]);
+                            if (want_chi2) acc += residual_sq<T>(obs[i] - 1.0, 0.0, sigma[i]);
                         }
                     }
                     bal[r] = __ballot_sync(0xffffffffu, inwin);
@@ -365,8 +415,6 @@ transit_kernel(const double* __restrict__ params, int B, const double* __restric
 #pragma unroll
                 for (int r = 0; r < MAXCLUSTER; ++r) pre[r + 1] = pre[r] + (r < csize ? s_rcnt[r] : 0);
                 const int M = pre[MAXCLUSTER];
-                const int m0 = (int)(((long long)M * crank) / csize);
-                const int m1 = (int)(((long long)M * (crank + 1)) / csize);
                 auto fetch = [&](int p) {   // p-th entry of the cluster-wide list
                     int r = 0, off = 0;
 #pragma unroll
@@ -377,12 +425,15 @@ transit_kernel(const double* __restrict__ params, int B, const double* __restric
                         }
                     return *cluster.map_shared_rank(&s_list[buf][p - off], r);
                 };
-                // ---- evaluate this CTA's share, each warp on its own (no block barriers)
+                // ---- evaluate the round's list: the cluster's warps take groups of exposures in
+                // turn (interleaved, so that ingress and egress are spread over every warp), each
+                // warp on its own (no block barriers)
+                const int gwarp = crank * NW + warp, gstride = csize * NW;
                 if (G) {
                     // a warp takes G whole exposures at a time: lane = (exposure slot, sub-exposure)
-                    for (int p0 = m0 + warp * G; p0 < m1; p0 += NW * G) {
+                    for (int p0 = gwarp * G; p0 < M; p0 += gstride * G) {
                         const int p = p0 + my_l;
-                        const bool active = (my_l < G) && (p < m1);
+                        const bool active = (my_l < G) && (p < M);
                         int i = 0;
                         T delta = T(0);
                         if (active) {
@@ -396,12 +447,12 @@ transit_kernel(const double* __restrict__ params, int B, const double* __restric
                         if (active && my_j == 0) {
                             const T dbar = sum * T(inv_ss);
                             if (frow) frow[i] = T(1) - dbar;
-                            if (want_chi2) acc += residual_sq(obs[i] - 1.0, (double)dbar, sigma[i]);
+                            if (want_chi2) acc += residual_sq<T>(obs[i] - 1.0, (double)dbar, sigma[i]);
                         }
                     }
                 } else {
                     // more sub-exposures than lanes: one exposure per warp, lanes stride over j
-                    for (int p = m0 + warp; p < m1; p += NW) {
+                    for (int p = gwarp; p < M; p += gstride) {
                         const int i = fetch(p);
                         const double tc = times[i];
                         T sum = T(0);
@@ -415,23 +466,25 @@ transit_kernel(const double* __restrict__ params, int B, const double* __restric
                         if (lane == 0) {
                             const T dbar = sum * T(inv_ss);
                             if (frow) frow[i] = T(1) - dbar;
-                            if (want_chi2) acc += residual_sq(obs[i] - 1.0, (double)dbar, sigma[i]);
+                            if (want_chi2) acc += residual_sq<T>(obs[i] - 1.0, (double)dbar, sigma[i]);
                         }
                     }
                 }
             }
         }
-        // ---- chi^2: CTA sum, then cluster rank 0 adds the partials in rank order over DSMEM
+        // ---- chi^2: CTA sum, then cluster rank 0 adds the partials in rank order over DSMEM.
+        // s_partial alternates between two slots, so the barrier of the NEXT walker (or the one at
+        // kernel exit) is what keeps a slot alive until rank 0 has read it.
         if (want_chi2) {
             const double tot = block_sum(acc, s_red);
-            if (tid == 0) s_partial = tot;
+            if (tid == 0) s_partial[wpar] = tot;
             cluster.sync();
             if (crank == 0 && tid == 0) {
                 double c2 = 0.0;
-                for (int r = 0; r < csize; ++r) c2 += *cluster.map_shared_rank(&s_partial, r);
+                for (int r = 0; r < csize; ++r) c2 += *cluster.map_shared_rank(&s_partial[wpar], r);
                 chi2[wk] = valid ? T(c2) : T(INFINITY);
             }
-            cluster.sync();   // keep every CTA's shared memory alive until rank 0 has read it
+            wpar ^= 1;
         }
     }
     cluster.sync();   // no CTA may exit while a neighbour can still read its lists
@@ -515,8 +568,9 @@ int ensure_tables() {
 // Cluster size: enough CTAs per walker that the batch fills the GPU, at most one tile each.
 int pick_cluster(int B, int nT) {
     const int ntiles = (nT + TILE - 1) / TILE;
+    const long long slots = 148LL * 16;   // CTAs of 128 threads x 64 registers resident on a B200
     int c = 1;
-    while (c < MAXCLUSTER && c * 2 <= ntiles && (long long)B * c < 4LL * 148) c *= 2;
+    while (c < MAXCLUSTER && c * 2 <= ntiles && (long long)B * c * 2 <= slots) c *= 2;
     return c;
 }
 
