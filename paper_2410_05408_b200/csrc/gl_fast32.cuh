@@ -99,25 +99,33 @@ template <bool CLAMP> GLF_DEV float pair_term(float m2p, float fp, float m2q, fl
     return fmaf(Wp, fp, Wq * fq);
 }
 
-// Integral over the WHOLE outline of W(r^2) (2 f_flat) dt by the N-point trapezoid rule, N = 8, 16
-// or 32.  2 f_flat = ab + u cos t + v sin t with u = b xc, v = a yc (gl_core.cuh).  Nodes k and k+N/2
-// are mirror images, so each table entry serves two nodes.
-template <int N, bool CLAMP>
-GLF_DEV float whole_outline_lin(float xc, float yc, float a, float b, float ab,
-                                                   float u, float v) {
-    constexpr int STRIDE = 32 / N;
+// Integral over the WHOLE outline of W(r^2) (2 f_flat) dt by the N-point trapezoid rule, N = 2 nh,
+// nh = 4, 8 or 16 chosen PER LANE: one loop serves every tier, so a warp whose lanes need
+// different orders runs the longest one once instead of one code copy per tier.
+// 2 f_flat = ab + u cos t + v sin t with u = b xc, v = a yc (gl_core.cuh).  Nodes k and k + N/2 are
+// mirror images, so each table entry serves two nodes.  trap[k] = (cos, sin)(2 pi k / 32), k < 16:
+// a copy of c_trap_cos/sin that the caller keeps in SHARED memory (per-lane strides would
+// serialise in the constant cache).
+struct TrapNode {
+    float c, s;
+};
+GLF_DEV float whole_outline_lin(const TrapNode* trap, int nh, float xc, float yc, float a, float b,
+                                float ab, float u, float v) {
+    const int stride = 16 / nh;
     float acc = 0.f;
+    for (int k0 = 0; k0 < nh; k0 += 4) {
 #pragma unroll
-    for (int k = 0; k < N / 2; ++k) {
-        const float c = c_trap_cos[k * STRIDE], s = c_trap_sin[k * STRIDE];
-        const float p = a * c, q = b * s;
-        const float xp = xc + p, yp = yc + q, xq = xc - p, yq = yc - q;
-        const float m2p = fmaf(-xp, xp, fmaf(-yp, yp, 1.f));
-        const float m2q = fmaf(-xq, xq, fmaf(-yq, yq, 1.f));
-        const float w = fmaf(u, c, v * s);
-        acc += pair_term<CLAMP>(m2p, ab + w, m2q, ab - w);
+        for (int kk = 0; kk < 4; ++kk) {
+            const TrapNode nd = trap[(k0 + kk) * stride];
+            const float p = a * nd.c, q = b * nd.s;
+            const float xp = xc + p, yp = yc + q, xq = xc - p, yq = yc - q;
+            const float m2p = fmaf(-xp, xp, fmaf(-yp, yp, 1.f));
+            const float m2q = fmaf(-xq, xq, fmaf(-yq, yq, 1.f));
+            const float w = fmaf(u, nd.c, v * nd.s);
+            acc += pair_term<true>(m2p, ab + w, m2q, ab - w);
+        }
     }
-    return acc * (kTwoPiF / float(N));
+    return acc * (kPiF / float(nh));
 }
 
 // The outline in the kernel frame, re-parametrised by tau = t - t_far (t_far = the outline point
@@ -197,47 +205,43 @@ GLF_DEV void critical_point(float xc, float yc, float a, float b, float* c,
 // Blocked fraction delta = k0 A_flat + k1 A_lin + k2 A_quad for an outline with centre (xc, yc) in
 // the kernel frame (any signs), semi-axes a >= b > 0, a < 1/2.  k0, k1, k2 = c0, c1, c2 of R8 divided
 // by pi (1 - u1/3 - u2/6).  Returns 0 when the overlap is empty.
-GLF_DEV float blocked_f32(float xc_in, float yc_in, float a, float b, float k0,
-                                             float k1, float k2) {
+GLF_DEV float blocked_f32(const TrapNode* trap, float xc_in, float yc_in, float a, float b, float k0,
+                          float k1, float k2) {
     const float xc = fabsf(xc_in), yc = fabsf(yc_in);   // mirror images have the same areas
     const float r0sq = fmaf(xc, xc, yc * yc);
     const float reach = 1.f + a;
     if (r0sq >= reach * reach) return 0.f;
     const float ab = a * b, u = b * xc, v = a * yc;
     const float e2 = (a - b) * (a + b);
-    // whole-outline closed forms: A_flat = pi a b, A_quad = pi a b (r0^2 + (a^2 + b^2)/4)
-    const float in_flat = kPiF * ab;
-    const float in_quad = in_flat * fmaf(0.25f, fmaf(a, a, b * b), r0sq);
     const float r0 = r0sq * mufu_rsqrt(fmaxf(r0sq, 1e-30f));
+    const float Aa = a * xc, Bb = b * yc;
+    // nh = half the trapezoid order for an outline wholly inside the disc, 0 = not (yet) known to be
+    int nh = 0;
+    float cf = 1.f, sf = 0.f, gfar = 0.f;
     if (r0 + a <= 0.99f) {
         // well inside the limb (gap >= 0.01): 16 fixed nodes; 8 once the gap exceeds the semi-major
         // axis or 0.3 (error <= 6e-9 in flux on the config-5 sample)
-        const float lin = (r0 + a + a <= 1.f || r0 + a <= 0.7f)
-                              ? whole_outline_lin<8, false>(xc, yc, a, b, ab, u, v)
-                              : whole_outline_lin<16, false>(xc, yc, a, b, ab, u, v);
-        return fmaf(k0, in_flat, fmaf(k1 * (1.f / 3.f), lin, k2 * in_quad));
-    }
-    const float Aa = a * xc, Bb = b * yc;
-    if (Aa < e2 && Bb < e2) {
+        nh = (r0 + a + a <= 1.f || r0 + a <= 0.7f) ? 4 : 8;
+    } else if (Aa < e2 && Bb < e2) {
         // the star centre may lie inside the evolute (up to four crossings): bracketed search
         float A[3];
         if (!glc::overlap_areas<float, 16>(xc, yc, a, b, c_gl_phi, c_gl_om, A)) return 0.f;
         return fmaf(k0, A[0], fmaf(k1, A[1], k2 * A[2]));
-    }
-    // farthest outline point from the star centre: the only maximum of g (first quadrant)
-    float cf, sf;
-    {
+    } else {
+        // farthest outline point from the star centre: the only maximum of g (first quadrant)
         const float rn = mufu_rsqrt(fmaf(Aa, Aa, Bb * Bb));   // Aa, Bb not both 0 here (r0 > 0.49)
         cf = Aa * rn;
         sf = Bb * rn;
         critical_point<1>(xc, yc, a, b, &cf, &sf, 1.f, 1.f);
+        const float xf = fmaf(a, cf, xc), yf = fmaf(b, sf, yc);
+        gfar = fmaf(xf, xf, fmaf(yf, yf, -1.f));
+        if (gfar <= 0.f) nh = (gfar < -0.04f) ? 8 : 16;   // wholly inside, close to the limb
     }
-    const float xf = fmaf(a, cf, xc), yf = fmaf(b, sf, yc);
-    const float gfar = fmaf(xf, xf, fmaf(yf, yf, -1.f));
-    if (gfar <= 0.f) {
-        // wholly inside, close to the limb
-        const float lin = (gfar < -0.04f) ? whole_outline_lin<16, false>(xc, yc, a, b, ab, u, v)
-                                          : whole_outline_lin<32, true>(xc, yc, a, b, ab, u, v);
+    if (nh) {
+        // whole-outline closed forms: A_flat = pi a b, A_quad = pi a b (r0^2 + (a^2 + b^2)/4)
+        const float in_flat = kPiF * ab;
+        const float in_quad = in_flat * fmaf(0.25f, fmaf(a, a, b * b), r0sq);
+        const float lin = whole_outline_lin(trap, nh, xc, yc, a, b, ab, u, v);
         return fmaf(k0, in_flat, fmaf(k1 * (1.f / 3.f), lin, k2 * in_quad));
     }
     // the outline crosses the limb twice (or misses the disc).  tau = t - t_far in [0, 2 pi).

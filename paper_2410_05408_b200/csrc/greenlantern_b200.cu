@@ -15,6 +15,7 @@
 #include <math.h>
 #include <stdint.h>
 #include <stdio.h>
+#include <stdlib.h>
 
 #include <mutex>
 
@@ -25,12 +26,35 @@
 
 namespace cg = cooperative_groups;
 
+// Development aid (off unless built with -DGL_TIMELINE): per-CTA phase timestamps of transit_kernel.
+#ifdef GL_TIMELINE
+__device__ long long g_timeline[8192 * 8];
+#define GL_TL(k)                                                                          \
+    do {                                                                                  \
+        const unsigned cta_ = blockIdx.y * gridDim.x + blockIdx.x;                        \
+        if (cta_ < 8192 && (threadIdx.x & 31) == 0) {                                     \
+            long long t_;                                                                 \
+            asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t_));                        \
+            atomicMax((unsigned long long*)&g_timeline[cta_ * 8 + (k)], (unsigned long long)t_); \
+        }                                                                                 \
+    } while (0)
+extern "C" int gl_debug_timeline(long long* host_out, int reset) {
+    if (reset) {
+        static long long zeros[8192 * 8];
+        return (int)cudaMemcpyToSymbol(g_timeline, zeros, sizeof(zeros));
+    }
+    return (int)cudaMemcpyFromSymbol(host_out, g_timeline, sizeof(long long) * 8192 * 8);
+}
+#else
+#define GL_TL(k) do { } while (0)
+#endif
+
 namespace {
 
 constexpr int NQ32 = 16;   // Gauss-Legendre points per outline arc, fp32 production path
 constexpr int NQ64 = 48;   // ... fp64 validation path
 constexpr int NT = 128;    // threads per CTA
-constexpr int TILE = 512;  // exposure times classified per tile
+constexpr int MAXTILE = 32 * NT;   // exposure times one CTA classifies per round, at most
 constexpr int MAXCLUSTER = 8;
 
 __constant__ double c_phi64[NQ64 / 2], c_om64[NQ64 / 2];
@@ -238,22 +262,26 @@ template <typename T> __device__ __forceinline__ WalkerT<T> narrow(const Walker&
 
 // a3 + a4 for an outline centred at (xc, yc) in the kernel frame: fp64 = generic bracketed search +
 // 48-point rule (validation), fp32 = gl_fast32.cuh (production).
-template <typename T> __device__ __forceinline__ T blocked_at(T xc, T yc, T a, T b, T k0, T k1, T k2);
-template <> __device__ __forceinline__ double blocked_at<double>(double xc, double yc, double a,
-                                                                 double b, double k0, double k1,
-                                                                 double k2) {
+template <typename T>
+__device__ __forceinline__ T blocked_at(const glf::TrapNode* trap, T xc, T yc, T a, T b, T k0, T k1,
+                                        T k2);
+template <> __device__ __forceinline__ double blocked_at<double>(const glf::TrapNode*, double xc,
+                                                                 double yc, double a, double b,
+                                                                 double k0, double k1, double k2) {
     double A[3];
     if (!glc::overlap_areas<double, NQ64>(xc, yc, a, b, c_phi64, c_om64, A)) return 0.0;
     return k0 * A[0] + k1 * A[1] + k2 * A[2];
 }
-template <> __device__ __forceinline__ float blocked_at<float>(float xc, float yc, float a, float b,
-                                                               float k0, float k1, float k2) {
-    return glf::blocked_f32(xc, yc, a, b, k0, k1, k2);
+template <> __device__ __forceinline__ float blocked_at<float>(const glf::TrapNode* trap, float xc,
+                                                               float yc, float a, float b, float k0,
+                                                               float k1, float k2) {
+    return glf::blocked_f32(trap, xc, yc, a, b, k0, k1, k2);
 }
 
 // Blocked fraction delta = 1 - F_inst at reduced phase ph (a1 + a3 + a4).
 template <typename T>
-__device__ __forceinline__ T blocked_fraction(const Walker& w, const WalkerT<T>& v, double ph) {
+__device__ __forceinline__ T blocked_fraction(const glf::TrapNode* trap, const Walker& w,
+                                              const WalkerT<T>& v, double ph) {
     T x0, y0;
     if (v.circular) {
         // phi = 2 pi ph, |ph| <= 1/2; narrowed AFTER the fp64 phase reduction
@@ -269,7 +297,7 @@ __device__ __forceinline__ T blocked_fraction(const Walker& w, const WalkerT<T>&
         y0 = T(Y);
     }
     const T xc = v.cpsi * x0 + v.spsi * y0, yc = v.cpsi * y0 - v.spsi * x0;
-    return blocked_at<T>(xc, yc, v.a, v.b, v.k0, v.k1, v.k2);
+    return blocked_at<T>(trap, xc, yc, v.a, v.b, v.k0, v.k1, v.k2);
 }
 
 // ------------------------------------------------------------------------------------------
@@ -292,66 +320,84 @@ __device__ __forceinline__ double block_sum(double v, double* warp_scratch) {
 // The fused kernel.  grid = (cluster size C, walkers in flight); cluster = (C, 1, 1).
 //   flux  : [B, T] of T-typed values or nullptr          chi2 : [B] or nullptr
 //   obs, sigma : [T] fp64 or nullptr (only read when chi2 != nullptr)
-// Per walker the exposure times are taken in rounds of C * TILE: CTA r classifies tile r of the
-// round against the transit window (out-of-window times are finished on the spot), compacts the
-// in-window indices into its own shared list, and after ONE cluster barrier every CTA takes an
-// equal share of the round's whole in-window list, reading the other CTAs' lists over DSMEM.
-// A K2-shaped series (1 % in transit, all of it inside one tile) is thereby spread over the whole
-// cluster.  Lists are double-buffered, so one barrier per round is enough.
+// Per walker the exposure times are taken in rounds of C tiles (one round unless T > C * 4096):
+// CTA r classifies tile r against the transit window -- out-of-window exposures are finished on
+// the spot (flux = 1, baseline residual) -- and compacts the in-window indices into its own
+// shared list; after ONE cluster barrier the cluster's warps take groups of in-window exposures
+// in turn, reading the other CTAs' lists over DSMEM.  A K2-shaped series (1 % in transit, all of
+// it inside one tile) is thereby spread over the whole cluster, and ingress/egress (the expensive
+// geometries) over every warp.
 // ------------------------------------------------------------------------------------------
-// Residual^2 of one exposure against the data (R19); a bad sigma poisons the walker's chi^2.
-// fp64 path: IEEE division.  fp32 path: 1/sigma from the MUFU reciprocal of float(sigma) refined by
-// two Newton steps in fp64 (2^-22 -> 2^-44 -> 2^-88 relative), 4 DFMA instead of a ~30-instruction
-// division; sigmas outside the comfortable float range take the division.
-template <typename T>
-__device__ __forceinline__ double residual_sq(double obs_m1, double delta, double sg) {
-    if (sizeof(T) == 4) {
-        const float sf = (float)sg;
-        if (sf > 1e-30f && sf < 1e30f) {
-            double r = (double)glf::mufu_rcp(sf);
-            r = fma(r, fma(-sg, r, 1.0), r);
-            r = fma(r, fma(-sg, r, 1.0), r);
-            const double rr = (obs_m1 + delta) * r;
-            return rr * rr;
-        }
-    }
+// Residual^2 of one exposure against the data (R19), in the compute type; a bad sigma poisons the
+// walker's chi^2.  fp64 path: IEEE division.  fp32 path: obs - 1 is formed in fp64 and narrowed (it
+// is ~1e-4, so fp32 keeps 7 digits of it), 1/sigma is the MUFU reciprocal plus one Newton step;
+// each term is good to ~2e-7 relative and the terms are summed in fp64 (chi^2 budget: 1e-4).
+template <typename T> __device__ __forceinline__ T residual_sq(double obs_m1, T delta, double sg);
+template <> __device__ __forceinline__ double residual_sq<double>(double obs_m1, double delta,
+                                                                  double sg) {
     const double rr = (obs_m1 + delta) / sg;
     return (sg > 0.0 && isfinite(sg)) ? rr * rr : (double)INFINITY;
+}
+template <> __device__ __forceinline__ float residual_sq<float>(double obs_m1, float delta,
+                                                                double sg) {
+    const float sf = (float)sg;
+    if (sf > 1e-30f && sf < 1e30f) {
+        float r = glf::mufu_rcp(sf);
+        r = r * fmaf(-sf, r, 2.f);
+        const float rr = ((float)obs_m1 + delta) * r;
+        return rr * rr;
+    }
+    return (float)residual_sq<double>(obs_m1, (double)delta, sg);   // out-of-range sigma
 }
 
 template <typename T>
 __global__ void __launch_bounds__(NT, sizeof(T) == 4 ? 8 : 2)
 transit_kernel(const double* __restrict__ params, int B, const double* __restrict__ times, int nT,
-               double t_exp, int n_ss, const double* __restrict__ obs,
+               int tile, double t_exp, int n_ss, const double* __restrict__ obs,
                const double* __restrict__ sigma, T* __restrict__ flux, T* __restrict__ chi2) {
     cg::cluster_group cluster = cg::this_cluster();
     const int crank = (int)cluster.block_rank(), csize = (int)cluster.num_blocks();
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-    constexpr int NW = NT / 32, NSUB = TILE / NT;
+    constexpr int NW = NT / 32;
 
     __shared__ Walker sw;
-    __shared__ int s_list[2][TILE];   // in-window time indices of this CTA's tile (double-buffered)
-    __shared__ int s_nlist[2];
-    __shared__ int s_cnt[NSUB * NW];  // in-window count per (sub-chunk, warp) of the tile
+    __shared__ int s_list[MAXTILE];   // in-window time indices of this CTA's tile
+    __shared__ int s_nlist;
+    __shared__ int s_cnt[NW];         // in-window count per warp of the tile
     __shared__ int s_rcnt[MAXCLUSTER];   // list lengths of the cluster's CTAs, this round
     __shared__ double s_red[NW];
     __shared__ double s_partial[2];   // this CTA's chi^2 partial (per walker parity), read by
                                       // cluster rank 0 via DSMEM
+    __shared__ glf::TrapNode s_trap[16];   // trapezoid nodes (per-lane strides: not constant memory)
+    if (tid < 16) s_trap[tid] = glf::TrapNode{glf::c_trap_cos[tid], glf::c_trap_sin[tid]};
 
     const double inv_ss = 1.0 / (double)n_ss;
-    const int round_span = csize * TILE;
+    const int nsub = tile / NT;   // exposures per thread and tile (<= 32: one mask bit each)
+    const int round_span = csize * tile;
     const int nrounds = (nT + round_span - 1) / round_span;
     const bool want_chi2 = (chi2 != nullptr);
     // lane -> (exposure slot l, sub-exposure j) when a warp holds G = 32 / n_ss whole exposures
     const int G = n_ss <= 32 ? 32 / n_ss : 0;
     const int my_l = G ? lane / n_ss : 0, my_j = G ? lane - my_l * n_ss : lane;
-    int buf = 0, wpar = 0;
+    int wpar = 0;
+    bool lists_live = false;   // uniform over the cluster
 
+    // warm the L2 with this CTA's first tile while the prelude runs (one line = 16 doubles)
+    for (int i = crank * tile + tid * 16; i < min(nT, (crank + 1) * tile); i += NT * 16) {
+        asm volatile("prefetch.global.L2 [%0];" ::"l"(times + i));
+        if (want_chi2) {
+            asm volatile("prefetch.global.L2 [%0];" ::"l"(obs + i));
+            asm volatile("prefetch.global.L2 [%0];" ::"l"(sigma + i));
+        }
+    }
+
+    GL_TL(0);
     for (int wk = blockIdx.y; wk < B; wk += gridDim.y) {
         __syncthreads();
         if (tid == 0) walker_prelude_orbit<T>(params + (size_t)wk * GL_NPARAMS, t_exp, &sw);
         if (tid == 32) walker_prelude_shape<T>(params + (size_t)wk * GL_NPARAMS, &sw);
         __syncthreads();
+        GL_TL(1);
         const bool valid = sw.valid != 0;
         double acc = 0.0;   // this thread's chi^2 terms
         T* frow = flux ? flux + (size_t)wk * nT : nullptr;
@@ -365,12 +411,14 @@ transit_kernel(const double* __restrict__ params, int B, const double* __restric
             const bool circ = v.circular;
             const double hwin = sw.half_win_phase;
             const double reach = sw.reach + 0.5 * t_exp * sw.vmax;
-            for (int round = 0; round < nrounds; ++round, buf ^= 1) {
-                const int i0 = (round * csize + crank) * TILE;
-                // ---- classify TILE exposure times against the transit window
-                unsigned bal[NSUB];
-#pragma unroll
-                for (int r = 0; r < NSUB; ++r) {
+            for (int round = 0; round < nrounds; ++round) {
+                const int i0 = (round * csize + crank) * tile;
+                // ---- pass 1: classify this thread's exposures of the tile against the window;
+                // out-of-window ones are finished here
+                unsigned mask = 0;   // bit r: exposure i0 + r NT + tid is in the window
+                int wcount = 0;
+#pragma unroll 4
+                for (int r = 0; r < nsub; ++r) {
                     const int i = i0 + r * NT + tid;
                     bool inwin = false;
                     if (i < nT) {
@@ -382,38 +430,47 @@ transit_kernel(const double* __restrict__ params, int B, const double* __restric
                             sky_position_f64(sw, ph, &X, &Y);
                             inwin = X * X + Y * Y < reach * reach;
                         }
-                        if (!inwin) {
-                            if (frow) frow[i] = T(1);
-                            if (want_chi2) acc += residual_sq<T>(obs[i] - 1.0, 0.0, sigma[i]);
+                        if (want_chi2) {
+                            const T r2 = residual_sq<T>(obs[i] - 1.0, T(0), sigma[i]);
+                            if (!inwin) acc += (double)r2;
+                        }
+                        if (!inwin && frow) frow[i] = T(1);
+                    }
+                    mask |= (inwin ? 1u : 0u) << r;
+                    wcount += __popc(__ballot_sync(0xffffffffu, inwin));
+                }
+                if (lane == 0) s_cnt[warp] = wcount;
+                // nobody may still be reading the lists of the previous round / walker
+                if (lists_live) cluster.sync(); else __syncthreads();
+                // ---- pass 2: compact the in-window indices into this CTA's list, ordered by
+                // (warp, sub-chunk, lane): fixed for a given launch, so chi^2 is reproducible
+                {
+                    int base = 0, total = 0;
+#pragma unroll
+                    for (int q = 0; q < NW; ++q) {
+                        if (q == warp) base = total;
+                        total += s_cnt[q];
+                    }
+                    if (wcount) {
+                        for (int r = 0; r < nsub; ++r) {
+                            const bool bit = (mask >> r) & 1u;
+                            const unsigned bal = __ballot_sync(0xffffffffu, bit);
+                            if (bit) s_list[base + __popc(bal & ((1u << lane) - 1u))] = i0 + r * NT + tid;
+                            base += __popc(bal);
                         }
                     }
-                    bal[r] = __ballot_sync(0xffffffffu, inwin);
-                    if (lane == 0) s_cnt[r * NW + warp] = __popc(bal[r]);
-                }
-                __syncthreads();
-                // ---- compact the in-window indices into this CTA's list, in index order
-                {
-                    int run = 0, base[NSUB];
-#pragma unroll
-                    for (int q = 0; q < NSUB * NW; ++q) {
-                        if ((q % NW) == warp) base[q / NW] = run;
-                        run += s_cnt[q];
-                    }
-#pragma unroll
-                    for (int r = 0; r < NSUB; ++r)
-                        if ((bal[r] >> lane) & 1u)
-                            s_list[buf][base[r] + __popc(bal[r] & ((1u << lane) - 1u))] =
-                                i0 + r * NT + tid;
-                    if (tid == 0) s_nlist[buf] = run;
+                    if (tid == 0) s_nlist = total;
                 }
                 // ---- share the round's list over the cluster
+                if (round == 0) GL_TL(2);
                 cluster.sync();
-                if (tid < csize) s_rcnt[tid] = *cluster.map_shared_rank(&s_nlist[buf], tid);
-                __syncthreads();
+                lists_live = true;
+                if (round == 0) GL_TL(3);
                 int pre[MAXCLUSTER + 1];
                 pre[0] = 0;
 #pragma unroll
-                for (int r = 0; r < MAXCLUSTER; ++r) pre[r + 1] = pre[r] + (r < csize ? s_rcnt[r] : 0);
+                for (int r = 0; r < MAXCLUSTER; ++r)
+                    pre[r + 1] = pre[r] + (r < csize ? *cluster.map_shared_rank(&s_nlist, r) : 0);
                 const int M = pre[MAXCLUSTER];
                 auto fetch = [&](int p) {   // p-th entry of the cluster-wide list
                     int r = 0, off = 0;
@@ -423,7 +480,7 @@ transit_kernel(const double* __restrict__ params, int B, const double* __restric
                             r = q;
                             off = pre[q];
                         }
-                    return *cluster.map_shared_rank(&s_list[buf][p - off], r);
+                    return *cluster.map_shared_rank(&s_list[p - off], r);
                 };
                 // ---- evaluate the round's list: the cluster's warps take groups of exposures in
                 // turn (interleaved, so that ingress and egress are spread over every warp), each
@@ -439,7 +496,7 @@ transit_kernel(const double* __restrict__ params, int B, const double* __restric
                         if (active) {
                             i = fetch(p);
                             const double t = times[i] + (((double)my_j + 0.5) * inv_ss - 0.5) * t_exp;
-                            delta = blocked_fraction<T>(sw, v, reduced_phase(sw, t));
+                            delta = blocked_fraction<T>(s_trap, sw, v, reduced_phase(sw, t));
                         }
                         T sum = T(0);   // exposure mean in sub-exposure order (R18)
                         for (int jj = 0; jj < n_ss; ++jj)
@@ -447,7 +504,8 @@ transit_kernel(const double* __restrict__ params, int B, const double* __restric
                         if (active && my_j == 0) {
                             const T dbar = sum * T(inv_ss);
                             if (frow) frow[i] = T(1) - dbar;
-                            if (want_chi2) acc += residual_sq<T>(obs[i] - 1.0, (double)dbar, sigma[i]);
+                            if (want_chi2)
+                                acc += (double)residual_sq<T>(obs[i] - 1.0, dbar, sigma[i]);
                         }
                     }
                 } else {
@@ -458,7 +516,7 @@ transit_kernel(const double* __restrict__ params, int B, const double* __restric
                         T sum = T(0);
                         for (int j = lane; j < n_ss; j += 32) {
                             const double t = tc + (((double)j + 0.5) * inv_ss - 0.5) * t_exp;
-                            sum += blocked_fraction<T>(sw, v, reduced_phase(sw, t));
+                            sum += blocked_fraction<T>(s_trap, sw, v, reduced_phase(sw, t));
                         }
 #pragma unroll
                         for (int off = 16; off > 0; off >>= 1)
@@ -466,19 +524,24 @@ transit_kernel(const double* __restrict__ params, int B, const double* __restric
                         if (lane == 0) {
                             const T dbar = sum * T(inv_ss);
                             if (frow) frow[i] = T(1) - dbar;
-                            if (want_chi2) acc += residual_sq<T>(obs[i] - 1.0, (double)dbar, sigma[i]);
+                            if (want_chi2)
+                                acc += (double)residual_sq<T>(obs[i] - 1.0, dbar, sigma[i]);
                         }
                     }
                 }
             }
         }
+        GL_TL(4);
         // ---- chi^2: CTA sum, then cluster rank 0 adds the partials in rank order over DSMEM.
         // s_partial alternates between two slots, so the barrier of the NEXT walker (or the one at
         // kernel exit) is what keeps a slot alive until rank 0 has read it.
         if (want_chi2) {
             const double tot = block_sum(acc, s_red);
+            GL_TL(5);
             if (tid == 0) s_partial[wpar] = tot;
             cluster.sync();
+            lists_live = false;   // every CTA is past its evaluation
+            GL_TL(6);
             if (crank == 0 && tid == 0) {
                 double c2 = 0.0;
                 for (int r = 0; r < csize; ++r) c2 += *cluster.map_shared_rank(&s_partial[wpar], r);
@@ -487,7 +550,8 @@ transit_kernel(const double* __restrict__ params, int B, const double* __restric
             wpar ^= 1;
         }
     }
-    cluster.sync();   // no CTA may exit while a neighbour can still read its lists
+    cluster.sync();   // no CTA may exit while a neighbour can still read its shared memory
+    GL_TL(7);
 }
 
 // ------------------------------------------------------------------------------------------
@@ -498,6 +562,10 @@ transit_kernel(const double* __restrict__ params, int B, const double* __restric
 template <typename T>
 __global__ void __launch_bounds__(NT)
 geometry_kernel(const double* __restrict__ geom, long long N, T* __restrict__ out) {
+    __shared__ glf::TrapNode s_trap[16];
+    if (threadIdx.x < 16)
+        s_trap[threadIdx.x] = glf::TrapNode{glf::c_trap_cos[threadIdx.x], glf::c_trap_sin[threadIdx.x]};
+    __syncthreads();
     const long long k = (long long)blockIdx.x * NT + threadIdx.x;
     if (k >= N) return;
     const double* g = geom + k * GL_NGEOM;
@@ -514,7 +582,7 @@ geometry_kernel(const double* __restrict__ geom, long long N, T* __restrict__ ou
     glc::gsincos(T(pa), &s, &c);
     const T a = T(Rp), b = T(Rp * (1.0 - fp));
     const double pn = kPi * norm;
-    const T delta = blocked_at<T>(T(d) * c, -T(d) * s, a, b, T((1.0 - u1 - 2.0 * u2) / pn),
+    const T delta = blocked_at<T>(s_trap, T(d) * c, -T(d) * s, a, b, T((1.0 - u1 - 2.0 * u2) / pn),
                                   T((u1 + 2.0 * u2) / pn), T(u2 / pn));
     out[k] = T(1) - delta;
 }
@@ -565,20 +633,29 @@ int ensure_tables() {
     return GL_OK;
 }
 
-// Cluster size: enough CTAs per walker that the batch fills the GPU, at most one tile each.
-int pick_cluster(int B, int nT) {
-    const int ntiles = (nT + TILE - 1) / TILE;
-    const long long slots = 148LL * 16;   // CTAs of 128 threads x 64 registers resident on a B200
+// Cluster size C and tile length: as many CTAs per walker as keep the whole batch resident in one
+// wave (8 CTAs of 128 threads x 64 registers per SM, 148 SMs), each with at least NT exposures;
+// the tile is the CTA's share of the series, so that one round covers it unless T > C * MAXTILE.
+void pick_shape(int B, int nT, int* C, int* tile) {
+    const long long slots = 148LL * 8;
     int c = 1;
-    while (c < MAXCLUSTER && c * 2 <= ntiles && (long long)B * c * 2 <= slots) c *= 2;
-    return c;
+    while (c < MAXCLUSTER && (long long)c * 2 * NT <= nT && (long long)B * c * 2 <= slots) c *= 2;
+    if (const char* env = getenv("GL_CLUSTER")) {   // experiments only
+        const int v = atoi(env);
+        if (v == 1 || v == 2 || v == 4 || v == 8) c = v;
+    }
+    int t = ((nT + c - 1) / c + NT - 1) / NT * NT;
+    t = t < NT ? NT : (t > MAXTILE ? MAXTILE : t);
+    *C = c;
+    *tile = t;
 }
 
 template <typename T>
 int launch_transit(const double* params, int B, const double* times, int nT, double t_exp, int n_ss,
                    const double* obs, const double* sigma, void* flux, void* chi2,
                    cudaStream_t st) {
-    const int C = pick_cluster(B, nT);
+    int C, tile;
+    pick_shape(B, nT, &C, &tile);
     cudaLaunchConfig_t cfg = {};
     cfg.gridDim = dim3((unsigned)C, (unsigned)(B < 65535 ? B : 65535), 1);
     cfg.blockDim = dim3(NT, 1, 1);
@@ -591,7 +668,7 @@ int launch_transit(const double* params, int B, const double* times, int nT, dou
     attr[0].val.clusterDim.z = 1;
     cfg.attrs = attr;
     cfg.numAttrs = 1;
-    cudaError_t e = cudaLaunchKernelEx(&cfg, transit_kernel<T>, params, B, times, nT, t_exp, n_ss,
+    cudaError_t e = cudaLaunchKernelEx(&cfg, transit_kernel<T>, params, B, times, nT, tile, t_exp, n_ss,
                                        obs, sigma, (T*)flux, (T*)chi2);
     if (e != cudaSuccess) return cuda_fail(e, "transit_kernel launch");
     ++tl_launches;
