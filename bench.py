@@ -214,12 +214,16 @@ def main():
     # ---- end to end through the HOST-buffer C ABI call, pinned host memory, copies timed
     pin = lambda x: torch.as_tensor(np.ascontiguousarray(x, dtype=np.float64)).pin_memory().numpy()  # noqa: E731
     hp, ht, ho, hs = pin(w.params), pin(w.times), pin(w.obs), pin(w.sigma)
-    for _ in range(2):
-        gl.gl_loglike_host(hp, ht, w.t_exp, w.n_ss, ho, hs, dtype="f32", want_flux=True)
+    c_h = torch.empty(w.B, dtype=torch.float32).pin_memory().numpy()          # pinned outputs too
+    f_h = torch.empty((w.B, w.T), dtype=torch.float32).pin_memory().numpy()
+    for _ in range(3):
+        gl.gl_loglike_host(hp, ht, w.t_exp, w.n_ss, ho, hs, dtype="f32", want_flux=True,
+                           chi2_out=c_h, flux_out=f_h)
     barrier()
     t0 = time.perf_counter()
     for _ in range(K):
-        c_h, f_h = gl.gl_loglike_host(hp, ht, w.t_exp, w.n_ss, ho, hs, dtype="f32", want_flux=True)
+        gl.gl_loglike_host(hp, ht, w.t_exp, w.n_ss, ho, hs, dtype="f32", want_flux=True,
+                           chi2_out=c_h, flux_out=f_h)
     e2e_s = time.perf_counter() - t0
     te = torch.tensor([e2e_s], device=dev, dtype=torch.float64)
     if dist is not None:
@@ -236,6 +240,7 @@ def main():
     # ---- roofline of the (only) kernel: plain FP32 ALU work
     sm_max = clocks.get("sm_max_mhz") or 1965.0
     peak_tflops = N_SM * LANES * 2 * sm_max * 1e6 / 1e12
+    probe = gl.gl_probe_peaks()      # FFMA / DFMA / MUFU chain kernels, measured now, on this GPU
     k_ms = float(np.mean(dev_ms))
     n_sub_in = n_in_exposures * w.n_ss
     alg_flop = ALG_FLOP_PER_SUBSAMPLE * n_sub_in
@@ -245,6 +250,9 @@ def main():
                 "kernel": "transit_kernel<float>", "kernel_ms": k_ms,
                 "peak_source": f"derived: {N_SM} SMs x {LANES} FP32 lanes x 2 x {sm_max:.0f} MHz "
                                "(MEASURED_PEAKS.json has no FP32 SIMT figure)",
+                "peak_measured_ffma_chain": probe["fp32_tflops"],
+                "frac_of_measured_peak": achieved / probe["fp32_tflops"],
+                "fp64_dfma_chain_tflops": probe["fp64_tflops"], "mufu_chain_tops": probe["mufu_tops"],
                 "alg_flop_per_in_transit_subsample": ALG_FLOP_PER_SUBSAMPLE,
                 "in_transit_subsamples_per_launch": n_sub_in,
                 "in_transit_fraction": n_sub_in / (w.B * w.T * w.n_ss),
@@ -260,7 +268,7 @@ def main():
         "wall_ms_per_step_incl_flush": 1e3 * wall / K,
         "clocks": clocks, "gpu_launches": int(launches),
         "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": h2d,
-                "d2h_bytes_per_step": d2h, "api": "gl_loglike_host (pinned host buffers)"},
+                "d2h_bytes_per_step": d2h, "api": "gl_loglike_host (pinned host inputs and outputs, wall clock over K calls)"},
         "roofline": roofline,
     }
     if world == 1 and not args.no_cpu_baseline:

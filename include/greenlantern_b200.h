@@ -98,6 +98,12 @@ int gl_loglike_host(const double* params, int B, const double* times, int T, dou
                     gl_dtype dtype);
 int gl_flux_geometry_host(const double* geom, long long N, void* flux_out, gl_dtype dtype);
 
+/* gl_probe_peaks: measures, on the current device, the arithmetic ceilings the roofline of
+ * bench.py divides by: register-only dependent-chain kernels of FFMA (fp32), DFMA
+ * (fp64) and MUFU.RSQ, 8 independent chains per thread, every SM full.  out3 (HOST) receives
+ * { fp32 TFLOP/s, fp64 TFLOP/s, MUFU Tops/s }.  Synchronises the device; not part of the hot path. */
+int gl_probe_peaks(double* out3);
+
 /* Number of kernel launches the calling thread's entry points have enqueued so far (HOST). */
 long long gl_launch_count(void);
 

@@ -17,7 +17,7 @@ _LIBPATH = Path(__file__).resolve().parent / "csrc" / "libgreenlantern_b200.so"
 _lib = None
 
 EXPORTS = ("gl_lightcurve", "gl_loglike", "gl_flux_geometry", "gl_lightcurve_host",
-           "gl_loglike_host", "gl_flux_geometry_host", "gl_launch_count", "gl_strerror",
+           "gl_loglike_host", "gl_flux_geometry_host", "gl_probe_peaks", "gl_launch_count", "gl_strerror",
            "gl_last_cuda_error", "gl_version")
 
 
@@ -45,6 +45,8 @@ def load_library():
     for name in ("gl_lightcurve", "gl_loglike", "gl_flux_geometry", "gl_lightcurve_host",
                  "gl_loglike_host", "gl_flux_geometry_host", "gl_version"):
         getattr(lib, name).restype = i
+    lib.gl_probe_peaks.argtypes = [vp]
+    lib.gl_probe_peaks.restype = i
     lib.gl_launch_count.restype = ll
     lib.gl_strerror.argtypes = [i]
     lib.gl_strerror.restype = ctypes.c_char_p
@@ -142,15 +144,28 @@ def _host_f64(x):
     return np.ascontiguousarray(x, dtype=np.float64)
 
 
-def gl_loglike_host(params, times, t_exp, n_ss, obs, sigma, dtype="f32", want_flux=False):
-    """HOST numpy in, HOST numpy out; the library does the copies (end-to-end path)."""
+def _host_out(out, shape, nd):
+    """A caller-supplied HOST output buffer (e.g. pinned memory), checked, or a fresh array."""
+    if out is None:
+        return np.empty(shape, dtype=nd)
+    if not (isinstance(out, np.ndarray) and out.dtype == nd and out.shape == tuple(shape)
+            and out.flags["C_CONTIGUOUS"] and out.flags["WRITEABLE"]):
+        raise GreenlanternError(f"out must be a writable C-contiguous {nd.__name__}{tuple(shape)} array")
+    return out
+
+
+def gl_loglike_host(params, times, t_exp, n_ss, obs, sigma, dtype="f32", want_flux=False,
+                    chi2_out=None, flux_out=None):
+    """HOST numpy in, HOST numpy out; the library does the copies (end-to-end path).
+    chi2_out / flux_out: optional preallocated HOST arrays (pinned memory makes the D2H copy
+    asynchronous and fast)."""
     lib = load_library()
     params, times, obs, sigma = map(_host_f64, (np.atleast_2d(params), times, obs, sigma))
     code = GL_F64 if dtype in (GL_F64, "f64", "float64") else GL_F32
     nd = np.float64 if code == GL_F64 else np.float32
     B, T = params.shape[0], times.shape[0]
-    chi2 = np.empty(B, dtype=nd)
-    flux = np.empty((B, T), dtype=nd) if want_flux else None
+    chi2 = _host_out(chi2_out, (B,), nd)
+    flux = _host_out(flux_out, (B, T), nd) if want_flux else None
     _check(lib.gl_loglike_host(params.ctypes.data, B, times.ctypes.data, T, float(t_exp),
                                int(n_ss), obs.ctypes.data, sigma.ctypes.data, chi2.ctypes.data,
                                flux.ctypes.data if want_flux else None, code))
@@ -175,6 +190,13 @@ def gl_flux_geometry_host(geom, dtype="f32"):
     out = np.empty(geom.shape[0], dtype=np.float64 if code == GL_F64 else np.float32)
     _check(lib.gl_flux_geometry_host(geom.ctypes.data, geom.shape[0], out.ctypes.data, code))
     return out
+
+
+def gl_probe_peaks():
+    """{fp32 TFLOP/s, fp64 TFLOP/s, MUFU Tops/s} of the current device (FMA / MUFU chain kernels)."""
+    out = (ctypes.c_double * 3)()
+    _check(load_library().gl_probe_peaks(out))
+    return {"fp32_tflops": out[0], "fp64_tflops": out[1], "mufu_tops": out[2]}
 
 
 def gl_launch_count():

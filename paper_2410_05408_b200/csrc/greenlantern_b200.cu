@@ -587,6 +587,36 @@ geometry_kernel(const double* __restrict__ geom, long long N, T* __restrict__ ou
     out[k] = T(1) - delta;
 }
 
+// ------------------------------------------------------------------------------------------
+// Ceiling probes (gl_probe_peaks): 8 independent register-only chains per thread.
+// ------------------------------------------------------------------------------------------
+template <typename T> __global__ void probe_fma(T* out, int iters, T a, T b) {
+    T x[8];
+#pragma unroll
+    for (int i = 0; i < 8; ++i) x[i] = T(threadIdx.x + i);
+    for (int it = 0; it < iters; ++it) {
+#pragma unroll
+        for (int i = 0; i < 8; ++i) x[i] = x[i] * a + b;
+    }
+    T s = T(0);
+#pragma unroll
+    for (int i = 0; i < 8; ++i) s += x[i];
+    out[blockIdx.x * blockDim.x + threadIdx.x] = s;
+}
+__global__ void probe_mufu(float* out, int iters) {
+    float x[8];
+#pragma unroll
+    for (int i = 0; i < 8; ++i) x[i] = 1.5f + threadIdx.x + i;
+    for (int it = 0; it < iters; ++it) {
+#pragma unroll
+        for (int i = 0; i < 8; ++i) asm volatile("rsqrt.approx.ftz.f32 %0, %0;" : "+f"(x[i]));
+    }
+    float s = 0.f;
+#pragma unroll
+    for (int i = 0; i < 8; ++i) s += x[i];
+    out[blockIdx.x * blockDim.x + threadIdx.x] = s;
+}
+
 }  // namespace
 
 // ==========================================================================================
@@ -732,6 +762,41 @@ int gl_flux_geometry(const double* geom, long long N, void* flux_out, gl_dtype d
     return GL_OK;
 }
 
+int gl_probe_peaks(double* out3) {
+    if (!out3) return GL_EINVAL;
+    void* scratch = nullptr;
+    const int blocks = 148 * 8, thr = 256, iters = 8192;
+    cudaError_t e = cudaMalloc(&scratch, (size_t)blocks * thr * sizeof(double));
+    if (e != cudaSuccess) return cuda_fail(e, "gl_probe_peaks cudaMalloc");
+    cudaEvent_t a, b;
+    cudaEventCreate(&a);
+    cudaEventCreate(&b);
+    for (int which = 0; which < 3; ++which) {
+        float best = 1e30f;
+        for (int rep = 0; rep < 4; ++rep) {   // rep 0 warms up
+            cudaEventRecord(a);
+            if (which == 0) probe_fma<float><<<blocks, thr>>>((float*)scratch, iters, 1.0001f, 0.5f);
+            if (which == 1) probe_fma<double><<<blocks, thr>>>((double*)scratch, iters / 2, 1.0001, 0.5);
+            if (which == 2) probe_mufu<<<blocks, thr>>>((float*)scratch, iters / 4);
+            cudaEventRecord(b);
+            cudaEventSynchronize(b);
+            float ms = 0.f;
+            cudaEventElapsedTime(&ms, a, b);
+            if (rep > 0 && ms < best) best = ms;
+        }
+        const double n = (double)blocks * thr * 8.0;
+        const double ops = which == 0 ? 2.0 * n * iters : which == 1 ? 2.0 * n * (iters / 2)
+                                                                     : n * (iters / 4);
+        out3[which] = ops / (best * 1e-3) / 1e12;
+    }
+    cudaEventDestroy(a);
+    cudaEventDestroy(b);
+    e = cudaGetLastError();
+    cudaFree(scratch);
+    if (e != cudaSuccess) return cuda_fail(e, "gl_probe_peaks");
+    return GL_OK;
+}
+
 long long gl_launch_count(void) { return tl_launches; }
 const char* gl_last_cuda_error(void) { return tl_cuda_err; }
 int gl_version(void) { return 100; }
@@ -754,12 +819,34 @@ const char* gl_strerror(int code) {
 // ------------------------------------------------------------------------------------------
 namespace {
 
+// One non-blocking stream per calling thread and device, created on first use and kept; the
+// device's default memory pool is told to keep its memory between calls (release threshold = max),
+// otherwise every synchronise hands the scratch back to the driver and the next call pays
+// milliseconds to get it again.
+cudaStream_t host_stream(cudaError_t* err) {
+    thread_local cudaStream_t streams[64] = {};
+    int dev = 0;
+    *err = cudaGetDevice(&dev);
+    if (*err != cudaSuccess) return nullptr;
+    if (dev < 0 || dev >= 64) dev = 63;
+    if (!streams[dev]) {
+        *err = cudaStreamCreateWithFlags(&streams[dev], cudaStreamNonBlocking);
+        if (*err != cudaSuccess) return nullptr;
+        cudaMemPool_t pool;
+        if (cudaDeviceGetDefaultMemPool(&pool, dev) == cudaSuccess) {
+            unsigned long long keep = ~0ull;
+            cudaMemPoolSetAttribute(pool, cudaMemPoolAttrReleaseThreshold, &keep);
+        }
+    }
+    return streams[dev];
+}
+
 struct HostCall {
     cudaStream_t st = nullptr;
     void* bufs[8];
     int nbufs = 0;
     cudaError_t err = cudaSuccess;
-    HostCall() { err = cudaStreamCreateWithFlags(&st, cudaStreamNonBlocking); }
+    HostCall() { st = host_stream(&err); }
     void* alloc(size_t bytes) {
         void* p = nullptr;
         if (err != cudaSuccess) return nullptr;
@@ -779,7 +866,6 @@ struct HostCall {
     int finish(int rc) {
         for (int i = 0; i < nbufs; ++i) cudaFreeAsync(bufs[i], st);
         cudaError_t e2 = st ? cudaStreamSynchronize(st) : cudaSuccess;
-        if (st) cudaStreamDestroy(st);
         if (rc != GL_OK) return rc;
         if (err != cudaSuccess) return cuda_fail(err, "host wrapper");
         if (e2 != cudaSuccess) return cuda_fail(e2, "host wrapper sync");
