@@ -350,11 +350,50 @@ template <> __device__ __forceinline__ float residual_sq<float>(double obs_m1, f
     return (float)residual_sq<double>(obs_m1, (double)delta, sg);   // out-of-range sigma
 }
 
+// chi^2 term of an in-window exposure.  shared_base: the launch-wide baseline
+// S = sum_i ((obs_i - 1)/sigma_i)^2 (baseline_kernel) already counts this exposure as if it were out
+// of transit, so the term is the DIFFERENCE model - baseline (0 when the baseline term is not finite:
+// S is then +inf already).
+template <typename T>
+__device__ __forceinline__ double listed_residual(double obs_m1, T dbar, double sg, int shared_base) {
+    const double term = (double)residual_sq<T>(obs_m1, dbar, sg);
+    if (!shared_base) return term;
+    const double base = (double)residual_sq<T>(obs_m1, T(0), sg);
+    return isfinite(base) ? term - base : 0.0;
+}
+
+// fp32 path only: the walker-independent baseline S = sum_i ((obs_i - 1)/sigma_i)^2 over ALL
+// exposures, once per launch instead of once per walker (every walker's chi^2 is S plus the
+// model-minus-baseline differences of its in-window exposures).  One CTA, fp64, fixed summation
+// order; S is left in chi2[0..B) (narrowed: 6e-8 relative, chi^2 budget 1e-4), where the transit
+// kernel, launched right behind with programmatic dependent launch, picks it up at its very end.
+__global__ void __launch_bounds__(1024)
+baseline_kernel(const double* __restrict__ obs, const double* __restrict__ sigma, int nT,
+                float* __restrict__ chi2, int B) {
+    asm volatile("griddepcontrol.launch_dependents;");
+    __shared__ double s_w[32];
+    __shared__ double s_tot;
+    double acc = 0.0;
+    for (int i = threadIdx.x; i < nT; i += 1024) acc += residual_sq<double>(obs[i] - 1.0, 0.0, sigma[i]);
+#pragma unroll
+    for (int off = 16; off > 0; off >>= 1) acc += __shfl_down_sync(0xffffffffu, acc, off);
+    if ((threadIdx.x & 31) == 0) s_w[threadIdx.x >> 5] = acc;
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        double tot = 0.0;
+        for (int k = 0; k < 32; ++k) tot += s_w[k];
+        s_tot = tot;
+    }
+    __syncthreads();
+    const float S = (float)s_tot;
+    for (int b = threadIdx.x; b < B; b += 1024) chi2[b] = S;
+}
+
 template <typename T>
 __global__ void __launch_bounds__(NT, sizeof(T) == 4 ? 8 : 2)
 transit_kernel(const double* __restrict__ params, int B, const double* __restrict__ times, int nT,
                int tile, double t_exp, int n_ss, const double* __restrict__ obs,
-               const double* __restrict__ sigma, T* __restrict__ flux, T* __restrict__ chi2) {
+               const double* __restrict__ sigma, T* __restrict__ flux, T* chi2, int shared_base) {
     cg::cluster_group cluster = cg::this_cluster();
     const int crank = (int)cluster.block_rank(), csize = (int)cluster.num_blocks();
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
@@ -417,7 +456,7 @@ transit_kernel(const double* __restrict__ params, int B, const double* __restric
                 // out-of-window ones are finished here
                 unsigned mask = 0;   // bit r: exposure i0 + r NT + tid is in the window
                 int wcount = 0;
-#pragma unroll 4
+#pragma unroll 2
                 for (int r = 0; r < nsub; ++r) {
                     const int i = i0 + r * NT + tid;
                     bool inwin = false;
@@ -430,7 +469,7 @@ transit_kernel(const double* __restrict__ params, int B, const double* __restric
                             sky_position_f64(sw, ph, &X, &Y);
                             inwin = X * X + Y * Y < reach * reach;
                         }
-                        if (want_chi2) {
+                        if (want_chi2 && !shared_base) {
                             const T r2 = residual_sq<T>(obs[i] - 1.0, T(0), sigma[i]);
                             if (!inwin) acc += (double)r2;
                         }
@@ -504,8 +543,7 @@ transit_kernel(const double* __restrict__ params, int B, const double* __restric
                         if (active && my_j == 0) {
                             const T dbar = sum * T(inv_ss);
                             if (frow) frow[i] = T(1) - dbar;
-                            if (want_chi2)
-                                acc += (double)residual_sq<T>(obs[i] - 1.0, dbar, sigma[i]);
+                            if (want_chi2) acc += listed_residual<T>(obs[i] - 1.0, dbar, sigma[i], shared_base);
                         }
                     }
                 } else {
@@ -524,8 +562,7 @@ transit_kernel(const double* __restrict__ params, int B, const double* __restric
                         if (lane == 0) {
                             const T dbar = sum * T(inv_ss);
                             if (frow) frow[i] = T(1) - dbar;
-                            if (want_chi2)
-                                acc += (double)residual_sq<T>(obs[i] - 1.0, dbar, sigma[i]);
+                            if (want_chi2) acc += listed_residual<T>(obs[i] - 1.0, dbar, sigma[i], shared_base);
                         }
                     }
                 }
@@ -545,6 +582,12 @@ transit_kernel(const double* __restrict__ params, int B, const double* __restric
             if (crank == 0 && tid == 0) {
                 double c2 = 0.0;
                 for (int r = 0; r < csize; ++r) c2 += *cluster.map_shared_rank(&s_partial[wpar], r);
+                if (shared_base) {
+                    // baseline_kernel left sum_i ((obs_i - 1)/sigma_i)^2 in chi2[wk]; it was launched
+                    // before this grid, which may have started early (programmatic dependent launch)
+                    asm volatile("griddepcontrol.wait;" ::: "memory");
+                    c2 += (double)*(volatile T*)&chi2[wk];
+                }
                 chi2[wk] = valid ? T(c2) : T(INFINITY);
             }
             wpar ^= 1;
@@ -686,20 +729,37 @@ int launch_transit(const double* params, int B, const double* times, int nT, dou
                    cudaStream_t st) {
     int C, tile;
     pick_shape(B, nT, &C, &tile);
+    // fp32 chi^2: launch-wide baseline first, the transit kernel right behind it (see baseline_kernel)
+    const int shared_base = (sizeof(T) == 4 && chi2 != nullptr && nT > 0) ? 1 : 0;
+    if (shared_base) {
+        baseline_kernel<<<1, 1024, 0, st>>>(obs, sigma, nT, (float*)chi2, B);
+        cudaError_t e0 = cudaGetLastError();
+        if (e0 != cudaSuccess) return cuda_fail(e0, "baseline_kernel launch");
+        ++tl_launches;
+    }
     cudaLaunchConfig_t cfg = {};
     cfg.gridDim = dim3((unsigned)C, (unsigned)(B < 65535 ? B : 65535), 1);
     cfg.blockDim = dim3(NT, 1, 1);
     cfg.dynamicSmemBytes = 0;
     cfg.stream = st;
-    cudaLaunchAttribute attr[1];
+    cudaLaunchAttribute attr[2];
     attr[0].id = cudaLaunchAttributeClusterDimension;
     attr[0].val.clusterDim.x = (unsigned)C;
     attr[0].val.clusterDim.y = 1;
     attr[0].val.clusterDim.z = 1;
+    attr[1].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    attr[1].val.programmaticStreamSerializationAllowed = 1;
     cfg.attrs = attr;
-    cfg.numAttrs = 1;
-    cudaError_t e = cudaLaunchKernelEx(&cfg, transit_kernel<T>, params, B, times, nT, tile, t_exp, n_ss,
-                                       obs, sigma, (T*)flux, (T*)chi2);
+    cfg.numAttrs = shared_base ? 2 : 1;
+    cudaError_t e = cudaLaunchKernelEx(&cfg, transit_kernel<T>, params, B, times, nT, tile, t_exp,
+                                       n_ss, obs, sigma, (T*)flux, (T*)chi2, shared_base);
+    if (e != cudaSuccess && shared_base) {
+        // no early start then: plain stream order is just as correct
+        (void)cudaGetLastError();
+        cfg.numAttrs = 1;
+        e = cudaLaunchKernelEx(&cfg, transit_kernel<T>, params, B, times, nT, tile, t_exp, n_ss, obs,
+                               sigma, (T*)flux, (T*)chi2, shared_base);
+    }
     if (e != cudaSuccess) return cuda_fail(e, "transit_kernel launch");
     ++tl_launches;
     return GL_OK;
