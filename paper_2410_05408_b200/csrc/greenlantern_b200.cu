@@ -415,9 +415,6 @@ transit_kernel(const double* __restrict__ params, int B, const double* __restric
     const int round_span = csize * tile;
     const int nrounds = (nT + round_span - 1) / round_span;
     const bool want_chi2 = (chi2 != nullptr);
-    // lane -> (exposure slot l, sub-exposure j) when a warp holds G = 32 / n_ss whole exposures
-    const int G = n_ss <= 32 ? 32 / n_ss : 0;
-    const int my_l = G ? lane / n_ss : 0, my_j = G ? lane - my_l * n_ss : lane;
     int wpar = 0;
     bool lists_live = false;   // uniform over the cluster
 
@@ -525,22 +522,33 @@ transit_kernel(const double* __restrict__ params, int B, const double* __restric
                 // turn (interleaved, so that ingress and egress are spread over every warp), each
                 // warp on its own (no block barriers)
                 const int gwarp = crank * NW + warp, gstride = csize * NW;
-                if (G) {
-                    // a warp takes G whole exposures at a time: lane = (exposure slot, sub-exposure)
-                    for (int p0 = gwarp * G; p0 < M; p0 += gstride * G) {
+                if (n_ss <= 32) {
+                    // a lane takes JS consecutive sub-exposures of one exposure, a warp G = 32 / JB
+                    // whole exposures (JB = blocks of JS per exposure).  Sparse lists (K2-shaped:
+                    // fewer pairs than the cluster has lanes) use JS = 1, one pair per lane; dense
+                    // lists raise JS up to n_ss, which amortises the list fetch, the mean and the
+                    // residual over more arithmetic and fills all 32 lanes.
+                    const long long pairs = (long long)M * n_ss;
+                    const int JS = (int)min((long long)n_ss, max(1LL, pairs / (4LL * 32 * gstride)));
+                    const int JB = (n_ss + JS - 1) / JS, Gr = 32 / JB;
+                    const int my_l = lane / JB, my_b = lane - my_l * JB;
+                    for (int p0 = gwarp * Gr; p0 < M; p0 += gstride * Gr) {
                         const int p = p0 + my_l;
-                        const bool active = (my_l < G) && (p < M);
+                        const bool active = (my_l < Gr) && (p < M);
                         int i = 0;
                         T delta = T(0);
                         if (active) {
                             i = fetch(p);
-                            const double t = times[i] + (((double)my_j + 0.5) * inv_ss - 0.5) * t_exp;
-                            delta = blocked_fraction<T>(s_trap, sw, v, reduced_phase(sw, t));
+                            const double tc = times[i];
+                            for (int j = my_b * JS; j < min(n_ss, (my_b + 1) * JS); ++j) {
+                                const double t = tc + (((double)j + 0.5) * inv_ss - 0.5) * t_exp;
+                                delta += blocked_fraction<T>(s_trap, sw, v, reduced_phase(sw, t));
+                            }
                         }
-                        T sum = T(0);   // exposure mean in sub-exposure order (R18)
-                        for (int jj = 0; jj < n_ss; ++jj)
-                            sum += __shfl_sync(0xffffffffu, delta, (lane + jj) & 31);
-                        if (active && my_j == 0) {
+                        T sum = T(0);   // exposure mean, blocks in sub-exposure order (R18)
+                        for (int bb = 0; bb < JB; ++bb)
+                            sum += __shfl_sync(0xffffffffu, delta, (lane + bb) & 31);
+                        if (active && my_b == 0) {
                             const T dbar = sum * T(inv_ss);
                             if (frow) frow[i] = T(1) - dbar;
                             if (want_chi2) acc += listed_residual<T>(obs[i] - 1.0, dbar, sigma[i], shared_base);
