@@ -128,6 +128,30 @@ GLF_DEV float whole_outline_lin(const TrapNode* trap, int nh, float xc, float yc
     return acc * (kPiF / float(nh));
 }
 
+// The same integral with SIX nodes (0, 60, ..., 300 degrees), for outlines deep inside the disc: the
+// node cosines and sines are immediates, and the pair on the major axis needs no y offset.  fp64
+// experiment (as above, 5e5 geometries): flux error <= 6.2e-9 once gap >= 3 a, <= 1.4e-8 for gap >= 0.5.
+GLF_DEV float whole_outline_lin6(float xc, float yc, float a, float b, float ab, float u, float v) {
+    constexpr float S60 = 0.86602540378443864676f;
+    const float yy = fmaf(-yc, yc, 1.f);
+    const float x0p = xc + a, x0q = xc - a;
+    float acc = pair_term<false>(fmaf(-x0p, x0p, yy), ab + u, fmaf(-x0q, x0q, yy), ab - u);
+    const float p = 0.5f * a, q = S60 * b, hu = 0.5f * u, sv = S60 * v;
+    {
+        const float xp = xc + p, yp = yc + q, xq = xc - p, yq = yc - q;
+        const float w = hu + sv;
+        acc += pair_term<false>(fmaf(-xp, xp, fmaf(-yp, yp, 1.f)), ab + w,
+                                fmaf(-xq, xq, fmaf(-yq, yq, 1.f)), ab - w);
+    }
+    {
+        const float xp = xc - p, yp = yc + q, xq = xc + p, yq = yc - q;
+        const float w = sv - hu;
+        acc += pair_term<false>(fmaf(-xp, xp, fmaf(-yp, yp, 1.f)), ab + w,
+                                fmaf(-xq, xq, fmaf(-yq, yq, 1.f)), ab - w);
+    }
+    return acc * (kPiF / 3.f);
+}
+
 // The outline in the kernel frame, re-parametrised by tau = t - t_far (t_far = the outline point
 // farthest from the star centre, given by its cosine/sine cf, sf).
 struct Arc {
@@ -222,6 +246,7 @@ GLF_DEV float blocked_f32(const TrapNode* trap, float xc_in, float yc_in, float 
         // well inside the limb (gap >= 0.01): 16 fixed nodes; 8 once the gap exceeds the semi-major
         // axis or 0.3 (error <= 6e-9 in flux on the config-5 sample)
         nh = (r0 + a + a <= 1.f || r0 + a <= 0.7f) ? 4 : 8;
+        if (fmaf(4.f, a, r0) <= 1.f || r0 + a <= 0.5f) nh = 3;   // deep inside: six immediate nodes
     } else if (Aa < e2 && Bb < e2) {
         // the star centre may lie inside the evolute (up to four crossings): bracketed search
         float A[3];
@@ -241,7 +266,8 @@ GLF_DEV float blocked_f32(const TrapNode* trap, float xc_in, float yc_in, float 
         // whole-outline closed forms: A_flat = pi a b, A_quad = pi a b (r0^2 + (a^2 + b^2)/4)
         const float in_flat = kPiF * ab;
         const float in_quad = in_flat * fmaf(0.25f, fmaf(a, a, b * b), r0sq);
-        const float lin = whole_outline_lin(trap, nh, xc, yc, a, b, ab, u, v);
+        const float lin = (nh == 3) ? whole_outline_lin6(xc, yc, a, b, ab, u, v)
+                                    : whole_outline_lin(trap, nh, xc, yc, a, b, ab, u, v);
         return fmaf(k0, in_flat, fmaf(k1 * (1.f / 3.f), lin, k2 * in_quad));
     }
     // the outline crosses the limb twice (or misses the disc).  tau = t - t_far in [0, 2 pi).

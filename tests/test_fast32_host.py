@@ -44,11 +44,12 @@ def test_fast32_matches_oracle_on_config5_mix(host_lib):
 
 
 def test_fast32_trapezoid_tiers(host_lib):
-    """Whole-outline-inside geometries at every tier boundary (gap = a, 0.3, 0.01, ~0)."""
+    """Whole-outline-inside geometries at every tier boundary (gap = 0.5, 3a, a, 0.3, 0.01, ~0)."""
     rows = []
     for rp, f in ((0.066, 0.5), (0.2, 0.9), (0.1, 0.0), (0.02, 0.3)):
         for pa in (0.0, 0.7, np.pi / 2, 2.5):
-            for gap in (0.5, 0.3001, 0.2999, rp * 1.001, rp * 0.999, 0.0101, 0.0099, 1e-3, 1e-5):
+            for gap in (0.7, 0.5001, 0.4999, rp * 3.001, rp * 2.999, 0.3001, 0.2999, rp * 1.001, rp * 0.999,
+                        0.0101, 0.0099, 1e-3, 1e-5):
                 d = 1.0 - gap - rp
                 if d > 0:
                     rows.append((d, rp, f, pa, 0.4, 0.25))
