@@ -67,7 +67,7 @@ constexpr double kTwoPi = 6.28318530717958647692;
 // ------------------------------------------------------------------------------------------
 struct Walker {
     // orbit (fp64: phases and Kepler's equation are always double)
-    double t0, inv_P, aR, e, omega, cosi, Mc, sq1pe, sq1me, half_win_phase, vmax, reach;
+    double t0, inv_P, aR, e, omega, cosi, Mc, sq1pe, sq1me, half_win_phase, hard_phase, vmax, reach;
     // projected outline: semi-axes and the rotation into the kernel frame
     double a, b, cpsi, spsi;
     // limb darkening, already divided by the disc-integrated intensity
@@ -155,6 +155,15 @@ __device__ void walker_prelude_orbit(const double* __restrict__ p, double t_exp,
                                     (lowp ? 1.0 + 1e-5 : 1.0);
         if (hw >= 0.0) hw += 0.5 * t_exp * w->inv_P + (lowp ? 1e-9 : 1e-13);
         w->vmax = kTwoPi * w->inv_P * aR;
+        // exposures wholly inside |phase| < hard_phase keep the outline at least 0.01 inside the
+        // limb (the cheap tiers of gl_fast32.cuh); the others (ingress, egress, grazing) are
+        // listed FIRST so that the expensive geometries start early (scheduling only)
+        const R qh = R(0.99 - Rp) / R(aR);
+        const R S2h = (qh * qh - ci2) / (R(1) - ci2);
+        double hp = 0.0;
+        if (S2h > R(0) && S2h < R(1))
+            hp = (double)(glc::gasin(glc::gsqrt(S2h)) * R(0.15915494309189535)) - 0.5 * t_exp * w->inv_P;
+        w->hard_phase = hp > 0.0 ? hp : 0.0;
     } else {
         // R7: conjunction at true anomaly pi/2 - omega; cos i from the impact parameter
         const double nuc = 0.5 * kPi - om;
@@ -167,6 +176,7 @@ __device__ void walker_prelude_orbit(const double* __restrict__ p, double t_exp,
         // largest sky-plane speed (periastron), in stellar radii per time unit: bounds how far
         // the centre moves within half an exposure (window test of eccentric orbits)
         w->vmax = kTwoPi * w->inv_P * aR * s1 / s2;
+        w->hard_phase = 0.0;
     }
     w->half_win_phase = hw;
     w->reach = reach;
@@ -401,9 +411,9 @@ transit_kernel(const double* __restrict__ params, int B, const double* __restric
 
     __shared__ Walker sw;
     __shared__ int s_list[MAXTILE];   // in-window time indices of this CTA's tile
-    __shared__ int s_nlist;
-    __shared__ int s_cnt[NW];         // in-window count per warp of the tile
-    __shared__ int s_rcnt[MAXCLUSTER];   // list lengths of the cluster's CTAs, this round
+    __shared__ int s_nlist[2];        // this CTA's list: [0] early (ingress/egress) entries, [1] the rest
+    __shared__ int s_cnt[2][NW];      // in-window count per warp of the tile, early / rest
+    __shared__ int s_pre[2][MAXCLUSTER + 1];   // prefix of the cluster's list lengths, early / rest
     __shared__ double s_red[NW];
     __shared__ double s_partial[2];   // this CTA's chi^2 partial (per walker parity), read by
                                       // cluster rank 0 via DSMEM
@@ -445,22 +455,24 @@ transit_kernel(const double* __restrict__ params, int B, const double* __restric
         } else {
             const WalkerT<T> v = narrow<T>(sw);
             const bool circ = v.circular;
-            const double hwin = sw.half_win_phase;
+            const double hwin = sw.half_win_phase, hard_ph = sw.hard_phase;
             const double reach = sw.reach + 0.5 * t_exp * sw.vmax;
             for (int round = 0; round < nrounds; ++round) {
                 const int i0 = (round * csize + crank) * tile;
                 // ---- pass 1: classify this thread's exposures of the tile against the window;
                 // out-of-window ones are finished here
-                unsigned mask = 0;   // bit r: exposure i0 + r NT + tid is in the window
-                int wcount = 0;
+                unsigned mask = 0;    // bit r: exposure i0 + r NT + tid is in the window
+                unsigned early = 0;   // ... and near its edge (ingress / egress): listed first
+                int wcount = 0, wearly = 0;
 #pragma unroll 2
                 for (int r = 0; r < nsub; ++r) {
                     const int i = i0 + r * NT + tid;
-                    bool inwin = false;
+                    bool inwin = false, isearly = false;
                     if (i < nT) {
                         const double ph = reduced_phase(sw, times[i]);
                         if (circ) {
                             inwin = fabs(ph) < hwin;
+                            isearly = inwin && !(fabs(ph) < hard_ph);
                         } else {
                             double X, Y;
                             sky_position_f64(sw, ph, &X, &Y);
@@ -473,50 +485,72 @@ transit_kernel(const double* __restrict__ params, int B, const double* __restric
                         if (!inwin && frow) frow[i] = T(1);
                     }
                     mask |= (inwin ? 1u : 0u) << r;
+                    early |= (isearly ? 1u : 0u) << r;
                     wcount += __popc(__ballot_sync(0xffffffffu, inwin));
+                    wearly += __popc(__ballot_sync(0xffffffffu, isearly));
                 }
-                if (lane == 0) s_cnt[warp] = wcount;
+                if (lane == 0) {
+                    s_cnt[0][warp] = wearly;
+                    s_cnt[1][warp] = wcount - wearly;
+                }
                 // nobody may still be reading the lists of the previous round / walker
                 if (lists_live) cluster.sync(); else __syncthreads();
-                // ---- pass 2: compact the in-window indices into this CTA's list, ordered by
-                // (warp, sub-chunk, lane): fixed for a given launch, so chi^2 is reproducible
+                // ---- pass 2: compact the in-window indices into this CTA's list: early entries
+                // first, then the rest, each ordered by (warp, sub-chunk, lane) -- fixed for a given
+                // launch, so chi^2 is reproducible
                 {
-                    int base = 0, total = 0;
+                    int base0 = 0, tot0 = 0, base1 = 0, tot1 = 0;
 #pragma unroll
                     for (int q = 0; q < NW; ++q) {
-                        if (q == warp) base = total;
-                        total += s_cnt[q];
+                        if (q == warp) {
+                            base0 = tot0;
+                            base1 = tot1;
+                        }
+                        tot0 += s_cnt[0][q];
+                        tot1 += s_cnt[1][q];
                     }
+                    base1 += tot0;
                     if (wcount) {
                         for (int r = 0; r < nsub; ++r) {
-                            const bool bit = (mask >> r) & 1u;
-                            const unsigned bal = __ballot_sync(0xffffffffu, bit);
-                            if (bit) s_list[base + __popc(bal & ((1u << lane) - 1u))] = i0 + r * NT + tid;
-                            base += __popc(bal);
+                            const bool b0 = (early >> r) & 1u, b1 = ((mask & ~early) >> r) & 1u;
+                            const unsigned bal0 = __ballot_sync(0xffffffffu, b0);
+                            const unsigned bal1 = __ballot_sync(0xffffffffu, b1);
+                            const unsigned lt = (1u << lane) - 1u;
+                            if (b0) s_list[base0 + __popc(bal0 & lt)] = i0 + r * NT + tid;
+                            if (b1) s_list[base1 + __popc(bal1 & lt)] = i0 + r * NT + tid;
+                            base0 += __popc(bal0);
+                            base1 += __popc(bal1);
                         }
                     }
-                    if (tid == 0) s_nlist = total;
+                    if (tid == 0) {
+                        s_nlist[0] = tot0;
+                        s_nlist[1] = tot1;
+                    }
                 }
-                // ---- share the round's list over the cluster
+                // ---- share the round's list over the cluster.  Cluster-wide order: the early
+                // entries of CTA 0, 1, ..., then the remaining entries of CTA 0, 1, ...
                 if (round == 0) GL_TL(2);
                 cluster.sync();
                 lists_live = true;
                 if (round == 0) GL_TL(3);
-                int pre[MAXCLUSTER + 1];
-                pre[0] = 0;
-#pragma unroll
-                for (int r = 0; r < MAXCLUSTER; ++r)
-                    pre[r + 1] = pre[r] + (r < csize ? *cluster.map_shared_rank(&s_nlist, r) : 0);
-                const int M = pre[MAXCLUSTER];
+                if (tid < 2) {
+                    int run = 0;
+                    for (int r = 0; r < csize; ++r) {
+                        s_pre[tid][r] = run;
+                        run += *cluster.map_shared_rank(&s_nlist[tid], r);
+                    }
+                    for (int r = csize; r <= MAXCLUSTER; ++r) s_pre[tid][r] = run;
+                }
+                __syncthreads();
+                const int M0 = s_pre[0][MAXCLUSTER], M = M0 + s_pre[1][MAXCLUSTER];
                 auto fetch = [&](int p) {   // p-th entry of the cluster-wide list
-                    int r = 0, off = 0;
+                    const int k = p >= M0 ? 1 : 0;
+                    const int q = p - (k ? M0 : 0);
+                    int r = 0;
 #pragma unroll
-                    for (int q = 1; q < MAXCLUSTER; ++q)
-                        if (q < csize && p >= pre[q]) {
-                            r = q;
-                            off = pre[q];
-                        }
-                    return *cluster.map_shared_rank(&s_list[p - off], r);
+                    for (int c = 1; c < MAXCLUSTER; ++c) r += (q >= s_pre[k][c] && c < csize) ? 1 : 0;
+                    const int local = q - s_pre[k][r] + (k ? s_pre[0][r + 1] - s_pre[0][r] : 0);
+                    return *cluster.map_shared_rank(&s_list[local], r);
                 };
                 // ---- evaluate the round's list: the cluster's warps take groups of exposures in
                 // turn (interleaved, so that ingress and egress are spread over every warp), each
@@ -532,7 +566,11 @@ transit_kernel(const double* __restrict__ params, int B, const double* __restric
                     const int JS = (int)min((long long)n_ss, max(1LL, pairs / (4LL * 32 * gstride)));
                     const int JB = (n_ss + JS - 1) / JS, Gr = 32 / JB;
                     const int my_l = lane / JB, my_b = lane - my_l * JB;
-                    for (int p0 = gwarp * Gr; p0 < M; p0 += gstride * Gr) {
+                    // sweep k hands group k gstride + (warp order, reversed on odd sweeps): the warps
+                    // that opened with the early (expensive) groups get the last groups, if any
+                    for (int k = 0, p0; (p0 = (k * gstride + ((k & 1) ? gstride - 1 - gwarp : gwarp)) * Gr) < M ||
+                                        k * gstride * Gr < M; ++k) {
+                        if (p0 >= M) continue;
                         const int p = p0 + my_l;
                         const bool active = (my_l < Gr) && (p < M);
                         int i = 0;
