@@ -568,9 +568,10 @@ transit_kernel(const double* __restrict__ params, int B, const double* __restric
                     const int my_l = lane / JB, my_b = lane - my_l * JB;
                     // sweep k hands group k gstride + (warp order, reversed on odd sweeps): the warps
                     // that opened with the early (expensive) groups get the last groups, if any
-                    for (int k = 0, p0; (p0 = (k * gstride + ((k & 1) ? gstride - 1 - gwarp : gwarp)) * Gr) < M ||
-                                        k * gstride * Gr < M; ++k) {
-                        if (p0 >= M) continue;
+                    const int nsweeps = (M + gstride * Gr - 1) / (gstride * Gr);
+                    for (int k = 0; k < nsweeps; ++k) {
+                        const int p0 = (k * gstride + ((k & 1) ? gstride - 1 - gwarp : gwarp)) * Gr;
+                        if (p0 >= M) continue;   // warp-uniform
                         const int p = p0 + my_l;
                         const bool active = (my_l < Gr) && (p < M);
                         int i = 0;
