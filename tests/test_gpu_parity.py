@@ -177,3 +177,73 @@ def test_host_wrappers_match_device_path(gl):
     assert np.array_equal(gl.gl_flux_geometry_host(geom, "f32").astype(np.float64),
                           host(gl.gl_flux_geometry(dev(geom), "f32")))
     assert gl.gl_launch_count() > 0
+
+
+@pytest.mark.parametrize("dtype", ["f32", "f64"])
+def test_many_rounds_and_many_walkers(gl, dtype):
+    """Launch shapes the five configs never reach: a series longer than one round of tiles
+    (T > C * tile capacity: the lists are reused under a cluster barrier), gl_lightcurve over
+    several rounds (no chi^2 barrier between them), and more walkers than grid rows (a cluster
+    loops over walkers)."""
+    base = wl.config2()
+    # 1) one walker, 40 000 exposures over two transits' worth of phase: >= 2 rounds in both dtypes
+    T = 40_000
+    t = np.linspace(-1.2, 1.2, T) + 542.0 * np.repeat([0.0, 3.0], T // 2)
+    rng = np.random.default_rng(5)
+    obs = 1.0 + 1e-4 * rng.standard_normal(T)
+    sig = np.full(T, 1e-4)
+    p = np.repeat(base.params, 3, axis=0)
+    p[1, 3], p[2, 7] = 0.45, 0.1
+    chi, out = gl.gl_loglike(dev(p), dev(t), base.t_exp, 3, dev(obs), dev(sig), dtype=dtype,
+                             want_flux=True)
+    chi_ref, ref = orc.loglike(p, t, base.t_exp, 3, obs, sig)
+    assert np.abs(host(out) - ref).max() <= FTOL[dtype]
+    assert np.abs(host(chi) / chi_ref - 1.0).max() <= CTOL[dtype]
+    lc = gl.gl_lightcurve(dev(p), dev(t), base.t_exp, 3, dtype=dtype)
+    assert np.array_equal(host(lc), host(out))
+    # 2) 70 000 walkers (> 65 535 grid rows) on a short stretch around mid-transit
+    B = 70_000
+    pw = wl.draw_walkers(B, 99)
+    ts = base.times[1945:1955]
+    chi2, flux = gl.gl_loglike(dev(pw), dev(ts), base.t_exp, 2, dev(base.obs[1945:1955]),
+                               dev(base.sigma[1945:1955]), dtype=dtype, want_flux=True)
+    rows = np.r_[0:50, 65_500:65_600, B - 50:B]
+    chi_ref, ref = orc.loglike(pw[rows], ts, base.t_exp, 2, base.obs[1945:1955], base.sigma[1945:1955])
+    assert np.abs(host(flux)[rows] - ref).max() <= FTOL[dtype]
+    assert np.abs(host(chi2)[rows] / chi_ref - 1.0).max() <= CTOL[dtype]
+    assert np.all(np.isfinite(host(flux))) and np.all(host(chi2) > 0)
+
+
+def test_eccentric_batch_fp32_vs_fp64(gl):
+    """e > 0 walkers through the fp32 path (fp64 Kepler + fp32 geometry) against the oracle."""
+    w = wl.config3(B=32)
+    p = w.params.copy()
+    rng = np.random.default_rng(17)
+    p[:, 4] = rng.uniform(0.05, 0.6, 32)
+    p[:, 5] = rng.uniform(0.0, 2 * np.pi, 32)
+    sel = slice(1850, 2050)
+    chi_ref, ref = orc.loglike(p, w.times[sel], w.t_exp, w.n_ss, w.obs[sel], w.sigma[sel])
+    for dtype in ("f32", "f64"):
+        chi, out = gl.gl_loglike(dev(p), dev(w.times[sel]), w.t_exp, w.n_ss, dev(w.obs[sel]),
+                                 dev(w.sigma[sel]), dtype=dtype, want_flux=True)
+        assert np.abs(host(out) - ref).max() <= FTOL[dtype], dtype
+        assert np.abs(host(chi) / chi_ref - 1.0).max() <= CTOL[dtype], dtype
+    assert (ref < 1.0).sum() > 500          # the transits are really in the stretch
+
+
+def test_bad_sigma_and_determinism(gl):
+    """A non-positive sigma makes every chi^2 +inf (in or out of the window, both dtypes); two
+    identical fp32 launches give bit-identical chi^2 and flux."""
+    w = wl.config3(B=8)
+    for bad_at in (10, 1950):              # out of every window / inside every window
+        sg = w.sigma.copy()
+        sg[bad_at] = 0.0
+        for dtype in ("f32", "f64"):
+            chi = host(gl.gl_loglike(dev(w.params), dev(w.times), w.t_exp, w.n_ss, dev(w.obs),
+                                     dev(sg), dtype=dtype))
+            assert np.all(np.isinf(chi)) and np.all(chi > 0), (bad_at, dtype, chi)
+    a = gl.gl_loglike(dev(w.params), dev(w.times), w.t_exp, w.n_ss, dev(w.obs), dev(w.sigma),
+                      dtype="f32", want_flux=True)
+    b = gl.gl_loglike(dev(w.params), dev(w.times), w.t_exp, w.n_ss, dev(w.obs), dev(w.sigma),
+                      dtype="f32", want_flux=True)
+    assert np.array_equal(host(a[0]), host(b[0])) and np.array_equal(host(a[1]), host(b[1]))
