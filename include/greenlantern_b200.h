@@ -88,6 +88,17 @@ int gl_loglike(const double* params, int B, const double* times, int T, double t
  *   0 <= f_proj < 1.  flux_out [N] float/double.  An invalid row gives NaN. */
 int gl_flux_geometry(const double* geom, long long N, void* flux_out, gl_dtype dtype, void* stream);
 
+/* gl_flux_geometry_simpson: the same rows and output as gl_flux_geometry, computed with the
+ * PAPER'S OWN algorithm instead of crossings + closed forms: every outline point outside the disc
+ * is snapped radially onto the limb (eqs. 16-20) and the three integrands of
+ * PAPER.md:127-135 (eqs. 21-23) are summed over theta in [0, 2 pi] by composite Simpson
+ * with n_intervals intervals (even, 2 <= n_intervals <= 2^24; else GL_EINVAL), one
+ * warp per geometry.  The discretisation error falls only like 1/n_intervals on
+ * limb-crossing geometries (the snapped integrand has a kink); it is here to be measured against
+ * gl_flux_geometry, not to replace it. */
+int gl_flux_geometry_simpson(const double* geom, long long N, int n_intervals, void* flux_out,
+                             gl_dtype dtype, void* stream);
+
 /* HOST-buffer convenience wrappers (used for the end-to-end numbers of bench.py): every pointer
  * below is a HOST pointer; the call allocates device scratch, copies in, runs the kernel above,
  * copies out and synchronises before it returns.  Same semantics and status codes otherwise. */

@@ -16,7 +16,7 @@ GL_NPARAMS, GL_NGEOM = 12, 6
 _LIBPATH = Path(__file__).resolve().parent / "csrc" / "libgreenlantern_b200.so"
 _lib = None
 
-EXPORTS = ("gl_lightcurve", "gl_loglike", "gl_flux_geometry", "gl_lightcurve_host",
+EXPORTS = ("gl_lightcurve", "gl_loglike", "gl_flux_geometry", "gl_flux_geometry_simpson", "gl_lightcurve_host",
            "gl_loglike_host", "gl_flux_geometry_host", "gl_probe_peaks", "gl_launch_count", "gl_strerror",
            "gl_last_cuda_error", "gl_version")
 
@@ -39,6 +39,8 @@ def load_library():
     lib.gl_lightcurve.argtypes = [vp, i, vp, i, d, i, vp, i, vp]
     lib.gl_loglike.argtypes = [vp, i, vp, i, d, i, vp, vp, vp, vp, i, vp]
     lib.gl_flux_geometry.argtypes = [vp, ll, vp, i, vp]
+    lib.gl_flux_geometry_simpson.argtypes = [vp, ll, i, vp, i, vp]
+    lib.gl_flux_geometry_simpson.restype = i
     lib.gl_lightcurve_host.argtypes = [vp, i, vp, i, d, i, vp, i]
     lib.gl_loglike_host.argtypes = [vp, i, vp, i, d, i, vp, vp, vp, vp, i]
     lib.gl_flux_geometry_host.argtypes = [vp, ll, vp, i]
@@ -137,6 +139,19 @@ def gl_flux_geometry(geom, dtype="f32"):
     with torch.cuda.device(geom.device):
         _check(lib.gl_flux_geometry(geom.data_ptr(), geom.shape[0], out.data_ptr(), code,
                                     _stream(geom)))
+    return out
+
+
+def gl_flux_geometry_simpson(geom, n_intervals, dtype="f32"):
+    """The paper's snap + Simpson algorithm (NEXT-1) on [N, 6] geometry rows; one warp per row."""
+    torch = _torch()
+    lib = load_library()
+    geom = _dev_f64(geom, GL_NGEOM)
+    code, td = _tdtype(dtype)
+    out = torch.empty((geom.shape[0],), dtype=td, device=geom.device)
+    with torch.cuda.device(geom.device):
+        _check(lib.gl_flux_geometry_simpson(geom.data_ptr(), geom.shape[0], int(n_intervals),
+                                            out.data_ptr(), code, _stream(geom)))
     return out
 
 

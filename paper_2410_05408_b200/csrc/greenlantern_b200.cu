@@ -22,6 +22,7 @@
 #include "../../include/greenlantern_b200.h"
 #include "gl_core.cuh"
 #include "gl_fast32.cuh"
+#include "gl_simpson.cuh"
 #include "gl_tables.h"
 
 namespace cg = cooperative_groups;
@@ -865,6 +866,27 @@ int gl_flux_geometry(const double* geom, long long N, void* flux_out, gl_dtype d
         geometry_kernel<double><<<blocks, NT, 0, st>>>(geom, N, (double*)flux_out);
     cudaError_t e = cudaGetLastError();
     if (e != cudaSuccess) return cuda_fail(e, "geometry_kernel launch");
+    ++tl_launches;
+    return GL_OK;
+}
+
+int gl_flux_geometry_simpson(const double* geom, long long N, int n_intervals, void* flux_out,
+                             gl_dtype dtype, void* stream) {
+    if (N < 0 || (dtype != GL_F32 && dtype != GL_F64)) return GL_EINVAL;
+    if (n_intervals < 2 || (n_intervals & 1) || n_intervals > (1 << 24)) return GL_EINVAL;
+    if (N == 0) return GL_OK;
+    if (!geom || !flux_out) return GL_EINVAL;
+    if (N >= (1LL << 40)) return GL_EUNSUPPORTED;
+    const long long threads = N * 32;   // one warp per geometry
+    const long long blocks = (threads + 127) / 128;
+    if (blocks > 0x7fffffffLL) return GL_EUNSUPPORTED;
+    cudaStream_t st = (cudaStream_t)stream;
+    if (dtype == GL_F32)
+        gls::simpson_kernel<float><<<(unsigned)blocks, 128, 0, st>>>(geom, N, n_intervals, (float*)flux_out);
+    else
+        gls::simpson_kernel<double><<<(unsigned)blocks, 128, 0, st>>>(geom, N, n_intervals, (double*)flux_out);
+    cudaError_t e = cudaGetLastError();
+    if (e != cudaSuccess) return cuda_fail(e, "simpson_kernel launch");
     ++tl_launches;
     return GL_OK;
 }

@@ -247,3 +247,46 @@ def test_bad_sigma_and_determinism(gl):
     b = gl.gl_loglike(dev(w.params), dev(w.times), w.t_exp, w.n_ss, dev(w.obs), dev(w.sigma),
                       dtype="f32", want_flux=True)
     assert np.array_equal(host(a[0]), host(b[0])) and np.array_equal(host(a[1]), host(b[1]))
+
+
+def _oracle_snap_simpson_flux(geom, n_int):
+    out = np.empty(geom.shape[0])
+    for k, (d, rp, fp, pa, u1, u2) in enumerate(geom):
+        a, b = rp, rp * (1 - fp)
+        dx = np.sqrt(a * a * np.cos(pa) ** 2 + b * b * np.sin(pa) ** 2)
+        A = orc.areas_snap_simpson(d, 0.0, dx, (a * a - b * b) * np.cos(pa) * np.sin(pa) / dx,
+                                   a * b / dx, n_int)
+        norm = np.pi * (1 - u1 / 3 - u2 / 6)
+        out[k] = 1.0 - ((1 - u1 - 2 * u2) * A[0] + (u1 + 2 * u2) * A[1] + u2 * A[2]) / norm
+    return out
+
+
+@pytest.mark.parametrize("dtype", ["f32", "f64"])
+def test_paper_snap_simpson_kernel(gl, dtype):
+    """NEXT-1: the paper's own algorithm (snapping, eqs. 16-20, + composite Simpson) as a kernel,
+    against the oracle's transcription of the same algorithm at the same node count (node for
+    node: same parametrisation), and -- loosely, it converges like 1/N -- against the exact flux."""
+    geom, cls = wl.config5(N=4000)
+    n_int = 512
+    ref = _oracle_snap_simpson_flux(geom, n_int)
+    out = host(gl.gl_flux_geometry_simpson(dev(geom), n_int, dtype=dtype))
+    tol = 5e-7 if dtype == "f32" else 1e-12
+    err = np.abs(out - ref)
+    assert err[cls != 4].max() <= tol, err[cls != 4].max()
+    # class 4 = flat side of a very oblate outline lying ALONG the limb (PA = pi/2 exactly): dozens of
+    # nodes sit within rounding of r = 1, and eq. 23's integrand is discontinuous across the snap
+    # (its radial part is dropped by eqs. 17-18), so each node whose r^2 > 1 test flips in fp32 moves
+    # A_quad by O(h): the paper's "numerical noise" (PAPER.md:149).  It happens in fp64 too (the
+    # kernel's sincospi and the oracle's sin(k h) differ in the last bit): a property of the
+    # algorithm, not of either implementation, so these rows get the discretisation-level bound.
+    assert err[cls == 4].max() <= 1e-5, err[cls == 4].max()
+    # against the exact flux: discretisation error of the paper's scheme, not rounding
+    exact = orc.flux_geometry(geom)
+    big = host(gl.gl_flux_geometry_simpson(dev(geom), 1 << 16, dtype="f64"))
+    assert np.abs(big - exact).max() <= 2e-7
+    assert np.abs(out - exact).max() <= 2e-4
+    with pytest.raises(gl.GreenlanternError):
+        gl.gl_flux_geometry_simpson(dev(geom), 511, dtype=dtype)
+    bad = geom[:4].copy()
+    bad[1, 1] = 0.7
+    assert np.isnan(host(gl.gl_flux_geometry_simpson(dev(bad), 64, dtype=dtype))[1])
