@@ -416,8 +416,8 @@ transit_kernel(const double* __restrict__ params, int B, const double* __restric
     __shared__ int s_cnt[2][NW];      // in-window count per warp of the tile, early / rest
     __shared__ int s_pre[2][MAXCLUSTER + 1];   // prefix of the cluster's list lengths, early / rest
     __shared__ double s_red[NW];
-    __shared__ double s_partial[2];   // this CTA's chi^2 partial (per walker parity), read by
-                                      // cluster rank 0 via DSMEM
+    __shared__ double s_gather[2][MAXCLUSTER];   // rank 0's copy collects the CTAs' chi^2 partials
+                                                 // (written over DSMEM; slot = walker parity)
     __shared__ glf::TrapNode s_trap[16];   // trapezoid nodes (per-lane strides: not constant memory)
     if (tid < 16) s_trap[tid] = glf::TrapNode{glf::c_trap_cos[tid], glf::c_trap_sin[tid]};
 
@@ -617,19 +617,21 @@ transit_kernel(const double* __restrict__ params, int B, const double* __restric
             }
         }
         GL_TL(4);
-        // ---- chi^2: CTA sum, then cluster rank 0 adds the partials in rank order over DSMEM.
-        // s_partial alternates between two slots, so the barrier of the NEXT walker (or the one at
-        // kernel exit) is what keeps a slot alive until rank 0 has read it.
+        // ---- chi^2: CTA sum; every CTA PUSHES its partial into rank 0's shared memory over DSMEM,
+        // one cluster barrier, then rank 0 adds them in rank order.  Nothing is read remotely after
+        // that barrier, so the other CTAs may move on (or exit) at once.  The slots alternate with
+        // the walker parity: a slot is rewritten two walkers later, i.e. after a barrier that rank 0
+        // can only pass once it has read the slot.
         if (want_chi2) {
             const double tot = block_sum(acc, s_red);
             GL_TL(5);
-            if (tid == 0) s_partial[wpar] = tot;
+            if (tid == 0) *cluster.map_shared_rank(&s_gather[wpar][crank], 0) = tot;
             cluster.sync();
             lists_live = false;   // every CTA is past its evaluation
             GL_TL(6);
             if (crank == 0 && tid == 0) {
                 double c2 = 0.0;
-                for (int r = 0; r < csize; ++r) c2 += *cluster.map_shared_rank(&s_partial[wpar], r);
+                for (int r = 0; r < csize; ++r) c2 += s_gather[wpar][r];
                 if (shared_base) {
                     // baseline_kernel left sum_i ((obs_i - 1)/sigma_i)^2 in chi2[wk]; it was launched
                     // before this grid, which may have started early (programmatic dependent launch)
@@ -641,7 +643,8 @@ transit_kernel(const double* __restrict__ params, int B, const double* __restric
             wpar ^= 1;
         }
     }
-    cluster.sync();   // no CTA may exit while a neighbour can still read its shared memory
+    // no CTA may exit while a neighbour can still read its lists (flux-only calls: no barrier above)
+    if (lists_live) cluster.sync();
     GL_TL(7);
 }
 
