@@ -61,6 +61,8 @@ def _load():
         lib.gl_oracle_flux_time.argtypes = [_dp, d, d, i]
         lib.gl_oracle_flux_time.restype = d
         lib.gl_oracle_lightcurve.argtypes = [_dp, i, _dp, i, d, i, _dp, i]
+        lib.gl_oracle_lightcurve_ex.argtypes = [_dp, i, _dp, i, d, i, _dp, i]
+        lib.gl_oracle_params_ex_valid.argtypes = [_dp]
         lib.gl_oracle_lightcurve.restype = i
         lib.gl_oracle_loglike.argtypes = [_dp, i, _dp, i, d, i, _dp, _dp, _dp, _dp, i]
         lib.gl_oracle_loglike.restype = i
@@ -151,6 +153,23 @@ def lightcurve(params, times, t_exp=0.0, n_ss=1, nthreads=0):
     _load().gl_oracle_lightcurve(pp, p.shape[0], tp, t.shape[0], float(t_exp), int(n_ss),
                                  flux.ctypes.data_as(_dp), int(nthreads))
     return flux
+
+
+def lightcurve_ex(params16, times, t_exp=0.0, n_ss=1, nthreads=0):
+    """flux[B,T] for the extended rows [B,16] of NEXT-2: triaxial and/or tidally locked planets
+    (columns 12-15 = zeta, b-axis/Rp_eq, c-axis/Rp_eq, locked flag)."""
+    p, pp = _c(np.atleast_2d(params16))
+    assert p.shape[1] == 16
+    t, tp = _c(times)
+    flux = np.empty((p.shape[0], t.shape[0]))
+    _load().gl_oracle_lightcurve_ex(pp, p.shape[0], tp, t.shape[0], float(t_exp), int(n_ss),
+                                    flux.ctypes.data_as(_dp), int(nthreads))
+    return flux
+
+
+def params_ex_valid(params16):
+    p, pp = _c(params16)
+    return bool(_load().gl_oracle_params_ex_valid(pp))
 
 
 def loglike(params, times, t_exp, n_ss, obs, sigma, nthreads=0, return_threads=False):

@@ -437,7 +437,14 @@ double gl_oracle_kepler(double M, double e) {
 /* Sky-plane position of the planet centre at time t.  p = the 12-vector
  * (t0, P, a/R*, b, e, omega, Rp_eq, f, xi, eta, u1, u2).  Returns 1 when the
  * planet is in front of the star (cos phi > 0), else 0. */
+int gl_oracle_orbit(const double *p, double t, double *x0, double *y0, double *phi_out);
 int gl_oracle_position(const double *p, double t, double *x0, double *y0) {
+    double phi;
+    return gl_oracle_orbit(p, t, x0, y0, &phi);
+}
+
+/* The same, also returning the orbital angle from conjunction phi (alpha of eqs. 9-10). */
+int gl_oracle_orbit(const double *p, double t, double *x0, double *y0, double *phi_out) {
     const double t0 = p[0], P = p[1], aR = p[2], b = p[3], e = p[4], om = p[5];
     const double nuc = 0.5 * GLO_PI - om;
     const double Ec = 2.0 * atan2(sqrt(1.0 - e) * sin(0.5 * nuc), sqrt(1.0 + e) * cos(0.5 * nuc));
@@ -454,6 +461,7 @@ int gl_oracle_position(const double *p, double t, double *x0, double *y0) {
     const double cosi = (b / aR) * (1.0 + e * sin(om)) / (1.0 - e * e);
     *x0 = r * cos(phi) * cosi;   /* eq. 9 with alpha -> phi, d -> r, sin(beta) = cos i */
     *y0 = r * sin(phi);          /* eq. 10 */
+    *phi_out = phi;
     return cos(phi) > 0.0;
 }
 
@@ -489,6 +497,51 @@ double gl_oracle_flux_time(const double *p, double t, double t_exp, int n_ss) {
         double x0, y0, F = 1.0;
         if (gl_oracle_position(p, tj, &x0, &y0))
             F = gl_oracle_flux_outline(x0, y0, d3[0], d3[1], d3[2], p[10], p[11]);
+        sum += F;
+    }
+    return sum / n_ss;
+}
+
+/* ------------------------------------------------------------------------ */
+/* NEXT-2: general triaxial ellipsoids and tidally locked    */
+/* planets.  Extended row p[16]: columns 0-11 as above, then                   */
+/*   12 zeta [rad] (third Euler angle of eq. 6)                */
+/*   13 rb, 14 rc: semi-axes b = Rp_eq rb along y', c = Rp_eq rc along z'      */
+/*      (a = Rp_eq (1-f) along x' as before; the oblate model is rb = rc = 1)  */
+/*   15 locked: 0 = orientation fixed in the observer frame (eq. 2, eqs.       */
+/*      11-13), 1 = tidally locked (eq. B13): the outline amplitudes follow    */
+/*      eqs. B14-B16 with alpha = the orbital angle from    */
+/*      conjunction (phi of reading R7; alpha of eqs. 9-10 for e = 0) and      */
+/*      sin(beta) = cos i; the centre still moves by eqs. 9-10.                */
+/* ------------------------------------------------------------------------ */
+int gl_oracle_params_ex_valid(const double *p) {
+    if (!gl_oracle_params_valid(p)) return 0;
+    for (int k = 12; k < 16; k++)
+        if (!isfinite(p[k])) return 0;
+    const double Rp = p[6], rb = p[13], rc = p[14];
+    if (!(rb > 0.0) || !(rc > 0.0) || !(Rp * rb < 0.5) || !(Rp * rc < 0.5)) return 0;
+    if (!(p[15] == 0.0 || p[15] == 1.0)) return 0;
+    return 1;
+}
+
+double gl_oracle_flux_time_ex(const double *p, double t, double t_exp, int n_ss) {
+    if (!gl_oracle_params_ex_valid(p)) return NAN;
+    const double Rp = p[6], f = p[7], xi = p[8], eta = p[9], zeta = p[12];
+    const double sa = Rp * (1.0 - f), sb = Rp * p[13], sc = Rp * p[14];
+    const int locked = p[15] == 1.0;
+    double d3[3];
+    gl_oracle_outline(sa, sb, sc, zeta, eta, xi, d3);
+    const double e = p[4], om = p[5];
+    const double cosi = (p[3] / p[2]) * (1.0 + e * sin(om)) / (1.0 - e * e);
+    const double beta = asin(cosi);   /* eq. 9: x0 = d cos(alpha) sin(beta) */
+    double sum = 0.0;
+    for (int j = 0; j < n_ss; j++) {
+        const double tj = t + ((j + 0.5) / n_ss - 0.5) * t_exp;
+        double x0, y0, alpha, F = 1.0;
+        if (gl_oracle_orbit(p, tj, &x0, &y0, &alpha)) {
+            if (locked) gl_oracle_outline_locked(sa, sb, sc, zeta, eta, xi, alpha, beta, d3);
+            F = gl_oracle_flux_outline(x0, y0, d3[0], d3[1], d3[2], p[10], p[11]);
+        }
         sum += F;
     }
     return sum / n_ss;
@@ -544,6 +597,22 @@ int gl_oracle_loglike(const double *params, int B, const double *times, int T, d
         chi2[b] = acc + comp;
     }
     if (!flux) free(tmp);
+    return nthreads;
+}
+
+/* flux[B,T] for params_ex[B,16] (NEXT-2). */
+int gl_oracle_lightcurve_ex(const double *params, int B, const double *times, int T, double t_exp,
+                            int n_ss, double *flux, int nthreads) {
+    ensure_tables();
+    nthreads = pick_threads(nthreads);
+    const long total = (long)B * T;
+#ifdef _OPENMP
+#pragma omp parallel for schedule(dynamic, 16) num_threads(nthreads)
+#endif
+    for (long k = 0; k < total; k++) {
+        const int b = (int)(k / T), i = (int)(k % T);
+        flux[k] = gl_oracle_flux_time_ex(params + 16 * (long)b, times[i], t_exp, n_ss);
+    }
     return nthreads;
 }
 

@@ -576,3 +576,90 @@ def test_chi2_definition_and_invalid_walkers():
     chi_self, _ = orc.loglike(rows[:1], times, 0.01, 3, flux[0], sigma)
     assert chi_self[0] == 0.0
     assert not orc.params_valid(rows[2]) and orc.params_valid(rows[0])
+
+
+# ---------------------------------------------------------------------------------------------
+# NEXT-2: extended rows (triaxial / tidally locked), oracle.lightcurve_ex.  The outline functions
+# (eqs. 11-13, B14-B16) are pinned above by brute-force projection; these pins fix how the light
+# curve USES them: which alpha and beta go into B14-B16 (reading R23), the axis columns, and the
+# reductions that must hold exactly.
+# ---------------------------------------------------------------------------------------------
+def _short_period_row(**kw):
+    row = dict(t0=0.0, P=3.0, aR=6.0, b=0.3, e=0.0, om=0.0, Rp=0.1, f=0.4, xi=0.5, eta=0.3,
+               u1=0.0, u2=0.0, zeta=0.0, rb=1.0, rc=1.0, locked=0.0)
+    row.update(kw)
+    return np.array([[row[k] for k in ("t0", "P", "aR", "b", "e", "om", "Rp", "f", "xi", "eta",
+                                       "u1", "u2", "zeta", "rb", "rc", "locked")]])
+
+
+def test_ex_rows_reduce_to_the_oblate_model():
+    t = np.linspace(-0.12, 0.12, 41)
+    p = _short_period_row(u1=0.4, u2=0.25)
+    assert np.array_equal(orc.lightcurve_ex(p, t, 0.01, 3), orc.lightcurve(p[:, :12], t, 0.01, 3))
+    # a sphere does not care about locking, zeta, or which way it turns
+    s0 = orc.lightcurve(_short_period_row(f=0.0, u1=0.4, u2=0.25)[:, :12], t)
+    s1 = orc.lightcurve_ex(_short_period_row(f=0.0, u1=0.4, u2=0.25, locked=1.0, zeta=0.7), t)
+    assert np.abs(s1 - s0).max() < 1e-14
+    # zeta spins an oblate spheroid (b = c) about its own symmetry axis: nothing changes
+    z = orc.lightcurve_ex(_short_period_row(u1=0.4, u2=0.25, zeta=1.1), t)
+    assert np.abs(z - orc.lightcurve(p[:, :12], t)).max() < 1e-13
+    # invalid extended columns
+    assert not orc.params_ex_valid(_short_period_row(rb=0.0)[0])
+    assert not orc.params_ex_valid(_short_period_row(locked=0.5)[0])
+    assert not orc.params_ex_valid(_short_period_row(rc=6.0)[0])
+    assert np.all(np.isnan(orc.lightcurve_ex(_short_period_row(rb=-1.0), t)))
+
+
+def test_ex_uniform_depth_is_the_projected_area():
+    """Uniform limb darkening, outline wholly inside the disc: 1 - F = dx * dy2 (pin P2), with the
+    outline of eqs. 11-13 (free) or of eqs. B14-B16 at alpha = 2 pi (t - t0)/P, sin(beta) = b/(a/R*)
+    (locked) -- computed here from the outline functions alone."""
+    for kw in (dict(rb=0.8, rc=0.6, zeta=0.4), dict(rb=1.3, rc=0.7, zeta=-0.9, xi=-0.4)):
+        free = _short_period_row(**kw)
+        lock = _short_period_row(locked=1.0, **kw)
+        a, b, c = 0.1 * 0.6, 0.1 * kw["rb"], 0.1 * kw["rc"]
+        ts = np.array([-0.05, -0.03, 0.0, 0.02, 0.045])
+        Ff = orc.lightcurve_ex(free, ts)[0]
+        Fl = orc.lightcurve_ex(lock, ts)[0]
+        d0 = orc.outline(a, b, c, kw["zeta"], 0.3, kw.get("xi", 0.5))
+        assert np.abs((1 - Ff) - d0[0] * d0[2]).max() < 1e-13
+        beta = np.arcsin(0.3 / 6.0)
+        for t, F in zip(ts, Fl):
+            dl = orc.outline_locked(a, b, c, kw["zeta"], 0.3, kw.get("xi", 0.5), 2 * np.pi * t / 3.0, beta)
+            assert abs((1 - F) - dl[0] * dl[2]) < 1e-13
+        # a locked triaxial body does change its projected area along the chord
+        assert np.ptp(1 - Fl) > 1e-5 and np.ptp(1 - Ff) < 1e-13
+
+
+def test_ex_locked_brute_force_pixels():
+    """One locked, limb-darkened, limb-crossing sample against a pixel sum over the outline
+    obtained by PROJECTING the rotated ellipsoid point by point (eq. B13), not from B14-B16."""
+    kw = dict(rb=0.7, rc=1.2, zeta=0.3, u1=0.4, u2=0.25, b=0.5, locked=1.0)
+    p = _short_period_row(**kw)
+    t = 0.069                                  # ingress: the outline straddles the limb
+    F = orc.lightcurve_ex(p, np.array([t]))[0, 0]
+    al, be = 2 * np.pi * t / 3.0, np.arcsin(0.5 / 6.0)
+    x0, y0, front = orc.position(p[0, :12], t)
+    assert front and 0.9 < np.hypot(x0, y0) < 1.1
+    # eq. B13: x' = R [Rx(-al) Ry(be) x + (0,0,d)] takes OBSERVER coordinates x to BODY coordinates
+    # x' (the ellipsoid's axes are the primed ones), so the body seen by the observer is x = M^T x' 
+    R = np.array(orc.rotation(0.3, 0.3, 0.5)).reshape(3, 3)
+    ca, sa, cb, sb = np.cos(al), np.sin(al), np.cos(be), np.sin(be)
+    Rx = np.array([[1, 0, 0], [0, ca, sa], [0, -sa, ca]])          # Rx(-alpha), eq. 3
+    Ry = np.array([[cb, 0, sb], [0, 1, 0], [-sb, 0, cb]])          # Ry(beta), eq. 4
+    M = R @ Rx @ Ry
+    S = np.diag([0.06, 0.07, 0.12]) ** 2
+    C = (M.T @ S @ M)[:2, :2]                  # covariance of the projected outline
+    Ci = np.linalg.inv(C)
+    n = 3000
+    h = 0.14
+    gx = x0 + (np.arange(n) + 0.5) * (2 * h / n) - h
+    gy = y0 + (np.arange(n) + 0.5) * (2 * h / n) - h
+    X, Y = np.meshgrid(gx, gy, indexing="ij")
+    dxp, dyp = X - x0, Y - y0
+    inside = (Ci[0, 0] * dxp * dxp + 2 * Ci[0, 1] * dxp * dyp + Ci[1, 1] * dyp * dyp <= 1.0)
+    r2 = X * X + Y * Y
+    mu = np.sqrt(np.clip(1 - r2, 0, None))
+    inten = np.where(r2 <= 1, 1 - 0.4 * (1 - mu) - 0.25 * (1 - mu) ** 2, 0.0)
+    blocked = (inten * inside).sum() * (2 * h / n) ** 2 / (np.pi * (1 - 0.4 / 3 - 0.25 / 6))
+    assert abs((1 - F) - blocked) < 3e-6
