@@ -52,6 +52,7 @@ extern "C" {
 
 #define GL_NPARAMS 12
 #define GL_NGEOM 6
+#define GL_NPARAMS_EX 16   /* extended row of gl_lightcurve_ex / gl_loglike_ex */
 
 typedef enum { GL_F32 = 0, GL_F64 = 1 } gl_dtype; /* arithmetic AND output precision */
 
@@ -80,6 +81,24 @@ int gl_lightcurve(const double* params, int B, const double* times, int T, doubl
 int gl_loglike(const double* params, int B, const double* times, int T, double t_exp, int n_ss,
                const double* obs, const double* sigma, void* chi2_out, void* flux_out_or_null,
                gl_dtype dtype, void* stream);
+
+/* gl_lightcurve_ex / gl_loglike_ex (NEXT-2 of SURVEY.md 8(f)): the same two calls for general
+ * triaxial ellipsoids and tidally locked planets.  params_ex [B, GL_NPARAMS_EX] row-major fp64
+ * (device): columns 0-11 as above, then
+ *   12 zeta [rad], third Euler angle of R(zeta, eta, xi) (eqs. 3-6)
+ *   13 rb, 14 rc: semi-axes b = Rp_eq rb along y', c = Rp_eq rc along z' (a = Rp_eq (1 - f) along x');
+ *      rb, rc > 0, every semi-axis < 0.5.  rb = rc = 1, zeta = 0 is the oblate model above.
+ *   15 locked: 0 = orientation fixed in the observer frame (eq. 2, eqs. 11-13);
+ *      1 = tidally locked (PAPER.md:452-466 eq. B13): the outline of EVERY sub-exposure follows
+ *      eqs. B14-B16 with alpha = the orbital angle from conjunction and sin(beta) = cos i (the
+ *      projected-ellipse geometry moves from the per-walker prelude into the per-sample loop).
+ * Any other value of column 15, or a bad axis, makes the walker invalid (NaN row, chi^2 = +inf).
+ * Everything else (layout, dtype, stream, status codes) as gl_lightcurve / gl_loglike. */
+int gl_lightcurve_ex(const double* params_ex, int B, const double* times, int T, double t_exp,
+                     int n_ss, void* flux_out, gl_dtype dtype, void* stream);
+int gl_loglike_ex(const double* params_ex, int B, const double* times, int T, double t_exp, int n_ss,
+                  const double* obs, const double* sigma, void* chi2_out, void* flux_out_or_null,
+                  gl_dtype dtype, void* stream);
 
 /* gl_flux_geometry: steps "crossings + boundary integrals" alone, for N bare geometries.
  *   geom [N, GL_NGEOM] row-major fp64 (device): (d, Rp, f_proj, PA, u1, u2) -- planet centre at

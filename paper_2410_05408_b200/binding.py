@@ -12,11 +12,11 @@ from pathlib import Path
 import numpy as np
 
 GL_F32, GL_F64 = 0, 1
-GL_NPARAMS, GL_NGEOM = 12, 6
+GL_NPARAMS, GL_NGEOM, GL_NPARAMS_EX = 12, 6, 16
 _LIBPATH = Path(__file__).resolve().parent / "csrc" / "libgreenlantern_b200.so"
 _lib = None
 
-EXPORTS = ("gl_lightcurve", "gl_loglike", "gl_flux_geometry", "gl_flux_geometry_simpson", "gl_lightcurve_host",
+EXPORTS = ("gl_lightcurve", "gl_loglike", "gl_lightcurve_ex", "gl_loglike_ex", "gl_flux_geometry", "gl_flux_geometry_simpson", "gl_lightcurve_host",
            "gl_loglike_host", "gl_flux_geometry_host", "gl_probe_peaks", "gl_launch_count", "gl_strerror",
            "gl_last_cuda_error", "gl_version")
 
@@ -38,6 +38,9 @@ def load_library():
     vp, i, d, ll = ctypes.c_void_p, ctypes.c_int, ctypes.c_double, ctypes.c_longlong
     lib.gl_lightcurve.argtypes = [vp, i, vp, i, d, i, vp, i, vp]
     lib.gl_loglike.argtypes = [vp, i, vp, i, d, i, vp, vp, vp, vp, i, vp]
+    lib.gl_lightcurve_ex.argtypes = lib.gl_lightcurve.argtypes
+    lib.gl_loglike_ex.argtypes = lib.gl_loglike.argtypes
+    lib.gl_lightcurve_ex.restype = lib.gl_loglike_ex.restype = i
     lib.gl_flux_geometry.argtypes = [vp, ll, vp, i, vp]
     lib.gl_flux_geometry_simpson.argtypes = [vp, ll, i, vp, i, vp]
     lib.gl_flux_geometry_simpson.restype = i
@@ -97,24 +100,43 @@ def _stream(x):
 
 def gl_lightcurve(params, times, t_exp=0.0, n_ss=1, dtype="f32", out=None):
     """flux[B, T] for params[B, 12] and times[T] (device tensors, fp64)."""
+    return _lightcurve("gl_lightcurve", GL_NPARAMS, params, times, t_exp, n_ss, dtype, out)
+
+
+def gl_lightcurve_ex(params_ex, times, t_exp=0.0, n_ss=1, dtype="f32", out=None):
+    """flux[B, T] for the extended rows params_ex[B, 16] (triaxial / tidally locked, NEXT-2)."""
+    return _lightcurve("gl_lightcurve_ex", GL_NPARAMS_EX, params_ex, times, t_exp, n_ss, dtype, out)
+
+
+def _lightcurve(fname, width, params, times, t_exp, n_ss, dtype, out):
     torch = _torch()
     lib = load_library()
-    params, times = _dev_f64(params, GL_NPARAMS), _dev_f64(times)
+    params, times = _dev_f64(params, width), _dev_f64(times)
     code, td = _tdtype(dtype)
     B, T = params.shape[0], times.shape[0]
     if out is None:
         out = torch.empty((B, T), dtype=td, device=params.device)
     with torch.cuda.device(params.device):
-        _check(lib.gl_lightcurve(params.data_ptr(), B, times.data_ptr(), T, float(t_exp),
-                                 int(n_ss), out.data_ptr(), code, _stream(params)))
+        _check(getattr(lib, fname)(params.data_ptr(), B, times.data_ptr(), T, float(t_exp),
+                                   int(n_ss), out.data_ptr(), code, _stream(params)))
     return out
 
 
 def gl_loglike(params, times, t_exp, n_ss, obs, sigma, dtype="f32", want_flux=False):
     """chi2[B] (and flux[B, T] when want_flux) -- one fused launch."""
+    return _loglike("gl_loglike", GL_NPARAMS, params, times, t_exp, n_ss, obs, sigma, dtype, want_flux)
+
+
+def gl_loglike_ex(params_ex, times, t_exp, n_ss, obs, sigma, dtype="f32", want_flux=False):
+    """gl_loglike for the extended rows params_ex[B, 16] (triaxial / tidally locked, NEXT-2)."""
+    return _loglike("gl_loglike_ex", GL_NPARAMS_EX, params_ex, times, t_exp, n_ss, obs, sigma, dtype,
+                    want_flux)
+
+
+def _loglike(fname, width, params, times, t_exp, n_ss, obs, sigma, dtype, want_flux):
     torch = _torch()
     lib = load_library()
-    params, times = _dev_f64(params, GL_NPARAMS), _dev_f64(times)
+    params, times = _dev_f64(params, width), _dev_f64(times)
     obs, sigma = _dev_f64(obs), _dev_f64(sigma)
     code, td = _tdtype(dtype)
     B, T = params.shape[0], times.shape[0]
@@ -123,9 +145,9 @@ def gl_loglike(params, times, t_exp, n_ss, obs, sigma, dtype="f32", want_flux=Fa
     chi2 = torch.empty((B,), dtype=td, device=params.device)
     flux = torch.empty((B, T), dtype=td, device=params.device) if want_flux else None
     with torch.cuda.device(params.device):
-        _check(lib.gl_loglike(params.data_ptr(), B, times.data_ptr(), T, float(t_exp), int(n_ss),
-                              obs.data_ptr(), sigma.data_ptr(), chi2.data_ptr(),
-                              flux.data_ptr() if want_flux else None, code, _stream(params)))
+        _check(getattr(lib, fname)(params.data_ptr(), B, times.data_ptr(), T, float(t_exp),
+                                   int(n_ss), obs.data_ptr(), sigma.data_ptr(), chi2.data_ptr(),
+                                   flux.data_ptr() if want_flux else None, code, _stream(params)))
     return (chi2, flux) if want_flux else chi2
 
 

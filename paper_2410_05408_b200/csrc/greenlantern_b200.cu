@@ -73,8 +73,85 @@ struct Walker {
     double a, b, cpsi, spsi;
     // limb darkening, already divided by the disc-integrated intensity
     double k0, k1, k2;
+    // tidally locked planets (NEXT-2): the outline changes along the orbit, so the
+    // squared semi-axes, the rows of R(zeta, eta, xi) and beta (sin(beta) = cos i) are kept, in both
+    // precisions, for the per-sample shape of locked_axes()
+    double S2[3], r[9], sinb, cosb;
+    float S2f[3], rf[9], sinbf, cosbf;
+    int locked;
     int valid;
 };
+
+// Walker::S2 / r / sinb / cosb in the compute type
+template <typename T> struct LockedView;
+template <> struct LockedView<double> {
+    static __device__ __forceinline__ const double* S2(const Walker& w) { return w.S2; }
+    static __device__ __forceinline__ const double* r(const Walker& w) { return w.r; }
+    static __device__ __forceinline__ double sinb(const Walker& w) { return w.sinb; }
+    static __device__ __forceinline__ double cosb(const Walker& w) { return w.cosb; }
+};
+template <> struct LockedView<float> {
+    static __device__ __forceinline__ const float* S2(const Walker& w) { return w.S2f; }
+    static __device__ __forceinline__ const float* r(const Walker& w) { return w.rf; }
+    static __device__ __forceinline__ float sinb(const Walker& w) { return w.sinbf; }
+    static __device__ __forceinline__ float cosb(const Walker& w) { return w.cosbf; }
+};
+
+// Semi-axes a >= b and the major-axis direction (cos psi >= 0, sin psi) of the ellipse with covariance
+// [[Cxx, Cxy], [Cxy, Cyy]] and determinant det (passed separately: eq. 13 / B16 give it without the
+// cancellation of Cxx Cyy - Cxy^2).  psi = atan2(Cxy, (Cxx - Cyy)/2) / 2 by half-angle formulas.
+template <typename R>
+__device__ __forceinline__ void axes_from_covariance(R Cxx, R Cxy, R Cyy, R det, R* a, R* b, R* cpsi,
+                                                     R* spsi) {
+    const R hd = R(0.5) * (Cxx - Cyy);
+    const R rad = glc::gsqrt(hd * hd + Cxy * Cxy);
+    *a = glc::gsqrt(R(0.5) * (Cxx + Cyy) + rad);
+    *b = glc::gsqrt(det) / *a;
+    if (!(rad > R(0))) {
+        *cpsi = R(1);
+        *spsi = R(0);
+        return;
+    }
+    const R c2 = hd / rad, s2 = Cxy / rad;
+    if (c2 >= R(0)) {
+        *cpsi = glc::gsqrt(R(0.5) * (R(1) + c2));
+        *spsi = s2 / (R(2) * *cpsi);
+    } else {
+        const R sa = glc::gsqrt(R(0.5) * (R(1) - c2));
+        *spsi = s2 < R(0) ? -sa : sa;
+        *cpsi = glc::gabs(s2) / (R(2) * sa);
+    }
+}
+
+// Outline of a tidally locked ellipsoid at orbital angle alpha (sa = sin alpha, ca = cos alpha):
+// eq. B13 maps observer coordinates x to body coordinates x' = R Rx(-alpha) Ry(beta) x + const, so
+// the body seen by the observer has covariance (M^T S M) with M = R Rx(-alpha) Ry(beta), whose sky
+// block is eqs. B14-B16:
+//   p_k = sin(beta) (r_k3 cos(alpha) + r_k2 sin(alpha)) - r_k1 cos(beta),  q_k = r_k3 sin(alpha) - r_k2 cos(alpha)
+//   Cxx = dx^2 = sum S_k p_k^2 (B14),  Cxy = dx dy1 = sum S_k p_k q_k (B15),  Cyy = sum S_k q_k^2,
+//   det = (dx dy2)^2 = S_a S_b s_c^2 + S_a S_c s_b^2 + S_b S_c s_a^2 (B16),
+//   s_k = r_k1 sin(beta) + cos(beta) (r_k3 cos(alpha) + r_k2 sin(alpha)).
+template <typename T>
+__device__ __forceinline__ void locked_axes(const Walker& w, T sa, T ca, T* a, T* b, T* cpsi, T* spsi) {
+    const T* S2 = LockedView<T>::S2(w);
+    const T* r = LockedView<T>::r(w);
+    const T sb = LockedView<T>::sinb(w), cb = LockedView<T>::cosb(w);
+    T Cxx = T(0), Cxy = T(0), Cyy = T(0), sk[3];
+#pragma unroll
+    for (int k = 0; k < 3; ++k) {
+        const T m = r[3 * k + 2] * ca + r[3 * k + 1] * sa;
+        const T p = sb * m - r[3 * k] * cb;
+        const T q = r[3 * k + 2] * sa - r[3 * k + 1] * ca;
+        sk[k] = r[3 * k] * sb + cb * m;
+        Cxx += S2[k] * p * p;
+        Cxy += S2[k] * p * q;
+        Cyy += S2[k] * q * q;
+    }
+    const T det = S2[0] * S2[1] * sk[2] * sk[2] + S2[0] * S2[2] * sk[1] * sk[1] +
+                  S2[1] * S2[2] * sk[0] * sk[0];
+    axes_from_covariance<T>(Cxx, Cxy, Cyy, det, a, b, cpsi, spsi);
+}
+
 
 // Semi-axes (a >= b) and major-axis angle psi of the sky-projected outline of an ellipsoid with
 // semi-axes (sa, sb, sc) along x', y', z' rotated by R = Rx(zeta) Ry(eta) Rz(xi)
@@ -87,7 +164,8 @@ struct Walker {
 // R = double for the validation path; float for the production path, whose per-walker constants
 // are narrowed to fp32 anyway (relative 1e-7 on a, b, psi: < 1e-8 in flux).
 template <typename R>
-__device__ void outline_axes(R sa, R sb, R sc, R zeta, R eta, R xi, R* a, R* b, R* cpsi, R* spsi) {
+__device__ void outline_axes(R sa, R sb, R sc, R zeta, R eta, R xi, R* a, R* b, R* cpsi, R* spsi,
+                             R* rows) {
     R sz, cz, se, ce, sx, cx;
     glc::gsincos(zeta, &sz, &cz);
     glc::gsincos(eta, &se, &ce);
@@ -101,16 +179,17 @@ __device__ void outline_axes(R sa, R sb, R sc, R zeta, R eta, R xi, R* a, R* b, 
     const R Cxy = A2 * r1 * r2 + B2 * r4 * r5 + C2 * r7 * r8;
     const R Cyy = A2 * r2 * r2 + B2 * r5 * r5 + C2 * r8 * r8;
     const R det = A2 * B2 * r9 * r9 + A2 * C2 * r6 * r6 + B2 * C2 * r3 * r3;
-    const R hd = R(0.5) * (Cxx - Cyy);
-    const R rad = glc::gsqrt(hd * hd + Cxy * Cxy);
-    const R lam = R(0.5) * (Cxx + Cyy) + rad;
-    *a = glc::gsqrt(lam);
-    *b = glc::gsqrt(det) / *a;
-    const R psi = (rad > R(0)) ? R(0.5) * glc::gatan2(Cxy, hd) : R(0);
-    glc::gsincos(psi, spsi, cpsi);
+    axes_from_covariance<R>(Cxx, Cxy, Cyy, det, a, b, cpsi, spsi);
+    if (rows) {
+        rows[0] = r1; rows[1] = r2; rows[2] = r3;
+        rows[3] = r4; rows[4] = r5; rows[5] = r6;
+        rows[6] = r7; rows[7] = r8; rows[8] = r9;
+    }
 }
 
-__device__ __forceinline__ bool walker_valid(const double* __restrict__ p) {
+// nparams = GL_NPARAMS (oblate, free orientation) or GL_NPARAMS_EX (NEXT-2: + zeta, b-axis/Rp_eq,
+// c-axis/Rp_eq, locked flag).
+__device__ __forceinline__ bool walker_valid(const double* __restrict__ p, int nparams) {
     const double P = p[1], aR = p[2], b = p[3], e = p[4], om = p[5];
     const double Rp = p[6], f = p[7], u1 = p[10], u2 = p[11];
     bool ok = true;
@@ -119,18 +198,33 @@ __device__ __forceinline__ bool walker_valid(const double* __restrict__ p) {
     ok = ok && (P > 0.0) && (e >= 0.0) && (e < 1.0) && (Rp > 0.0) && (Rp < 0.5) && (f >= 0.0) &&
          (f < 1.0) && (aR * (1.0 - e) > 1.0) && (norm > 0.0);
     if (ok) ok = (e == 0.0) ? (fabs(b) <= aR) : (fabs(b) * (1.0 + e * sin(om)) <= aR * (1.0 - e * e));
+    if (ok && nparams == GL_NPARAMS_EX) {
+        const double rb = p[13], rc = p[14];
+        ok = isfinite(p[12]) && isfinite(rb) && isfinite(rc) && (rb > 0.0) && (rc > 0.0) &&
+             (Rp * rb < 0.5) && (Rp * rc < 0.5) && (p[15] == 0.0 || p[15] == 1.0);
+    }
     return ok;
 }
 
 // The prelude is split in two independent halves so that two warps can run them side by side:
 // ORBIT (validity, phase constants, cos i, transit window, Kepler constants) and SHAPE (projected
 // outline, limb-darkening constants).  R as in outline_axes.
+// Largest semi-axis of the ellipsoid = upper bound of the projected semi-major axis (equal to it
+// for the oblate model, whose projected semi-major axis is the equatorial radius).
+__device__ __forceinline__ double largest_axis(const double* __restrict__ p, int nparams) {
+    double m = fmax(p[6] * (1.0 - p[7]), p[6]);
+    if (nparams == GL_NPARAMS_EX) m = fmax(p[6] * (1.0 - p[7]), fmax(p[6] * p[13], p[6] * p[14]));
+    return m;
+}
+
 template <typename R>
-__device__ void walker_prelude_orbit(const double* __restrict__ p, double t_exp, Walker* w) {
-    const bool ok = walker_valid(p);
+__device__ void walker_prelude_orbit(const double* __restrict__ p, int nparams, double t_exp, Walker* w) {
+    const bool ok = walker_valid(p, nparams);
     w->valid = ok ? 1 : 0;
     if (!ok) return;
-    const double t0 = p[0], P = p[1], aR = p[2], b = p[3], e = p[4], om = p[5], Rp = p[6];
+    const double t0 = p[0], P = p[1], aR = p[2], b = p[3], e = p[4], om = p[5];
+    const double Rp = largest_axis(p, nparams);
+    w->locked = (nparams == GL_NPARAMS_EX && p[15] == 1.0) ? 1 : 0;
     w->t0 = t0;
     w->inv_P = 1.0 / P;
     w->aR = aR;
@@ -181,18 +275,39 @@ __device__ void walker_prelude_orbit(const double* __restrict__ p, double t_exp,
     }
     w->half_win_phase = hw;
     w->reach = reach;
+    if (w->locked) {
+        // eq. 9: x0 = d cos(alpha) sin(beta)  =>  sin(beta) = cos i  (used by locked_axes)
+        w->sinb = w->cosi;
+        w->cosb = sqrt(fmax(1.0 - w->cosi * w->cosi, 0.0));
+        w->sinbf = (float)w->sinb;
+        w->cosbf = (float)w->cosb;
+    }
 }
 
 template <typename R>
-__device__ void walker_prelude_shape(const double* __restrict__ p, Walker* w) {
+__device__ void walker_prelude_shape(const double* __restrict__ p, int nparams, Walker* w) {
     const double Rp = p[6], f = p[7], xi = p[8], eta = p[9], u1 = p[10], u2 = p[11];
-    // oblate spheroid: polar semi-axis Rp (1-f) along x', equatorial Rp; zeta = 0 (R4, R5)
-    R a, b, cpsi, spsi;
-    outline_axes<R>(R(Rp * (1.0 - f)), R(Rp), R(Rp), R(0), R(eta), R(xi), &a, &b, &cpsi, &spsi);
+    // semi-axes along x', y', z': polar Rp (1-f) and, for the oblate model, equatorial Rp twice with
+    // zeta = 0 (R4, R5); the extended row gives zeta and the two other axes in units of Rp
+    const bool ex = nparams == GL_NPARAMS_EX;
+    const double sa = Rp * (1.0 - f), sb = ex ? Rp * p[13] : Rp, sc = ex ? Rp * p[14] : Rp;
+    const double zeta = ex ? p[12] : 0.0;
+    R a, b, cpsi, spsi, rows[9];
+    outline_axes<R>(R(sa), R(sb), R(sc), R(zeta), R(eta), R(xi), &a, &b, &cpsi, &spsi, rows);
     w->a = a;
     w->b = b;
     w->cpsi = cpsi;
     w->spsi = spsi;
+    if (ex && p[15] == 1.0) {   // what locked_axes() needs
+        w->S2[0] = sa * sa;
+        w->S2[1] = sb * sb;
+        w->S2[2] = sc * sc;
+        for (int k = 0; k < 3; ++k) w->S2f[k] = (float)w->S2[k];
+        for (int k = 0; k < 9; ++k) {
+            w->r[k] = rows[k];
+            w->rf[k] = (float)rows[k];
+        }
+    }
     const R pn = R(kPi * (1.0 - u1 / 3.0 - u2 / 6.0));
     w->k0 = R(1.0 - u1 - 2.0 * u2) / pn;
     w->k1 = R(u1 + 2.0 * u2) / pn;
@@ -229,12 +344,15 @@ __device__ double kepler_E(double M, double e) {
 }
 
 // fp64 position in the SKY frame (x0 along the projected orbit normal, y0 along the chord).
-__device__ bool sky_position_f64(const Walker& w, double ph, double* x0, double* y0) {
+__device__ bool sky_position_f64(const Walker& w, double ph, double* x0, double* y0, double* sphi,
+                                 double* cphi) {
     if (w.e == 0.0) {
         double s, c;
         sincospi(2.0 * ph, &s, &c);
         *x0 = w.aR * c * w.cosi;
         *y0 = w.aR * s;
+        *sphi = s;
+        *cphi = c;
         return c > 0.0;
     }
     const double M = w.Mc + kTwoPi * ph;
@@ -248,6 +366,8 @@ __device__ bool sky_position_f64(const Walker& w, double ph, double* x0, double*
     sincos(nu + w.omega - 0.5 * kPi, &sp, &cp);
     *x0 = r * cp * w.cosi;
     *y0 = r * sp;
+    *sphi = sp;
+    *cphi = cp;
     return cp > 0.0;
 }
 
@@ -290,26 +410,30 @@ template <> __device__ __forceinline__ float blocked_at<float>(const glf::TrapNo
 }
 
 // Blocked fraction delta = 1 - F_inst at reduced phase ph (a1 + a3 + a4).
-template <typename T>
+template <typename T, bool EX>
 __device__ __forceinline__ T blocked_fraction(const glf::TrapNode* trap, const Walker& w,
                                               const WalkerT<T>& v, double ph) {
-    T x0, y0;
+    T x0, y0, s, c;   // (s, c) = sine and cosine of the orbital angle from conjunction
     if (v.circular) {
         // phi = 2 pi ph, |ph| <= 1/2; narrowed AFTER the fp64 phase reduction
-        T s, c;
         glc::gsincos(T(kTwoPi * ph), &s, &c);
         if (!(c > T(0))) return T(0);
         x0 = v.aR * c * v.cosi;
         y0 = v.aR * s;
     } else {
-        double X, Y;
-        if (!sky_position_f64(w, ph, &X, &Y)) return T(0);
+        double X, Y, sphi, cphi;
+        if (!sky_position_f64(w, ph, &X, &Y, &sphi, &cphi)) return T(0);
         x0 = T(X);
         y0 = T(Y);
+        s = T(sphi);
+        c = T(cphi);
     }
-    const T xc = v.cpsi * x0 + v.spsi * y0, yc = v.cpsi * y0 - v.spsi * x0;
-    return blocked_at<T>(trap, xc, yc, v.a, v.b, v.k0, v.k1, v.k2);
+    T a = v.a, b = v.b, cpsi = v.cpsi, spsi = v.spsi;
+    if (EX && w.locked) locked_axes<T>(w, s, c, &a, &b, &cpsi, &spsi);   // outline of THIS sub-exposure
+    const T xc = cpsi * x0 + spsi * y0, yc = cpsi * y0 - spsi * x0;
+    return blocked_at<T>(trap, xc, yc, a, b, v.k0, v.k1, v.k2);
 }
+
 
 // ------------------------------------------------------------------------------------------
 // Deterministic sum of one double per thread over the CTA (fixed shuffle tree, fixed warp order).
@@ -400,15 +524,18 @@ baseline_kernel(const double* __restrict__ obs, const double* __restrict__ sigma
     for (int b = threadIdx.x; b < B; b += 1024) chi2[b] = S;
 }
 
-template <typename T>
+// EX = extended parameter rows (NEXT-2); the 12-column instantiation carries none of that code.
+template <typename T, bool EX>
 __global__ void __launch_bounds__(NT, sizeof(T) == 4 ? 8 : 2)
-transit_kernel(const double* __restrict__ params, int B, const double* __restrict__ times, int nT,
+transit_kernel(const double* __restrict__ params, int B,
+               const double* __restrict__ times, int nT,
                int tile, double t_exp, int n_ss, const double* __restrict__ obs,
                const double* __restrict__ sigma, T* __restrict__ flux, T* chi2, int shared_base) {
     cg::cluster_group cluster = cg::this_cluster();
     const int crank = (int)cluster.block_rank(), csize = (int)cluster.num_blocks();
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     constexpr int NW = NT / 32;
+    constexpr int nparams = EX ? GL_NPARAMS_EX : GL_NPARAMS;
 
     __shared__ Walker sw;
     __shared__ int s_list[MAXTILE];   // in-window time indices of this CTA's tile
@@ -441,8 +568,8 @@ transit_kernel(const double* __restrict__ params, int B, const double* __restric
     GL_TL(0);
     for (int wk = blockIdx.y; wk < B; wk += gridDim.y) {
         __syncthreads();
-        if (tid == 0) walker_prelude_orbit<T>(params + (size_t)wk * GL_NPARAMS, t_exp, &sw);
-        if (tid == 32) walker_prelude_shape<T>(params + (size_t)wk * GL_NPARAMS, &sw);
+        if (tid == 0) walker_prelude_orbit<T>(params + (size_t)wk * nparams, nparams, t_exp, &sw);
+        if (tid == 32) walker_prelude_shape<T>(params + (size_t)wk * nparams, nparams, &sw);
         __syncthreads();
         GL_TL(1);
         const bool valid = sw.valid != 0;
@@ -475,8 +602,8 @@ transit_kernel(const double* __restrict__ params, int B, const double* __restric
                             inwin = fabs(ph) < hwin;
                             isearly = inwin && !(fabs(ph) < hard_ph);
                         } else {
-                            double X, Y;
-                            sky_position_f64(sw, ph, &X, &Y);
+                            double X, Y, sphi, cphi;
+                            sky_position_f64(sw, ph, &X, &Y, &sphi, &cphi);
                             inwin = X * X + Y * Y < reach * reach;
                         }
                         if (want_chi2 && !shared_base) {
@@ -582,7 +709,7 @@ transit_kernel(const double* __restrict__ params, int B, const double* __restric
                             const double tc = times[i];
                             for (int j = my_b * JS; j < min(n_ss, (my_b + 1) * JS); ++j) {
                                 const double t = tc + (((double)j + 0.5) * inv_ss - 0.5) * t_exp;
-                                delta += blocked_fraction<T>(s_trap, sw, v, reduced_phase(sw, t));
+                                delta += blocked_fraction<T, EX>(s_trap, sw, v, reduced_phase(sw, t));
                             }
                         }
                         T sum = T(0);   // exposure mean, blocks in sub-exposure order (R18)
@@ -602,7 +729,7 @@ transit_kernel(const double* __restrict__ params, int B, const double* __restric
                         T sum = T(0);
                         for (int j = lane; j < n_ss; j += 32) {
                             const double t = tc + (((double)j + 0.5) * inv_ss - 0.5) * t_exp;
-                            sum += blocked_fraction<T>(s_trap, sw, v, reduced_phase(sw, t));
+                            sum += blocked_fraction<T, EX>(s_trap, sw, v, reduced_phase(sw, t));
                         }
 #pragma unroll
                         for (int off = 16; off > 0; off >>= 1)
@@ -775,7 +902,8 @@ void pick_shape(int B, int nT, int* C, int* tile) {
 }
 
 template <typename T>
-int launch_transit(const double* params, int B, const double* times, int nT, double t_exp, int n_ss,
+int launch_transit(const double* params, int nparams, int B, const double* times, int nT,
+                   double t_exp, int n_ss,
                    const double* obs, const double* sigma, void* flux, void* chi2,
                    cudaStream_t st) {
     int C, tile;
@@ -802,21 +930,28 @@ int launch_transit(const double* params, int B, const double* times, int nT, dou
     attr[1].val.programmaticStreamSerializationAllowed = 1;
     cfg.attrs = attr;
     cfg.numAttrs = shared_base ? 2 : 1;
-    cudaError_t e = cudaLaunchKernelEx(&cfg, transit_kernel<T>, params, B, times, nT, tile, t_exp,
-                                       n_ss, obs, sigma, (T*)flux, (T*)chi2, shared_base);
+    cudaError_t e = (nparams == GL_NPARAMS_EX)
+            ? cudaLaunchKernelEx(&cfg, transit_kernel<T, true>, params, B, times, nT, tile, t_exp, n_ss,
+                                 obs, sigma, (T*)flux, (T*)chi2, shared_base)
+            : cudaLaunchKernelEx(&cfg, transit_kernel<T, false>, params, B, times, nT, tile, t_exp, n_ss,
+                                 obs, sigma, (T*)flux, (T*)chi2, shared_base);
     if (e != cudaSuccess && shared_base) {
         // no early start then: plain stream order is just as correct
         (void)cudaGetLastError();
         cfg.numAttrs = 1;
-        e = cudaLaunchKernelEx(&cfg, transit_kernel<T>, params, B, times, nT, tile, t_exp, n_ss, obs,
-                               sigma, (T*)flux, (T*)chi2, shared_base);
+        e = (nparams == GL_NPARAMS_EX)
+                ? cudaLaunchKernelEx(&cfg, transit_kernel<T, true>, params, B, times, nT, tile, t_exp,
+                                     n_ss, obs, sigma, (T*)flux, (T*)chi2, shared_base)
+                : cudaLaunchKernelEx(&cfg, transit_kernel<T, false>, params, B, times, nT, tile, t_exp,
+                                     n_ss, obs, sigma, (T*)flux, (T*)chi2, shared_base);
     }
     if (e != cudaSuccess) return cuda_fail(e, "transit_kernel launch");
     ++tl_launches;
     return GL_OK;
 }
 
-int run_transit(const double* params, int B, const double* times, int nT, double t_exp, int n_ss,
+int run_transit(const double* params, int nparams, int B, const double* times, int nT, double t_exp,
+                int n_ss,
                 const double* obs, const double* sigma, void* flux, void* chi2, gl_dtype dtype,
                 void* stream, bool need_flux, bool need_chi2) {
     if (B < 0 || nT < 0 || n_ss < 1 || !(t_exp >= 0.0) || !isfinite(t_exp)) return GL_EINVAL;
@@ -831,9 +966,10 @@ int run_transit(const double* params, int B, const double* times, int nT, double
     if (rc != GL_OK) return rc;
     cudaStream_t st = (cudaStream_t)stream;
     return dtype == GL_F32
-               ? launch_transit<float>(params, B, times, nT, t_exp, n_ss, obs, sigma, flux, chi2, st)
-               : launch_transit<double>(params, B, times, nT, t_exp, n_ss, obs, sigma, flux, chi2,
-                                        st);
+               ? launch_transit<float>(params, nparams, B, times, nT, t_exp, n_ss, obs, sigma, flux,
+                                       chi2, st)
+               : launch_transit<double>(params, nparams, B, times, nT, t_exp, n_ss, obs, sigma, flux,
+                                        chi2, st);
 }
 
 }  // namespace
@@ -842,15 +978,28 @@ extern "C" {
 
 int gl_lightcurve(const double* params, int B, const double* times, int T, double t_exp, int n_ss,
                   void* flux_out, gl_dtype dtype, void* stream) {
-    return run_transit(params, B, times, T, t_exp, n_ss, nullptr, nullptr, flux_out, nullptr, dtype,
-                       stream, true, false);
+    return run_transit(params, GL_NPARAMS, B, times, T, t_exp, n_ss, nullptr, nullptr, flux_out,
+                       nullptr, dtype, stream, true, false);
+}
+
+int gl_lightcurve_ex(const double* params_ex, int B, const double* times, int T, double t_exp,
+                     int n_ss, void* flux_out, gl_dtype dtype, void* stream) {
+    return run_transit(params_ex, GL_NPARAMS_EX, B, times, T, t_exp, n_ss, nullptr, nullptr, flux_out,
+                       nullptr, dtype, stream, true, false);
+}
+
+int gl_loglike_ex(const double* params_ex, int B, const double* times, int T, double t_exp, int n_ss,
+                  const double* obs, const double* sigma, void* chi2_out, void* flux_out_or_null,
+                  gl_dtype dtype, void* stream) {
+    return run_transit(params_ex, GL_NPARAMS_EX, B, times, T, t_exp, n_ss, obs, sigma,
+                       flux_out_or_null, chi2_out, dtype, stream, false, true);
 }
 
 int gl_loglike(const double* params, int B, const double* times, int T, double t_exp, int n_ss,
                const double* obs, const double* sigma, void* chi2_out, void* flux_out_or_null,
                gl_dtype dtype, void* stream) {
-    return run_transit(params, B, times, T, t_exp, n_ss, obs, sigma, flux_out_or_null, chi2_out,
-                       dtype, stream, false, true);
+    return run_transit(params, GL_NPARAMS, B, times, T, t_exp, n_ss, obs, sigma, flux_out_or_null,
+                       chi2_out, dtype, stream, false, true);
 }
 
 int gl_flux_geometry(const double* geom, long long N, void* flux_out, gl_dtype dtype,

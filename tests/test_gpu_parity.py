@@ -290,3 +290,68 @@ def test_paper_snap_simpson_kernel(gl, dtype):
     bad = geom[:4].copy()
     bad[1, 1] = 0.7
     assert np.isnan(host(gl.gl_flux_geometry_simpson(dev(bad), 64, dtype=dtype))[1])
+
+
+def _ex_rows(B, seed, locked):
+    """Short-period planets (a/R* ~ 4-8: the orbital angle sweeps +-0.2 rad in transit, so locking
+    matters), triaxial axes, all three Euler angles; circular and eccentric."""
+    rng = np.random.default_rng(seed)
+    p = np.zeros((B, 16))
+    p[:, 0] = rng.normal(0, 0.002, B)             # t0
+    p[:, 1] = rng.uniform(2.5, 4.0, B)            # P
+    p[:, 2] = rng.uniform(4.0, 8.0, B)            # a/R*
+    p[:, 3] = rng.uniform(-0.7, 0.9, B)           # b (signed; some grazing)
+    p[:, 4] = np.where(rng.random(B) < 0.3, rng.uniform(0.05, 0.4, B), 0.0)
+    p[:, 5] = rng.uniform(0, 2 * np.pi, B)
+    p[:, 6] = rng.uniform(0.05, 0.15, B)          # Rp_eq
+    p[:, 7] = rng.uniform(0.0, 0.7, B)            # f
+    p[:, 8] = rng.uniform(-np.pi, np.pi, B)       # xi
+    p[:, 9] = rng.uniform(-np.pi / 2, np.pi / 2, B)
+    q1, q2 = rng.random(B), rng.random(B)
+    p[:, 10], p[:, 11] = 2 * np.sqrt(q1) * q2, np.sqrt(q1) * (1 - 2 * q2)
+    p[:, 12] = rng.uniform(-np.pi, np.pi, B)      # zeta
+    p[:, 13] = rng.uniform(0.4, 1.5, B)           # b-axis / Rp_eq
+    p[:, 14] = rng.uniform(0.4, 1.5, B)           # c-axis / Rp_eq
+    p[:, 15] = locked
+    return p
+
+
+@pytest.mark.parametrize("dtype", ["f32", "f64"])
+@pytest.mark.parametrize("locked", [0.0, 1.0])
+def test_extended_rows_triaxial_and_locked(gl, dtype, locked):
+    """NEXT-2: gl_loglike_ex / gl_lightcurve_ex against oracle.lightcurve_ex."""
+    p = _ex_rows(48, 31 + int(locked), locked)
+    assert all(orc.params_ex_valid(r) for r in p)
+    t = np.linspace(-0.32, 0.32, 1500)            # +- 2.3 h around t0 at 37 s cadence, ragged
+    rng = np.random.default_rng(8)
+    obs = 1.0 - 0.005 * np.exp(-(t / 0.05) ** 2) + 1e-4 * rng.standard_normal(t.size)
+    sig = np.full(t.size, 1e-4)
+    ref = orc.lightcurve_ex(p, t, 0.004, 5)
+    chi_ref = (((obs - ref) / sig) ** 2).sum(axis=1)
+    chi, out = gl.gl_loglike_ex(dev(p), dev(t), 0.004, 5, dev(obs), dev(sig), dtype=dtype,
+                                want_flux=True)
+    err = np.abs(host(out) - ref)
+    assert err.max() <= FTOL[dtype], (err.max(), np.unravel_index(err.argmax(), err.shape))
+    assert np.abs(host(chi) / chi_ref - 1.0).max() <= CTOL[dtype]
+    assert (ref < 1.0).sum() > 5000
+    lc = gl.gl_lightcurve_ex(dev(p), dev(t), 0.004, 5, dtype=dtype)
+    assert np.array_equal(host(lc), host(out))
+    if locked:
+        # locking really changes these curves (else the test would not see a wrong alpha)
+        free = p.copy()
+        free[:, 15] = 0.0
+        assert np.abs(orc.lightcurve_ex(free, t, 0.004, 5) - ref).max() > 1e-4
+    # the extended row with the oblate defaults is the 12-column model (two instantiations of the
+    # kernel: equal up to the rounding of differently contracted FMAs)
+    q = wl.config3(B=8).params
+    q16 = np.concatenate([q, np.tile([0.0, 1.0, 1.0, 0.0], (8, 1))], axis=1)
+    w = wl.config3(B=8)
+    a = gl.gl_lightcurve_ex(dev(q16), dev(w.times[1900:2000]), w.t_exp, 3, dtype=dtype)
+    b = gl.gl_lightcurve(dev(q), dev(w.times[1900:2000]), w.t_exp, 3, dtype=dtype)
+    assert np.abs(host(a) - host(b)).max() <= (2e-7 if dtype == "f32" else 1e-14)
+    # invalid extended columns: NaN row
+    bad = p[:3].copy()
+    bad[1, 15] = 0.5
+    bad[2, 13] = -1.0
+    o = host(gl.gl_lightcurve_ex(dev(bad), dev(t[:64]), 0.0, 1, dtype=dtype))
+    assert np.all(np.isfinite(o[0])) and np.all(np.isnan(o[1])) and np.all(np.isnan(o[2]))
