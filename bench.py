@@ -46,6 +46,15 @@ def make_workload(name, rank):
         w = wl.config4()
         if rank:
             w.params = wl.draw_walkers(w.B, wl.SEED_CFG4_WALKERS + 1000 * rank)
+    elif name in ("cfg4ex_free", "cfg4ex_locked"):
+        # NEXT-2 context lines: config 4's batch with the extended rows of gl_loglike_ex (triaxial
+        # axes 1 : 0.9 : 1.1 x (1-f), zeta = 0.3 rad), orientation free or tidally locked
+        w = wl.config4()
+        if rank:
+            w.params = wl.draw_walkers(w.B, wl.SEED_CFG4_WALKERS + 1000 * rank)
+        ext = np.tile([0.3, 0.9, 1.1, 1.0 if name.endswith("locked") else 0.0], (w.B, 1))
+        w.params = np.concatenate([w.params, ext], axis=1)
+        w.name = w.name.replace("cfg4", name)
     else:
         raise SystemExit(f"unknown workload {name}")
     return w
@@ -141,7 +150,8 @@ def main():
     ap.add_argument("--gpus", type=int, default=1)
     ap.add_argument("--steps", type=int, default=50)
     ap.add_argument("--warmup", type=int, default=5)
-    ap.add_argument("--workload", default="cfg3", choices=["cfg3", "cfg4"])
+    ap.add_argument("--workload", default="cfg3",
+                    choices=["cfg3", "cfg4", "cfg4ex_free", "cfg4ex_locked"])
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
     args = ap.parse_args()
@@ -171,8 +181,11 @@ def main():
     P, Tm, O, S = d(w.params), d(w.times), d(w.obs), d(w.sigma)
     flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)   # > 126 MB L2
 
+    extended = w.params.shape[1] == 16
+    loglike = gl.gl_loglike_ex if extended else gl.gl_loglike
+
     def step():
-        return gl.gl_loglike(P, Tm, w.t_exp, w.n_ss, O, S, dtype="f32", want_flux=True)
+        return loglike(P, Tm, w.t_exp, w.n_ss, O, S, dtype="f32", want_flux=True)
 
     def barrier():
         if dist is not None:
@@ -227,14 +240,30 @@ def main():
     hp, ht, ho, hs = pin(w.params), pin(w.times), pin(w.obs), pin(w.sigma)
     c_h = torch.empty(w.B, dtype=torch.float32).pin_memory().numpy()          # pinned outputs too
     f_h = torch.empty((w.B, w.T), dtype=torch.float32).pin_memory().numpy()
+    if extended:
+        # no host-pointer variant of the _ex entry points: the same copies, issued from here
+        pins = [torch.from_numpy(x) for x in (hp, ht, ho, hs)]
+        c_t, f_t = torch.from_numpy(c_h), torch.from_numpy(f_h)
+
+        def e2e_call():
+            for dst, src in zip((P, Tm, O, S), pins):
+                dst.copy_(src, non_blocking=True)
+            chi2_d, flux_d = step()
+            c_t.copy_(chi2_d, non_blocking=True)
+            f_t.copy_(flux_d, non_blocking=True)
+            torch.cuda.synchronize()
+        api = "gl_loglike_ex + pinned H2D/D2H copies issued by bench.py (wall clock over K calls)"
+    else:
+        def e2e_call():
+            gl.gl_loglike_host(hp, ht, w.t_exp, w.n_ss, ho, hs, dtype="f32", want_flux=True,
+                               chi2_out=c_h, flux_out=f_h)
+        api = "gl_loglike_host (pinned host inputs and outputs, wall clock over K calls)"
     for _ in range(3):
-        gl.gl_loglike_host(hp, ht, w.t_exp, w.n_ss, ho, hs, dtype="f32", want_flux=True,
-                           chi2_out=c_h, flux_out=f_h)
+        e2e_call()
     barrier()
     t0 = time.perf_counter()
     for _ in range(K):
-        gl.gl_loglike_host(hp, ht, w.t_exp, w.n_ss, ho, hs, dtype="f32", want_flux=True,
-                           chi2_out=c_h, flux_out=f_h)
+        e2e_call()
     e2e_s = time.perf_counter() - t0
     te = torch.tensor([e2e_s], device=dev, dtype=torch.float64)
     if dist is not None:
@@ -281,10 +310,10 @@ def main():
         "wall_ms_per_step_incl_flush": 1e3 * wall / K,
         "clocks": clocks, "gpu_launches": int(launches),
         "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": h2d,
-                "d2h_bytes_per_step": d2h, "api": "gl_loglike_host (pinned host inputs and outputs, wall clock over K calls)"},
+                "d2h_bytes_per_step": d2h, "api": api},
         "roofline": roofline,
     }
-    if world == 1 and not args.no_cpu_baseline:
+    if world == 1 and not args.no_cpu_baseline and not extended:
         v, used, dt = oracle_timed(w, repeat=1)
         out["cpu_baseline"] = {"value": v, "unit": UNIT, "cores": used, "kind": "oracle",
                                "sample": f"whole workload {w.name} once ({dt:.2f} s), OpenMP over (walker,time)"}
