@@ -271,6 +271,19 @@ def main():
     e2e_value = evals_per_step * K / float(te.item())
     h2d = int(hp.nbytes + ht.nbytes + ho.nbytes + hs.nbytes)
     d2h = int(c_h.nbytes + f_h.nbytes)
+    # what an MCMC caller needs back is chi2[B] alone (flux never leaves the GPU): same call, no flux
+    e2e_chi2_only = None
+    if not extended:
+        for _ in range(3):
+            gl.gl_loglike_host(hp, ht, w.t_exp, w.n_ss, ho, hs, dtype="f32", chi2_out=c_h)
+        barrier()
+        t0 = time.perf_counter()
+        for _ in range(K):
+            gl.gl_loglike_host(hp, ht, w.t_exp, w.n_ss, ho, hs, dtype="f32", chi2_out=c_h)
+        tc = torch.tensor([time.perf_counter() - t0], device=dev, dtype=torch.float64)
+        if dist is not None:
+            dist.all_reduce(tc, op=dist.ReduceOp.MAX)
+        e2e_chi2_only = evals_per_step * K / float(tc.item())
 
     if rank != 0:
         if dist is not None:
@@ -310,7 +323,8 @@ def main():
         "wall_ms_per_step_incl_flush": 1e3 * wall / K,
         "clocks": clocks, "gpu_launches": int(launches),
         "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": h2d,
-                "d2h_bytes_per_step": d2h, "api": api},
+                "d2h_bytes_per_step": d2h, "api": api,
+                "chi2_only_value": e2e_chi2_only, "chi2_only_d2h_bytes_per_step": int(c_h.nbytes)},
         "roofline": roofline,
     }
     if world == 1 and not args.no_cpu_baseline and not extended:
