@@ -63,6 +63,12 @@ def _load():
         lib.gl_oracle_lightcurve.argtypes = [_dp, i, _dp, i, d, i, _dp, i]
         lib.gl_oracle_lightcurve_ex.argtypes = [_dp, i, _dp, i, d, i, _dp, i]
         lib.gl_oracle_params_ex_valid.argtypes = [_dp]
+        lib.gl_oracle_munu_of.argtypes = [d, d, _dp]
+        lib.gl_oracle_feta_of.argtypes = [d, d, _dp]
+        lib.gl_oracle_log_prior_munu.argtypes = [d, d]
+        lib.gl_oracle_log_prior_munu.restype = d
+        lib.gl_oracle_munu_from_uniform.argtypes = [d, d, _dp]
+        lib.gl_oracle_params_from_munu.argtypes = [_dp, _dp, _dp]
         lib.gl_oracle_lightcurve.restype = i
         lib.gl_oracle_loglike.argtypes = [_dp, i, _dp, i, d, i, _dp, _dp, _dp, _dp, i]
         lib.gl_oracle_loglike.restype = i
@@ -170,6 +176,47 @@ def lightcurve_ex(params16, times, t_exp=0.0, n_ss=1, nthreads=0):
 def params_ex_valid(params16):
     p, pp = _c(params16)
     return bool(_load().gl_oracle_params_ex_valid(pp))
+
+
+def munu_of(f, eta):
+    """(mu, nu) of eqs. A1, A4."""
+    o = np.zeros(2)
+    _load().gl_oracle_munu_of(float(f), float(eta), o.ctypes.data_as(_dp))
+    return o
+
+
+def feta_of(mu, nu):
+    """(f, eta) from eqs. A2-A3 and A1 solved for eta in [0, pi/2]."""
+    o = np.zeros(2)
+    _load().gl_oracle_feta_of(float(mu), float(nu), o.ctypes.data_as(_dp))
+    return o
+
+
+def log_prior_munu(mu, nu):
+    """ln p(mu, nu), eq. A6."""
+    return _load().gl_oracle_log_prior_munu(float(mu), float(nu))
+
+
+def munu_from_uniform(u, w):
+    """(mu, nu) drawn by inverse-transform sampling, eqs. A10, A12."""
+    o = np.zeros(2)
+    _load().gl_oracle_munu_from_uniform(float(u), float(w), o.ctypes.data_as(_dp))
+    return o
+
+
+def params_from_munu(sampling):
+    """Sampling rows [B,12] (t0,P,a/R*,b,e,omega,r_mean,mu,nu,xi,q1,q2) -> (model rows [B,12],
+    ln p(mu,nu) [B])."""
+    srows, _ = _c(np.atleast_2d(sampling))
+    out = np.empty_like(srows)
+    lp = np.empty(srows.shape[0])
+    one = np.zeros(1)
+    for k in range(srows.shape[0]):
+        r, rp = _c(srows[k])
+        o = np.zeros(12)
+        _load().gl_oracle_params_from_munu(rp, o.ctypes.data_as(_dp), one.ctypes.data_as(_dp))
+        out[k], lp[k] = o, one[0]
+    return out, lp
 
 
 def loglike(params, times, t_exp, n_ss, obs, sigma, nthreads=0, return_threads=False):

@@ -547,6 +547,73 @@ double gl_oracle_flux_time_ex(const double *p, double t, double t_exp, int n_ss)
     return sum / n_ss;
 }
 
+/* ------------------------------------------------------------------------ */
+/* NEXT-3: the paper's sampling parameters (App. A,           */
+/* PAPER.md:366-430).  mu, nu replace (f, eta); q1, q2 replace (u1, u2)        */
+/* (Kipping's map, as in BASELINE.json config 3); the mean radius r replaces   */
+/* the equatorial one, R_eq = r / (1-f)^(1/3) (volume-equivalent sphere:       */
+/* a b c = R_eq^3 (1-f); SURVEY.md ambiguity 22).                              */
+/* ------------------------------------------------------------------------ */
+
+/* eqs. A1 and A4: (f, eta) -> (mu, nu). */
+void gl_oracle_munu_of(double f, double eta, double *out2) {
+    const double c2 = cos(2.0 * eta), g = f * (f - 2.0);
+    out2[0] = (f - 1.0) * (f - 1.0) + g * c2;                                         /* A1 */
+    out2[1] = (2.0 + 2.0 * g * cos(eta) * cos(eta) + (f - 1.0) * sqrt(4.0 + 2.0 * g * (1.0 + c2))) /
+              (2.0 + g * (1.0 + c2));                                                 /* A4 */
+}
+
+/* eqs. A2-A3 and A1 solved for eta in [0, pi/2]: (mu, nu) -> (f, eta). */
+void gl_oracle_feta_of(double mu, double nu, double *out2) {
+    const double fmin = 1.0 - sqrt(0.5 * (mu + 1.0));                                 /* A2 */
+    const double f = fmin + (1.0 - fmin) * nu;                                        /* A3 */
+    double c2 = (f > 0.0) ? (mu - (f - 1.0) * (f - 1.0)) / (f * (f - 2.0)) : 1.0;     /* A1 */
+    if (c2 > 1.0) c2 = 1.0;
+    if (c2 < -1.0) c2 = -1.0;
+    out2[0] = f;
+    out2[1] = 0.5 * acos(c2);
+}
+
+/* eq. A6: ln p(mu, nu). */
+double gl_oracle_log_prior_munu(double mu, double nu) {
+    const double q = nu * (nu - 2.0) * (mu * (nu - 1.0) * (nu - 1.0) + nu * (nu - 2.0) - 1.0);
+    if (!(mu > -1.0 && mu < 1.0 && nu > 0.0 && nu <= 1.0) || !(q > 0.0)) return -INFINITY;
+    return -1.5 * log(2.0) - 0.5 * log(q);
+}
+
+/* eqs. A10 and A12: two uniform variates (u, w) -> (mu, nu) distributed as eq. A6. */
+void gl_oracle_munu_from_uniform(double u, double w, double *out2) {
+    const double nu = u * u / (u * u - 2.0 * u + 2.0);                                /* A10 */
+    const double s = sqrt(nu * (2.0 - nu)), d = (nu - 1.0) * (nu - 1.0);
+    out2[0] = (4.0 * w + 4.0 * (w * w - w) * s + 2.0 * (nu * (nu - 2.0) - 1.0) * w * w - d) / d; /* A12 */
+    out2[1] = nu;
+}
+
+/* Sampling row (t0, P, a/R*, b, e, omega, r_mean, mu, nu, xi, q1, q2) -> model row
+ * (t0, P, a/R*, b, e, omega, Rp_eq, f, xi, eta, u1, u2) and ln p(mu, nu).  A row outside
+ * mu in (-1,1), nu in (0,1], q1, q2 in [0,1], r_mean > 0 gives NaNs and -inf. */
+void gl_oracle_params_from_munu(const double *srow, double *prow, double *logprior) {
+    const double r = srow[6], mu = srow[7], nu = srow[8], q1 = srow[10], q2 = srow[11];
+    const double lp = gl_oracle_log_prior_munu(mu, nu);
+    int ok = isfinite(lp) && (r > 0.0) && (q1 >= 0.0 && q1 <= 1.0) && (q2 >= 0.0 && q2 <= 1.0);
+    for (int k = 0; k < 12; k++) ok = ok && isfinite(srow[k]);
+    if (!ok) {
+        for (int k = 0; k < 12; k++) prow[k] = NAN;
+        if (logprior) *logprior = -INFINITY;
+        return;
+    }
+    double fe[2];
+    gl_oracle_feta_of(mu, nu, fe);
+    for (int k = 0; k < 6; k++) prow[k] = srow[k];
+    prow[6] = r / cbrt(1.0 - fe[0]);
+    prow[7] = fe[0];
+    prow[8] = srow[9];
+    prow[9] = fe[1];
+    prow[10] = 2.0 * sqrt(q1) * q2;
+    prow[11] = sqrt(q1) * (1.0 - 2.0 * q2);
+    if (logprior) *logprior = lp;
+}
+
 static int pick_threads(int nthreads) {
 #ifdef _OPENMP
     if (nthreads <= 0) nthreads = omp_get_max_threads();

@@ -663,3 +663,71 @@ def test_ex_locked_brute_force_pixels():
     inten = np.where(r2 <= 1, 1 - 0.4 * (1 - mu) - 0.25 * (1 - mu) ** 2, 0.0)
     blocked = (inten * inside).sum() * (2 * h / n) ** 2 / (np.pi * (1 - 0.4 / 3 - 0.25 / 6))
     assert abs((1 - F) - blocked) < 3e-6
+
+
+# ---------------------------------------------------------------------------------------------
+# NEXT-3: the sampling parameters of App. A.  Pins: the forward map (A1, A4)
+# against the defining relations A2-A3; the Jacobian A5 by finite differences; A6 |det J| = cos(eta)
+# (eq. A7, with its normalisation); the sampler A10/A12 by a Monte-Carlo test of what it is FOR
+# (f uniform, eta cosine-distributed), which goes through the inverse map as well; and App. A's
+# physical claim (equal mu, equal R_eq => identical light curves) through the whole front end.
+# ---------------------------------------------------------------------------------------------
+def test_munu_forward_inverse_and_jacobian():
+    rng = np.random.default_rng(21)
+    for _ in range(200):
+        f, eta = rng.uniform(0.01, 0.97), rng.uniform(0.02, PI / 2 - 0.02)
+        mu, nu = orc.munu_of(f, eta)
+        # A1 by its own definition and A3 through A2
+        assert abs(mu - ((f - 1) ** 2 + f * (f - 2) * np.cos(2 * eta))) < 1e-15
+        fmin = 1 - np.sqrt((mu + 1) / 2)
+        assert abs(f - (fmin + (1 - fmin) * nu)) < 1e-13
+        assert -1 < mu < 1 and 0 < nu <= 1
+        f2, eta2 = orc.feta_of(mu, nu)
+        assert abs(f2 - f) < 1e-13 and abs(eta2 - eta) < 1e-9 / max(np.sin(2 * eta), 1e-3)
+        # eq. A5 by central differences of the forward map
+        h = 1e-6
+        J = np.array([(orc.munu_of(f + h, eta) - orc.munu_of(f - h, eta)) / (2 * h),
+                      (orc.munu_of(f, eta + h) - orc.munu_of(f, eta - h)) / (2 * h)]).T
+        detJ = np.linalg.det(J)
+        A5 = 2 ** 1.5 * f * (f - 2) * np.sin(2 * eta) / np.sqrt(2 + f * (f - 2) * (1 + np.cos(2 * eta)))
+        assert abs(detJ - A5) < 1e-6 * max(1.0, abs(A5))
+        # eq. A6 |det J| = cos(eta): eq. A7 including the constant (uniform f on [0,1], cos eta on [0, pi/2])
+        assert abs(np.exp(orc.log_prior_munu(mu, nu)) * abs(A5) - np.cos(eta)) < 1e-9
+    assert orc.log_prior_munu(1.2, 0.5) == -np.inf and orc.log_prior_munu(0.2, 0.0) == -np.inf
+
+
+def test_munu_sampler_gives_uniform_f_and_cosine_eta():
+    from scipy import stats
+    rng = np.random.default_rng(22)
+    n = 40_000
+    f, eta = np.empty(n), np.empty(n)
+    for k, (u, w) in enumerate(rng.random((n, 2))):
+        mu, nu = orc.munu_from_uniform(u, w)
+        f[k], eta[k] = orc.feta_of(mu, nu)
+    assert stats.kstest(f, "uniform").pvalue > 1e-3                 # p(f) = 1 on [0, 1]
+    assert stats.kstest(np.sin(eta), "uniform").pvalue > 1e-3       # p(eta) = cos(eta): CDF sin(eta)
+    assert abs(np.corrcoef(f, np.sin(eta))[0, 1]) < 0.02            # and independent (eq. A7)
+
+
+def test_params_from_munu_front_end():
+    # two (f, eta) pairs on one mu contour, same equatorial radius: identical curves (App. A, R22)
+    f1, eta1 = 0.5, 0.9
+    mu, _ = orc.munu_of(f1, eta1)
+    f2 = 0.3
+    eta2 = 0.5 * np.arccos((mu - (f2 - 1) ** 2) / (f2 * (f2 - 2)))
+    rows = []
+    for f, eta in ((f1, eta1), (f2, eta2)):
+        m, n = orc.munu_of(f, eta)
+        assert abs(m - mu) < 1e-14
+        rows.append([0.0, 10.0, 20.0, 0.3, 0.0, 0.0, 0.1 * (1 - f) ** (1 / 3), m, n, 0.5, 0.36, 0.3])
+    p, lp = orc.params_from_munu(rows)
+    assert np.allclose(p[:, 6], 0.1, rtol=1e-14) and np.allclose(p[:, 7], [f1, f2], atol=1e-13)
+    assert np.allclose(p[:, 9], [eta1, eta2], atol=1e-12)
+    # Kipping: u1 = 2 sqrt(q1) q2, u2 = sqrt(q1)(1 - 2 q2)  <=>  q1 = (u1 + u2)^2, q2 = u1 / (2 (u1 + u2))
+    assert np.allclose((p[:, 10] + p[:, 11]) ** 2, 0.36) and np.allclose(p[:, 10] / (2 * (p[:, 10] + p[:, 11])), 0.3)
+    t = np.linspace(-0.15, 0.15, 61)
+    a, b = orc.lightcurve(p[:1], t), orc.lightcurve(p[1:], t)
+    assert np.abs(a - b).max() < 1e-13 and a.min() < 0.995
+    assert np.all(np.isfinite(lp))
+    bad, lpb = orc.params_from_munu([[0, 10, 20, 0.3, 0, 0, 0.1, 1.5, 0.5, 0.5, 0.3, 0.3]])
+    assert np.all(np.isnan(bad)) and lpb[0] == -np.inf
