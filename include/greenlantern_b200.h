@@ -100,6 +100,20 @@ int gl_loglike_ex(const double* params_ex, int B, const double* times, int T, do
                   const double* obs, const double* sigma, void* chi2_out, void* flux_out_or_null,
                   gl_dtype dtype, void* stream);
 
+/* gl_params_from_munu (NEXT-3 of SURVEY.md 8(f)): the paper's SAMPLING parameters (App. A,
+ * PAPER.md:366-430) -> the model rows gl_lightcurve / gl_loglike take, on the device.
+ *   sampling [B, 12] fp64 (device): t0, P, a/R*, b, e, omega, r_mean, mu, nu, xi, q1, q2
+ *     r_mean = volume-equivalent radius ratio (R_eq = r_mean / (1-f)^(1/3)); mu in (-1, 1),
+ *     nu in (0, 1] (eqs. A1-A4); q1, q2 in [0, 1] (u1 = 2 sqrt(q1) q2, u2 = sqrt(q1)(1 - 2 q2)).
+ *   params_out [B, GL_NPARAMS] fp64 (device), fully overwritten; f by eqs. A2-A3, eta in [0, pi/2]
+ *     by eq. A1.  logprior_out_or_null [B] fp64: ln p(mu, nu) of eq. A6.
+ * A row outside the domain gives a NaN row (an invalid walker downstream) and -inf.
+ * gl_munu_from_uniform: uw [B, 2] uniform variates in [0, 1] -> munu_out [B, 2] distributed as eq. A6
+ * (inverse-transform sampling, eqs. A10 and A12).  Both are fp64 only and enqueue one launch. */
+int gl_params_from_munu(const double* sampling, int B, double* params_out,
+                        double* logprior_out_or_null, void* stream);
+int gl_munu_from_uniform(const double* uw, int B, double* munu_out, void* stream);
+
 /* gl_flux_geometry: steps "crossings + boundary integrals" alone, for N bare geometries.
  *   geom [N, GL_NGEOM] row-major fp64 (device): (d, Rp, f_proj, PA, u1, u2) -- planet centre at
  *   (d, 0), d >= 0; projected semi-major axis Rp (0 < Rp < 0.5) at position angle PA [rad],

@@ -16,7 +16,7 @@ GL_NPARAMS, GL_NGEOM, GL_NPARAMS_EX = 12, 6, 16
 _LIBPATH = Path(__file__).resolve().parent / "csrc" / "libgreenlantern_b200.so"
 _lib = None
 
-EXPORTS = ("gl_lightcurve", "gl_loglike", "gl_lightcurve_ex", "gl_loglike_ex", "gl_flux_geometry", "gl_flux_geometry_simpson", "gl_lightcurve_host",
+EXPORTS = ("gl_lightcurve", "gl_loglike", "gl_lightcurve_ex", "gl_loglike_ex", "gl_params_from_munu", "gl_munu_from_uniform", "gl_flux_geometry", "gl_flux_geometry_simpson", "gl_lightcurve_host",
            "gl_loglike_host", "gl_flux_geometry_host", "gl_probe_peaks", "gl_launch_count", "gl_strerror",
            "gl_last_cuda_error", "gl_version")
 
@@ -41,6 +41,9 @@ def load_library():
     lib.gl_lightcurve_ex.argtypes = lib.gl_lightcurve.argtypes
     lib.gl_loglike_ex.argtypes = lib.gl_loglike.argtypes
     lib.gl_lightcurve_ex.restype = lib.gl_loglike_ex.restype = i
+    lib.gl_params_from_munu.argtypes = [vp, i, vp, vp, vp]
+    lib.gl_munu_from_uniform.argtypes = [vp, i, vp, vp]
+    lib.gl_params_from_munu.restype = lib.gl_munu_from_uniform.restype = i
     lib.gl_flux_geometry.argtypes = [vp, ll, vp, i, vp]
     lib.gl_flux_geometry_simpson.argtypes = [vp, ll, i, vp, i, vp]
     lib.gl_flux_geometry_simpson.restype = i
@@ -149,6 +152,32 @@ def _loglike(fname, width, params, times, t_exp, n_ss, obs, sigma, dtype, want_f
                                    int(n_ss), obs.data_ptr(), sigma.data_ptr(), chi2.data_ptr(),
                                    flux.data_ptr() if want_flux else None, code, _stream(params)))
     return (chi2, flux) if want_flux else chi2
+
+
+def gl_params_from_munu(sampling, want_logprior=True):
+    """Sampling rows [B, 12] (t0, P, a/R*, b, e, omega, r_mean, mu, nu, xi, q1, q2; App. A of the paper)
+    -> model rows [B, 12] (and ln p(mu, nu) [B])."""
+    torch = _torch()
+    lib = load_library()
+    sampling = _dev_f64(sampling, GL_NPARAMS)
+    B = sampling.shape[0]
+    params = torch.empty((B, GL_NPARAMS), dtype=torch.float64, device=sampling.device)
+    lp = torch.empty((B,), dtype=torch.float64, device=sampling.device) if want_logprior else None
+    with torch.cuda.device(sampling.device):
+        _check(lib.gl_params_from_munu(sampling.data_ptr(), B, params.data_ptr(),
+                                       lp.data_ptr() if want_logprior else None, _stream(sampling)))
+    return (params, lp) if want_logprior else params
+
+
+def gl_munu_from_uniform(uw):
+    """[B, 2] uniform variates -> [B, 2] (mu, nu) distributed as eq. A6 of the paper."""
+    torch = _torch()
+    lib = load_library()
+    uw = _dev_f64(uw, 2)
+    out = torch.empty_like(uw)
+    with torch.cuda.device(uw.device):
+        _check(lib.gl_munu_from_uniform(uw.data_ptr(), uw.shape[0], out.data_ptr(), _stream(uw)))
+    return out
 
 
 def gl_flux_geometry(geom, dtype="f32"):

@@ -23,6 +23,7 @@
 #include "gl_core.cuh"
 #include "gl_fast32.cuh"
 #include "gl_simpson.cuh"
+#include "gl_frontend.cuh"
 #include "gl_tables.h"
 
 namespace cg = cooperative_groups;
@@ -1039,6 +1040,31 @@ int gl_flux_geometry_simpson(const double* geom, long long N, int n_intervals, v
         gls::simpson_kernel<double><<<(unsigned)blocks, 128, 0, st>>>(geom, N, n_intervals, (double*)flux_out);
     cudaError_t e = cudaGetLastError();
     if (e != cudaSuccess) return cuda_fail(e, "simpson_kernel launch");
+    ++tl_launches;
+    return GL_OK;
+}
+
+int gl_params_from_munu(const double* sampling, int B, double* params_out,
+                        double* logprior_out_or_null, void* stream) {
+    if (B < 0) return GL_EINVAL;
+    if (B == 0) return GL_OK;
+    if (!sampling || !params_out) return GL_EINVAL;
+    glm::params_from_munu_kernel<<<(unsigned)((B + 127) / 128), 128, 0, (cudaStream_t)stream>>>(
+        sampling, B, params_out, logprior_out_or_null);
+    cudaError_t e = cudaGetLastError();
+    if (e != cudaSuccess) return cuda_fail(e, "params_from_munu_kernel launch");
+    ++tl_launches;
+    return GL_OK;
+}
+
+int gl_munu_from_uniform(const double* uw, int B, double* munu_out, void* stream) {
+    if (B < 0) return GL_EINVAL;
+    if (B == 0) return GL_OK;
+    if (!uw || !munu_out) return GL_EINVAL;
+    glm::munu_from_uniform_kernel<<<(unsigned)((B + 127) / 128), 128, 0, (cudaStream_t)stream>>>(
+        uw, B, munu_out);
+    cudaError_t e = cudaGetLastError();
+    if (e != cudaSuccess) return cuda_fail(e, "munu_from_uniform_kernel launch");
     ++tl_launches;
     return GL_OK;
 }

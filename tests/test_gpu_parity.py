@@ -355,3 +355,45 @@ def test_extended_rows_triaxial_and_locked(gl, dtype, locked):
     bad[2, 13] = -1.0
     o = host(gl.gl_lightcurve_ex(dev(bad), dev(t[:64]), 0.0, 1, dtype=dtype))
     assert np.all(np.isfinite(o[0])) and np.all(np.isnan(o[1])) and np.all(np.isnan(o[2]))
+
+
+def test_sampling_parameter_front_end(gl):
+    """NEXT-3: gl_params_from_munu / gl_munu_from_uniform against the oracle's App. A functions, and
+    the whole chain sampler -> front end -> light curve against the oracle's own chain."""
+    import torch
+    rng = np.random.default_rng(41)
+    B = 5000
+    uw = rng.random((B, 2))
+    munu = host(gl.gl_munu_from_uniform(dev(uw)))
+    ref = np.array([orc.munu_from_uniform(u, w) for u, w in uw])
+    # eq. A12 divides a cancelling numerator by (nu - 1)^2: its rounding error grows like eps/(1-nu)^2
+    # in ANY fp64 evaluation (differently contracted FMAs suffice), hence the scaled bound
+    assert np.all(np.abs(munu[:, 1] - ref[:, 1]) <= 1e-15)
+    assert np.all(np.abs(munu[:, 0] - ref[:, 0]) <= 1e-14 + 1e-14 / (1.0 - ref[:, 1]) ** 2)
+    s = np.zeros((B, 12))
+    s[:, 1], s[:, 2], s[:, 3] = 542.0, rng.uniform(200, 260, B), rng.uniform(0, 0.5, B)
+    s[:, 6] = rng.uniform(0.05, 0.07, B)
+    s[:, 7], s[:, 8] = munu[:, 0], munu[:, 1]
+    s[:, 9] = rng.uniform(0, np.pi / 2, B)
+    s[:, 10], s[:, 11] = rng.random(B), rng.random(B)
+    s[7, 7] = 1.3           # mu out of range
+    s[8, 8] = 0.0           # nu = 0: the density is not finite there
+    s[9, 10] = -0.1         # q1 out of range
+    p, lp = gl.gl_params_from_munu(dev(s))
+    p_ref, lp_ref = orc.params_from_munu(s)
+    good = np.isfinite(lp_ref)
+    assert good.sum() == B - 3 and not good[7] and not good[8] and not good[9]
+    assert np.abs(host(p)[good] - p_ref[good]).max() <= 1e-12
+    assert np.abs(host(lp)[good] - lp_ref[good]).max() <= 1e-12
+    assert np.all(np.isnan(host(p)[~good])) and np.all(host(lp)[~good] == -np.inf)
+    # chain: the converted rows go straight into the transit kernel (bad rows: NaN flux, inf chi2)
+    w = wl.config2()
+    sel = slice(1900, 2000)
+    chi, flux = gl.gl_loglike(p[:64], dev(w.times[sel]), w.t_exp, w.n_ss, dev(w.obs[sel]),
+                              dev(w.sigma[sel]), dtype="f64", want_flux=True)
+    chi_ref, flux_ref = orc.loglike(p_ref[:64], w.times[sel], w.t_exp, w.n_ss, w.obs[sel], w.sigma[sel])
+    g64 = good[:64]
+    assert np.abs(host(flux)[g64] - flux_ref[g64]).max() <= 1e-11
+    assert np.all(np.isnan(host(flux)[~g64])) and np.all(np.isinf(host(chi)[~g64]))
+    assert gl.gl_params_from_munu(dev(np.zeros((0, 12))), want_logprior=False).shape == (0, 12)
+    assert isinstance(p, torch.Tensor)
