@@ -114,6 +114,21 @@ int gl_params_from_munu(const double* sampling, int B, double* params_out,
                         double* logprior_out_or_null, void* stream);
 int gl_munu_from_uniform(const double* uw, int B, double* munu_out, void* stream);
 
+/* gl_gp_loglike (NEXT-4 of SURVEY.md 8(f)): the paper's objective in place of
+ * chi^2 -- the Gaussian-process log-likelihood of the residuals r_i = obs_i - F_b(t_i) under
+ *   K_ij = s^2 (1 + sqrt(3) d/rho) exp(-sqrt(3) d/rho) + delta_ij (sigma_i^2 + jit^2),  d = |t_i - t_j|
+ * (Matern-3/2 + jitter):  loglike_out[b] = -1/2 r^T K^-1 r - 1/2 ln det K - (T/2) ln 2 pi, fp64.
+ *   gp [B, 3] fp64 (device): (s, rho, jit) per walker, s >= 0, rho > 0, jit >= 0 (else NaN).
+ *   times MUST be sorted ascending (else NaN).  flux_work [B, T] of dtype (device, required): the
+ *   model flux is written there by the transit kernel (as gl_lightcurve) and read back by the
+ *   likelihood kernel, which evaluates the likelihood exactly in O(T) per walker with a Kalman
+ *   filter on the state-space form of the Matern-3/2 process -- the quantity celerite computes
+ *   for the paper, not celerite's algorithm.  An invalid walker (NaN flux row) gives -inf.
+ *   Two launches on `stream`; no synchronisation. */
+int gl_gp_loglike(const double* params, int B, const double* times, int T, double t_exp, int n_ss,
+                  const double* obs, const double* sigma, const double* gp, double* loglike_out,
+                  void* flux_work, gl_dtype dtype, void* stream);
+
 /* gl_flux_geometry: steps "crossings + boundary integrals" alone, for N bare geometries.
  *   geom [N, GL_NGEOM] row-major fp64 (device): (d, Rp, f_proj, PA, u1, u2) -- planet centre at
  *   (d, 0), d >= 0; projected semi-major axis Rp (0 < Rp < 0.5) at position angle PA [rad],

@@ -219,6 +219,23 @@ def params_from_munu(sampling):
     return out, lp
 
 
+def matern32(dt, s, rho):
+    """Matern-3/2 covariance s^2 (1 + sqrt(3)|dt|/rho) exp(-sqrt(3)|dt|/rho)."""
+    x = np.sqrt(3.0) * np.abs(dt) / rho
+    return s * s * (1.0 + x) * np.exp(-x)
+
+
+def gp_loglike_dense(resid, times, sigma, s, rho, jit):
+    """NEXT-4, the plain definition: ln N(resid; 0, K) with
+    K = Matern-3/2(s, rho) + diag(sigma^2 + jit^2), by a dense Cholesky factorisation (O(T^3): small T)."""
+    r = np.asarray(resid, dtype=np.float64)
+    t = np.asarray(times, dtype=np.float64)
+    K = matern32(t[:, None] - t[None, :], s, rho) + np.diag(np.asarray(sigma, dtype=np.float64) ** 2 + jit * jit)
+    L = np.linalg.cholesky(K)
+    z = np.linalg.solve(L, r)            # r^T K^-1 r = |L^-1 r|^2
+    return -0.5 * (z @ z) - np.log(np.diag(L)).sum() - 0.5 * r.size * np.log(2.0 * np.pi)
+
+
 def loglike(params, times, t_exp, n_ss, obs, sigma, nthreads=0, return_threads=False):
     """(chi2[B], flux[B,T]) in fp64."""
     p, pp = _c(np.atleast_2d(params))

@@ -16,7 +16,7 @@ GL_NPARAMS, GL_NGEOM, GL_NPARAMS_EX = 12, 6, 16
 _LIBPATH = Path(__file__).resolve().parent / "csrc" / "libgreenlantern_b200.so"
 _lib = None
 
-EXPORTS = ("gl_lightcurve", "gl_loglike", "gl_lightcurve_ex", "gl_loglike_ex", "gl_params_from_munu", "gl_munu_from_uniform", "gl_flux_geometry", "gl_flux_geometry_simpson", "gl_lightcurve_host",
+EXPORTS = ("gl_lightcurve", "gl_loglike", "gl_lightcurve_ex", "gl_loglike_ex", "gl_params_from_munu", "gl_munu_from_uniform", "gl_gp_loglike", "gl_flux_geometry", "gl_flux_geometry_simpson", "gl_lightcurve_host",
            "gl_loglike_host", "gl_flux_geometry_host", "gl_probe_peaks", "gl_launch_count", "gl_strerror",
            "gl_last_cuda_error", "gl_version")
 
@@ -44,6 +44,8 @@ def load_library():
     lib.gl_params_from_munu.argtypes = [vp, i, vp, vp, vp]
     lib.gl_munu_from_uniform.argtypes = [vp, i, vp, vp]
     lib.gl_params_from_munu.restype = lib.gl_munu_from_uniform.restype = i
+    lib.gl_gp_loglike.argtypes = [vp, i, vp, i, d, i, vp, vp, vp, vp, vp, i, vp]
+    lib.gl_gp_loglike.restype = i
     lib.gl_flux_geometry.argtypes = [vp, ll, vp, i, vp]
     lib.gl_flux_geometry_simpson.argtypes = [vp, ll, i, vp, i, vp]
     lib.gl_flux_geometry_simpson.restype = i
@@ -178,6 +180,26 @@ def gl_munu_from_uniform(uw):
     with torch.cuda.device(uw.device):
         _check(lib.gl_munu_from_uniform(uw.data_ptr(), uw.shape[0], out.data_ptr(), _stream(uw)))
     return out
+
+
+def gl_gp_loglike(params, times, t_exp, n_ss, obs, sigma, gp, dtype="f32", want_flux=False):
+    """ln L[B] (fp64) of the residuals under a Matern-3/2 + jitter Gaussian process (NEXT-4);
+    gp[B, 3] = (amplitude, timescale, jitter); times sorted ascending."""
+    torch = _torch()
+    lib = load_library()
+    params, times = _dev_f64(params, GL_NPARAMS), _dev_f64(times)
+    obs, sigma, gp = _dev_f64(obs), _dev_f64(sigma), _dev_f64(gp, 3)
+    code, td = _tdtype(dtype)
+    B, T = params.shape[0], times.shape[0]
+    if obs.shape[0] != T or sigma.shape[0] != T or gp.shape[0] != B:
+        raise GreenlanternError("obs, sigma must have the length of times and gp one row per walker")
+    out = torch.empty((B,), dtype=torch.float64, device=params.device)
+    flux = torch.empty((B, T), dtype=td, device=params.device)
+    with torch.cuda.device(params.device):
+        _check(lib.gl_gp_loglike(params.data_ptr(), B, times.data_ptr(), T, float(t_exp), int(n_ss),
+                                 obs.data_ptr(), sigma.data_ptr(), gp.data_ptr(), out.data_ptr(),
+                                 flux.data_ptr(), code, _stream(params)))
+    return (out, flux) if want_flux else out
 
 
 def gl_flux_geometry(geom, dtype="f32"):

@@ -24,6 +24,7 @@
 #include "gl_fast32.cuh"
 #include "gl_simpson.cuh"
 #include "gl_frontend.cuh"
+#include "gl_gp.cuh"
 #include "gl_tables.h"
 
 namespace cg = cooperative_groups;
@@ -1065,6 +1066,28 @@ int gl_munu_from_uniform(const double* uw, int B, double* munu_out, void* stream
         uw, B, munu_out);
     cudaError_t e = cudaGetLastError();
     if (e != cudaSuccess) return cuda_fail(e, "munu_from_uniform_kernel launch");
+    ++tl_launches;
+    return GL_OK;
+}
+
+int gl_gp_loglike(const double* params, int B, const double* times, int T, double t_exp, int n_ss,
+                  const double* obs, const double* sigma, const double* gp, double* loglike_out,
+                  void* flux_work, gl_dtype dtype, void* stream) {
+    if (B < 0 || T < 0 || (dtype != GL_F32 && dtype != GL_F64)) return GL_EINVAL;
+    if (B == 0) return GL_OK;
+    if (!gp || !loglike_out || (T > 0 && (!obs || !sigma || !flux_work))) return GL_EINVAL;
+    int rc = gl_lightcurve(params, B, times, T, t_exp, n_ss, flux_work, dtype, stream);
+    if (rc != GL_OK) return rc;
+    cudaStream_t st = (cudaStream_t)stream;
+    const unsigned blocks = (unsigned)((B + 31) / 32);
+    if (dtype == GL_F32)
+        glg::gp_kernel<float><<<blocks, 32, 0, st>>>((const float*)flux_work, B, times, T, obs, sigma, gp,
+                                                     loglike_out);
+    else
+        glg::gp_kernel<double><<<blocks, 32, 0, st>>>((const double*)flux_work, B, times, T, obs, sigma,
+                                                      gp, loglike_out);
+    cudaError_t e = cudaGetLastError();
+    if (e != cudaSuccess) return cuda_fail(e, "gp_kernel launch");
     ++tl_launches;
     return GL_OK;
 }

@@ -397,3 +397,48 @@ def test_sampling_parameter_front_end(gl):
     assert np.all(np.isnan(host(flux)[~g64])) and np.all(np.isinf(host(chi)[~g64]))
     assert gl.gl_params_from_munu(dev(np.zeros((0, 12))), want_logprior=False).shape == (0, 12)
     assert isinstance(p, torch.Tensor)
+
+
+@pytest.mark.parametrize("dtype", ["f32", "f64"])
+def test_gp_likelihood(gl, dtype):
+    """NEXT-4: gl_gp_loglike (transit kernel + O(T) Kalman filter) against the dense definition
+    ln N(obs - F; 0, Matern-3/2 + diag(sigma^2 + jit^2)) on an unevenly sampled, sorted series with
+    unequal error bars; F from the oracle."""
+    rng = np.random.default_rng(51)
+    w = wl.config3(B=12)
+    T = 400
+    t = np.sort(rng.uniform(-1.0, 1.0, T))
+    t[100:140] = t[100] + 0.002 * np.arange(40)          # a uniformly sampled stretch (exp() reuse)
+    t = np.sort(t)
+    sig = rng.uniform(0.5e-4, 2e-4, T)
+    obs = 1.0 - 0.004 * (np.abs(t) < 0.35) + 1e-4 * rng.standard_normal(T)
+    gp = np.column_stack([rng.uniform(0.3e-4, 5e-4, 12), rng.uniform(0.01, 1.0, 12),
+                          rng.uniform(0.0, 2e-4, 12)])
+    gp[3, 0] = 0.0                                       # no correlated term: white noise only
+    p = w.params.copy()
+    p[5, 6] = 0.7                                        # invalid walker
+    ll, flux = gl.gl_gp_loglike(dev(p), dev(t), 0.0, 1, dev(obs), dev(sig), dev(gp), dtype=dtype,
+                                want_flux=True)
+    ll, flux = host(ll), host(flux)
+    F = orc.lightcurve(p, t, 0.0, 1)
+    assert np.isneginf(ll[5]) and np.all(np.isnan(flux[5]))
+    good = [k for k in range(12) if k != 5]
+    assert np.abs(flux[good] - F[good]).max() <= FTOL[dtype]
+    ref = np.array([orc.gp_loglike_dense(obs - F[k], t, sig, *gp[k]) for k in good])
+    # fp64: filter vs Cholesky, both exact up to rounding.  fp32: the stored flux is rounded to fp32
+    # (half an ulp of 1 = 3e-8, up to 5e-7 allowed), i.e. ~1e-3 sigma per point; over T = 400 points
+    # that moves ln L ~ 3600 by a few 1e-2: 1e-4 relative, the same budget as chi^2.
+    rel = np.abs(ll[good] / ref - 1.0).max()
+    assert rel <= (1e-9 if dtype == "f64" else 1e-4), rel
+    # the filter itself, isolated from the flux precision: dense likelihood of the kernel's OWN flux
+    own = np.array([orc.gp_loglike_dense(obs - flux[k], t, sig, *gp[k]) for k in good])
+    assert np.abs(ll[good] / own - 1.0).max() <= 1e-9
+    # unsorted times and bad hyper-parameters: NaN
+    tt = t.copy()
+    tt[[10, 11]] = tt[[11, 10]]
+    assert np.all(np.isnan(host(gl.gl_gp_loglike(dev(p[:2]), dev(tt), 0.0, 1, dev(obs), dev(sig),
+                                                 dev(gp[:2]), dtype=dtype))))
+    gbad = gp[:2].copy()
+    gbad[0, 1] = 0.0
+    out = host(gl.gl_gp_loglike(dev(p[:2]), dev(t), 0.0, 1, dev(obs), dev(sig), dev(gbad), dtype=dtype))
+    assert np.isnan(out[0]) and np.isfinite(out[1])

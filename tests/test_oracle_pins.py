@@ -731,3 +731,31 @@ def test_params_from_munu_front_end():
     assert np.all(np.isfinite(lp))
     bad, lpb = orc.params_from_munu([[0, 10, 20, 0.3, 0, 0, 0.1, 1.5, 0.5, 0.5, 0.3, 0.3]])
     assert np.all(np.isnan(bad)) and lpb[0] == -np.inf
+
+
+# ---------------------------------------------------------------------------------------------
+# NEXT-4: Gaussian-process likelihood (Matern-3/2 + jitter), dense definition.
+# ---------------------------------------------------------------------------------------------
+def test_gp_dense_definition():
+    from scipy import stats
+    rng = np.random.default_rng(33)
+    t = np.sort(rng.uniform(0, 3, 60))
+    sig = rng.uniform(0.5e-4, 2e-4, 60)
+    r = 1e-4 * rng.standard_normal(60)
+    s, rho, jit = 3e-4, 0.2, 1e-4
+    # kernel values: variance at zero lag, textbook value at one timescale, decay
+    assert abs(orc.matern32(0.0, s, rho) - s * s) < 1e-20
+    assert abs(orc.matern32(rho, s, rho) - s * s * (1 + np.sqrt(3)) * np.exp(-np.sqrt(3))) < 1e-20
+    assert orc.matern32(10 * rho, s, rho) < 1e-6 * s * s
+    # against a library routine on the same covariance
+    K = orc.matern32(t[:, None] - t[None, :], s, rho) + np.diag(sig ** 2 + jit ** 2)
+    want = stats.multivariate_normal(mean=np.zeros(60), cov=K, allow_singular=False).logpdf(r)
+    assert abs(orc.gp_loglike_dense(r, t, sig, s, rho, jit) - want) < 1e-8 * abs(want)
+    # white-noise limit: s -> 0 gives -chi^2/2 - sum ln sqrt(sigma^2 + jit^2) - T/2 ln 2 pi
+    v = sig ** 2 + jit ** 2
+    white = -0.5 * (r * r / v).sum() - 0.5 * np.log(v).sum() - 30 * np.log(2 * np.pi)
+    assert abs(orc.gp_loglike_dense(r, t, sig, 0.0, rho, jit) - white) < 1e-9 * abs(white)
+    # a draw from the process is more likely under its own hyper-parameters than under wrong ones
+    L = np.linalg.cholesky(K)
+    y = L @ rng.standard_normal(60)
+    assert orc.gp_loglike_dense(y, t, sig, s, rho, jit) > orc.gp_loglike_dense(y, t, sig, 30 * s, rho, jit)
