@@ -25,6 +25,7 @@
 #include "gl_simpson.cuh"
 #include "gl_frontend.cuh"
 #include "gl_gp.cuh"
+#include "gl_gp_scan.cuh"
 #include "gl_tables.h"
 
 namespace cg = cooperative_groups;
@@ -1079,13 +1080,24 @@ int gl_gp_loglike(const double* params, int B, const double* times, int T, doubl
     int rc = gl_lightcurve(params, B, times, T, t_exp, n_ss, flux_work, dtype, stream);
     if (rc != GL_OK) return rc;
     cudaStream_t st = (cudaStream_t)stream;
-    const unsigned blocks = (unsigned)((B + 31) / 32);
-    if (dtype == GL_F32)
-        glg::gp_kernel<float><<<blocks, 32, 0, st>>>((const float*)flux_work, B, times, T, obs, sigma, gp,
-                                                     loglike_out);
-    else
-        glg::gp_kernel<double><<<blocks, 32, 0, st>>>((const double*)flux_work, B, times, T, obs, sigma,
-                                                      gp, loglike_out);
+    // one CTA per walker, parallel in time (gl_gp_scan.cuh); GL_GP_SERIAL=1 selects the one-thread-
+    // per-walker filter of gl_gp.cuh (kept as the plain version the scan is checked against)
+    static const bool serial = getenv("GL_GP_SERIAL") && atoi(getenv("GL_GP_SERIAL")) != 0;
+    if (serial) {
+        const unsigned blocks = (unsigned)((B + 31) / 32);
+        if (dtype == GL_F32)
+            glg::gp_kernel<float><<<blocks, 32, 0, st>>>((const float*)flux_work, B, times, T, obs, sigma,
+                                                         gp, loglike_out);
+        else
+            glg::gp_kernel<double><<<blocks, 32, 0, st>>>((const double*)flux_work, B, times, T, obs,
+                                                          sigma, gp, loglike_out);
+    } else if (dtype == GL_F32) {
+        glg::gp_scan_kernel<float><<<(unsigned)B, glg::GP_NT, 0, st>>>((const float*)flux_work, B, times, T, obs,
+                                                               sigma, gp, loglike_out);
+    } else {
+        glg::gp_scan_kernel<double><<<(unsigned)B, glg::GP_NT, 0, st>>>((const double*)flux_work, B, times, T, obs,
+                                                                sigma, gp, loglike_out);
+    }
     cudaError_t e = cudaGetLastError();
     if (e != cudaSuccess) return cuda_fail(e, "gp_kernel launch");
     ++tl_launches;

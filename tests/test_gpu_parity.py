@@ -442,3 +442,32 @@ def test_gp_likelihood(gl, dtype):
     gbad[0, 1] = 0.0
     out = host(gl.gl_gp_loglike(dev(p[:2]), dev(t), 0.0, 1, dev(obs), dev(sig), dev(gbad), dtype=dtype))
     assert np.isnan(out[0]) and np.isfinite(out[1])
+
+
+def test_gp_serial_and_scan_filters_agree(gl, tmp_path):
+    """The one-thread-per-walker filter (GL_GP_SERIAL=1, read once per process: run in a child) and
+    the parallel-in-time scan give the same likelihood (both were checked against the dense
+    definition above; this keeps the plain version alive)."""
+    import subprocess
+    import sys
+    rng = np.random.default_rng(61)
+    w = wl.config3(B=6)
+    T = 700                                    # not a multiple of the 256 chunks, ragged last chunk
+    t = np.sort(rng.uniform(-1.0, 1.0, T))
+    sig = rng.uniform(0.5e-4, 2e-4, T)
+    obs = 1.0 + 1e-4 * rng.standard_normal(T)
+    gp = np.column_stack([rng.uniform(0.3e-4, 5e-4, 6), rng.uniform(0.01, 1.0, 6), np.full(6, 1e-4)])
+    np.savez(tmp_path / "in.npz", p=w.params, t=t, obs=obs, sig=sig, gp=gp)
+    code = ("import numpy as np, torch, sys; sys.path.insert(0, %r); import paper_2410_05408_b200 as g; "
+            "z = np.load(%r); d = lambda x: torch.as_tensor(x, device='cuda'); "
+            "np.save(%r, g.gl_gp_loglike(d(z['p']), d(z['t']), 0.0, 1, d(z['obs']), d(z['sig']), d(z['gp']), "
+            "dtype='f64').cpu().numpy())") % (str(wl.__file__.rsplit('/', 2)[0]), str(tmp_path / "in.npz"),
+                                              str(tmp_path / "serial.npy"))
+    import os
+    subprocess.run([sys.executable, "-c", code], check=True, env=dict(os.environ, GL_GP_SERIAL="1"))
+    serial = np.load(tmp_path / "serial.npy")
+    scan = host(gl.gl_gp_loglike(dev(w.params), dev(t), 0.0, 1, dev(obs), dev(sig), dev(gp), dtype="f64"))
+    assert np.abs(scan / serial - 1.0).max() <= 1e-10
+    F = orc.lightcurve(w.params, t, 0.0, 1)
+    ref = np.array([orc.gp_loglike_dense(obs - F[k], t, sig, *gp[k]) for k in range(6)])
+    assert np.abs(scan / ref - 1.0).max() <= 1e-9
