@@ -22,7 +22,9 @@ namespace glc {
 template <typename T> struct num;
 template <> struct num<float> {
     static constexpr float pi = 3.14159265358979323846f;
-    static constexpr float tol = 2.5e-7f;   // angle tolerance of the bracketed solves
+    // angle tolerance of the bracketed solves: an angle error eps moves the areas by O(eps^2) only
+    // (gl_fast32.cuh header), so fp32 does not chase the last ulp
+    static constexpr float tol = 2e-5f;
     static constexpr float nudge = 2.5e-7f; // quadrant brackets are pulled strictly inside by this
     static constexpr int maxit = 40;
 };
@@ -50,6 +52,25 @@ GL_DEV double gmax(double a, double b) { return fmax(a, b); }
 GL_DEV float gmin(float a, float b) { return fminf(a, b); }
 GL_DEV double gmin(double a, double b) { return fmin(a, b); }
 GL_DEV void gsincos(float t, float* s, float* c) { sincosf(t, s, c); }
+// Sine and cosine of an OUTLINE angle in [0, 3 pi] (the geometry routines below; never the orbital
+// phase, whose sine is multiplied by a/R*).  FT = false: libm.  FT = true (fp32 on the device only):
+// MUFU, angle folded into [-pi, pi] -- absolute error 2^-21, inside the fp32 budget (gl_fast32.cuh
+// header).  A template flag and not a global choice because MUFU sine/cosine in this code, which is
+// inlined into the fused transit kernel but rarely executed there, made that kernel's register
+// allocation spill three times as much (cfg3 +2 us, cfg4 +6 us); the bare-geometry kernel, where the
+// evolute regime is common (config 5), instantiates FT = true.
+template <bool FT> GL_DEV void gtrig(float t, float* s, float* c) {
+#ifdef __CUDACC__
+    if (FT) {
+        const float tr = t > 3.14159265358979323846f ? t - 6.28318530717958647692f : t;
+        *s = __sinf(tr);
+        *c = __cosf(tr);
+        return;
+    }
+#endif
+    sincosf(t, s, c);
+}
+template <bool FT> GL_DEV void gtrig(double t, double* s, double* c) { sincos(t, s, c); }
 GL_DEV void gsincos(double t, double* s, double* c) { sincos(t, s, c); }
 
 // The outline in the kernel frame and everything derived from it once per sub-sample.
@@ -59,17 +80,17 @@ template <typename T> struct Outline {
 
 // g(t) = x^2 + y^2 - 1 and h(t) = g'(t)/2 = x x' + y y'  (x' = -a sin t, y' = b cos t;
 // PAPER.md:102-104 eqs. 14-15 in the kernel frame).
-template <typename T> GL_DEV void eval_g(const Outline<T>& o, T t, T* g, T* h) {
+template <typename T, bool FT = false> GL_DEV void eval_g(const Outline<T>& o, T t, T* g, T* h) {
     T s, c;
-    gsincos(t, &s, &c);
+    gtrig<FT>(t, &s, &c);
     const T x = o.xc + o.a * c, y = o.yc + o.b * s;
     *g = x * x + (y * y - T(1));
     *h = o.b * c * y - o.a * s * x;
 }
 // h(t) and h'(t) for the critical points of g.
-template <typename T> GL_DEV void eval_h(const Outline<T>& o, T t, T* h, T* hp) {
+template <typename T, bool FT = false> GL_DEV void eval_h(const Outline<T>& o, T t, T* h, T* hp) {
     T s, c;
-    gsincos(t, &s, &c);
+    gtrig<FT>(t, &s, &c);
     const T x = o.xc + o.a * c, y = o.yc + o.b * s;
     *h = o.b * c * y - o.a * s * x;
     const T bc = o.b * c, as = o.a * s;
@@ -79,16 +100,16 @@ template <typename T> GL_DEV void eval_h(const Outline<T>& o, T t, T* h, T* hp) 
 // Root of a function that changes sign exactly once on [lo, hi]: Newton, with bisection whenever
 // the Newton step leaves the bracket.  rising = the function is <= 0 at lo and >= 0 at hi.
 // WHICH = 0: root of g, WHICH = 1: root of h.
-template <typename T, int WHICH>
+template <typename T, int WHICH, bool FT = false>
 GL_DEV T solve_in(const Outline<T>& o, T lo, T hi, T t, bool rising) {
     t = gmin(gmax(t, lo), hi);
     for (int it = 0; it < num<T>::maxit; ++it) {
         T f, df;
         if (WHICH == 0) {
-            eval_g(o, t, &f, &df);
+            eval_g<T, FT>(o, t, &f, &df);
             df = df + df;
         } else {
-            eval_h(o, t, &f, &df);
+            eval_h<T, FT>(o, t, &f, &df);
         }
         if ((f > T(0)) == rising) hi = t; else lo = t;
         T tn = t - f / df;
@@ -153,7 +174,7 @@ template <typename T> GL_DEV void arc_primitive(const ArcCoef<T>& k, T s, T c, T
 
 // Adds the integrals of f_flat, f_lin, f_quad along the outline from t1 to t2 (t2 >= t1) to A[0..2].
 // qphi[k] = (3 z_k - z_k^3)/2 and qom[k] = w_k * 1.5 (1 - z_k^2) for the NQ/2 positive nodes z_k.
-template <typename T, int NQ>
+template <typename T, int NQ, bool FT = false>
 GL_DEV void add_outline_arc(const Outline<T>& o, const ArcCoef<T>& k, T t1, T s1, T c1, T t2, T s2,
                             T c2, const T* qphi, const T* qom, T* A) {
     const T dt = t2 - t1;
@@ -164,12 +185,12 @@ GL_DEV void add_outline_arc(const Outline<T>& o, const ArcCoef<T>& k, T t1, T s1
     A[2] += T(0.25) * (k.k0 * dt + (q2 - q1));
     const T hw = T(0.5) * dt, tm = t1 + hw;
     T sm, cm;
-    gsincos(tm, &sm, &cm);
+    gtrig<FT>(tm, &sm, &cm);
     T acc = T(0);
 #pragma unroll
     for (int i = 0; i < NQ / 2; ++i) {
         T sd, cd;
-        gsincos(hw * qphi[i], &sd, &cd);
+        gtrig<FT>(hw * qphi[i], &sd, &cd);
         const T cp = cm * cd - sm * sd, sp = sm * cd + cm * sd;   // t = tm + delta
         const T cq = cm * cd + sm * sd, sq = sm * cd - cm * sd;   // t = tm - delta
         const T xp = o.xc + o.a * cp, yp = o.yc + o.b * sp;
@@ -205,7 +226,7 @@ template <typename T> GL_DEV void add_limb_arc(T xa, T ya, T xb, T yb, T* A) {
 //   t_a < t* and a local maximum t_b > t* of g).  Between consecutive critical points g is
 //   monotone, so each crossing is the single root of g in a known bracket: no quartic algebra.
 // ---------------------------------------------------------------------------------------------
-template <typename T, int NQ>
+template <typename T, int NQ, bool FT = false>
 GL_DEV bool overlap_areas(T xc_in, T yc_in, T a, T b, const T* qphi, const T* qom, T* A) {
     const T pi = num<T>::pi, half = T(0.5) * pi;
     // quadrant boundaries pulled strictly inside their quadrant, so that a rounded boundary can
@@ -225,9 +246,9 @@ GL_DEV bool overlap_areas(T xc_in, T yc_in, T a, T b, const T* qphi, const T* qo
     const T Aa = a * o.xc, Bb = b * o.yc;
     T g, hd;
     T tfar = T(0);
-    if (Aa > T(0) || Bb > T(0)) tfar = solve_in<T, 1>(o, T(0), q1hi, gatan2(Bb, Aa), false);
+    if (Aa > T(0) || Bb > T(0)) tfar = solve_in<T, 1, FT>(o, T(0), q1hi, gatan2(Bb, Aa), false);
     T gfar;
-    eval_g(o, tfar, &gfar, &hd);
+    eval_g<T, FT>(o, tfar, &gfar, &hd);
 
     bool evol = false;
     T ta = T(0), tb = T(0), ga = T(0), gb = T(0);
@@ -236,10 +257,10 @@ GL_DEV bool overlap_areas(T xc_in, T yc_in, T a, T b, const T* qphi, const T* qo
         if (cA * cA + cB * cB < cE * cE) {
             evol = true;
             const T tstar = gmin(gmax(pi - gatan2(cB, cA), q2lo), q2hi);
-            ta = solve_in<T, 1>(o, q2lo, tstar, T(0.5) * (q2lo + tstar), true);
-            tb = solve_in<T, 1>(o, tstar, q2hi, T(0.5) * (tstar + q2hi), false);
-            eval_g(o, ta, &ga, &hd);
-            eval_g(o, tb, &gb, &hd);
+            ta = solve_in<T, 1, FT>(o, q2lo, tstar, T(0.5) * (q2lo + tstar), true);
+            tb = solve_in<T, 1, FT>(o, tstar, q2hi, T(0.5) * (tstar + q2hi), false);
+            eval_g<T, FT>(o, ta, &ga, &hd);
+            eval_g<T, FT>(o, tb, &gb, &hd);
         }
     }
 
@@ -258,28 +279,28 @@ GL_DEV bool overlap_areas(T xc_in, T yc_in, T a, T b, const T* qphi, const T* qo
             ae[1] = tfar + T(2) * pi;
         }
     } else {
-        const T tnear = solve_in<T, 1>(o, q3lo, q3hi, pi + gatan2(Bb, Aa), true);
+        const T tnear = solve_in<T, 1, FT>(o, q3lo, q3hi, pi + gatan2(Bb, Aa), true);
         T gnear;
-        eval_g(o, tnear, &gnear, &hd);
+        eval_g<T, FT>(o, tnear, &gnear, &hd);
         if (gnear >= T(0)) return false;
         const T tend = tfar + T(2) * pi;
-        const T rexit = solve_in<T, 0>(o, tnear, tend, cosine_guess(tnear, tend, gnear, gfar), true);
+        const T rexit = solve_in<T, 0, FT>(o, tnear, tend, cosine_guess(tnear, tend, gnear, gfar), true);
         if (!evol) {
-            as[0] = solve_in<T, 0>(o, tfar, tnear, cosine_guess(tfar, tnear, gfar, gnear), false);
+            as[0] = solve_in<T, 0, FT>(o, tfar, tnear, cosine_guess(tfar, tnear, gfar, gnear), false);
             ae[0] = rexit;
         } else if (ga < T(0) && gb > T(0)) {
             narc = 2;
-            as[0] = solve_in<T, 0>(o, tfar, ta, cosine_guess(tfar, ta, gfar, ga), false);
-            ae[0] = solve_in<T, 0>(o, ta, tb, cosine_guess(ta, tb, ga, gb), true);
-            as[1] = solve_in<T, 0>(o, tb, tnear, cosine_guess(tb, tnear, gb, gnear), false);
+            as[0] = solve_in<T, 0, FT>(o, tfar, ta, cosine_guess(tfar, ta, gfar, ga), false);
+            ae[0] = solve_in<T, 0, FT>(o, ta, tb, cosine_guess(ta, tb, ga, gb), true);
+            as[1] = solve_in<T, 0, FT>(o, tb, tnear, cosine_guess(tb, tnear, gb, gnear), false);
             ae[1] = rexit;
         } else if (ga >= T(0)) {
-            as[0] = solve_in<T, 0>(o, tb, tnear, cosine_guess(tb, tnear, gb, gnear), false);
+            as[0] = solve_in<T, 0, FT>(o, tb, tnear, cosine_guess(tb, tnear, gb, gnear), false);
             ae[0] = rexit;
         } else {
             // local maximum at t_b stays inside the disc: split there (near-singular integrand)
             narc = 2;
-            as[0] = solve_in<T, 0>(o, tfar, ta, cosine_guess(tfar, ta, gfar, ga), false);
+            as[0] = solve_in<T, 0, FT>(o, tfar, ta, cosine_guess(tfar, ta, gfar, ga), false);
             ae[0] = tb;
             as[1] = tb;
             ae[1] = rexit;
@@ -290,9 +311,9 @@ GL_DEV bool overlap_areas(T xc_in, T yc_in, T a, T b, const T* qphi, const T* qo
     A[0] = A[1] = A[2] = T(0);
     T ss[2], cs[2], se[2], ce[2];
     for (int i = 0; i < narc; ++i) {
-        gsincos(as[i], &ss[i], &cs[i]);
-        gsincos(ae[i], &se[i], &ce[i]);
-        add_outline_arc<T, NQ>(o, k, as[i], ss[i], cs[i], ae[i], se[i], ce[i], qphi, qom, A);
+        gtrig<FT>(as[i], &ss[i], &cs[i]);
+        gtrig<FT>(ae[i], &se[i], &ce[i]);
+        add_outline_arc<T, NQ, FT>(o, k, as[i], ss[i], cs[i], ae[i], se[i], ce[i], qphi, qom, A);
     }
     if (limb) {
         for (int i = 0; i < narc; ++i) {

@@ -226,9 +226,23 @@ GLF_DEV void critical_point(float xc, float yc, float a, float b, float* c,
     }
 }
 
+// Is the star centre inside the outline's evolute, A^(2/3) + B^(2/3) < (a^2 - b^2)^(2/3) (a second
+// pair of critical points of g)?  Decided with a 30 % safety margin towards "yes": just outside the evolute the maximum of g is nearly
+// degenerate and the unbracketed Newton of critical_point converges slowly (the generic path
+// is always correct, only slower); A, B < e2 is the cheap necessary condition tested first.
+GLF_DEV bool evolute_inside(float A, float B, float e2) {
+    const float ie = mufu_rcp(e2);
+    const float ca = cbrtf(A * ie), cb = cbrtf(B * ie);
+    return fmaf(ca, ca, cb * cb) < 1.3f;
+}
+
 // Blocked fraction delta = k0 A_flat + k1 A_lin + k2 A_quad for an outline with centre (xc, yc) in
 // the kernel frame (any signs), semi-axes a >= b > 0, a < 1/2.  k0, k1, k2 = c0, c1, c2 of R8 divided
 // by pi (1 - u1/3 - u2/6).  Returns 0 when the overlap is empty.
+// EVOL_EXACT (the bare-geometry kernel, where very flat outlines near the limb are common: config 5):
+// decide the evolute regime with evolute_inside() instead of its cheap necessary condition alone, and
+// run the bracketed search with MUFU sine/cosine (glc::gtrig<true>).
+template <bool EVOL_EXACT = false>
 GLF_DEV float blocked_f32(const TrapNode* trap, float xc_in, float yc_in, float a, float b, float k0,
                           float k1, float k2) {
     const float xc = fabsf(xc_in), yc = fabsf(yc_in);   // mirror images have the same areas
@@ -247,10 +261,10 @@ GLF_DEV float blocked_f32(const TrapNode* trap, float xc_in, float yc_in, float 
         // axis or 0.3 (error <= 6e-9 in flux on the config-5 sample)
         nh = (r0 + a + a <= 1.f || r0 + a <= 0.7f) ? 4 : 8;
         if (fmaf(4.f, a, r0) <= 1.f || r0 + a <= 0.5f) nh = 3;   // deep inside: six immediate nodes
-    } else if (Aa < e2 && Bb < e2) {
-        // the star centre may lie inside the evolute (up to four crossings): bracketed search
+    } else if (Aa < e2 && Bb < e2 && (!EVOL_EXACT || evolute_inside(Aa, Bb, e2))) {
+        // the star centre lies inside the evolute (up to four crossings): bracketed search
         float A[3];
-        if (!glc::overlap_areas<float, 16>(xc, yc, a, b, c_gl_phi, c_gl_om, A)) return 0.f;
+        if (!glc::overlap_areas<float, 16, EVOL_EXACT>(xc, yc, a, b, c_gl_phi, c_gl_om, A)) return 0.f;
         return fmaf(k0, A[0], fmaf(k1, A[1], k2 * A[2]));
     } else {
         // farthest outline point from the star centre: the only maximum of g (first quadrant)
