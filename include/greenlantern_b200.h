@@ -77,7 +77,11 @@ int gl_lightcurve(const double* params, int B, const double* times, int T, doubl
  *   obs, sigma [T] fp64 (device), sigma > 0 (a non-positive or non-finite sigma makes every
  *   chi^2 +inf).  chi2_out [B] float/double per dtype, fully overwritten.
  *   flux_out_or_null: optional [B, T] output as in gl_lightcurve; NULL => the model flux never
- *   leaves registers.  The residual sum is accumulated in fp64 in both dtypes. */
+ *   leaves registers.  The residual sum is accumulated in fp64 in both dtypes (GL_F32: the
+ *   residuals themselves are formed in fp32 from the fp64 difference obs - 1, and the walker-
+ *   independent part sum_i ((obs_i - 1)/sigma_i)^2 is formed once per call by a one-CTA kernel
+ *   launched just before the transit kernel, which starts early by programmatic dependent launch:
+ *   two launches on `stream`; GL_F64: one launch, everything per walker in fp64). */
 int gl_loglike(const double* params, int B, const double* times, int T, double t_exp, int n_ss,
                const double* obs, const double* sigma, void* chi2_out, void* flux_out_or_null,
                gl_dtype dtype, void* stream);
