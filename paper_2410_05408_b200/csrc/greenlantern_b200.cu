@@ -1,15 +1,18 @@
 // greenlantern_b200.cu -- kernels and C ABI of the B200 oblate-transit library (sm_100a).
 //
-// One fused kernel does the whole hot path of DESIGN.md section 1 for a batch of walkers:
-//   a0 per-walker prelude (fp64)            -> shared memory
-//   a1 Kepler + sky position per sub-sample  (phase in fp64, then the compute type)
-//   a2 projected-outline geometry            (in the prelude: constant over a transit)
-//   a3 outline/limb crossings, a4 boundary integrals   (gl_core.cuh)
+// transit_kernel<T, EX> does the whole hot path of DESIGN.md section 1 for a batch of walkers:
+//   a0 per-walker prelude                    -> shared memory (fp32 path: outline and window in fp32)
+//   a1 Kepler + sky position per sub-sample  (phase formed and reduced in fp64, then the compute type)
+//   a2 projected-outline geometry            (in the prelude; per sub-sample for tidally locked rows)
+//   a3 outline/limb crossings, a4 boundary integrals   (fp64: gl_core.cuh, fp32: gl_fast32.cuh)
 //   a5 exposure mean, residual^2, deterministic block + cluster reduction of chi^2
-// Work layout: one thread-block CLUSTER per walker (1..8 CTAs, DSMEM reduction, no atomics, no
-// scratch in HBM); each CTA classifies tiles of exposure times against the walker's transit
-// window, compacts the in-window ones into shared memory and spreads their (time, sub-exposure)
-// pairs over its threads, so the lanes of a warp all do in-transit work.
+// Work layout: one thread-block CLUSTER per walker (1..8 CTAs of 128 threads, no
+// atomics, no scratch in HBM); each CTA classifies its tile of the series against the walker's
+// transit window and lists the in-window exposures in shared memory; after one cluster barrier the
+// cluster's warps share the whole list over DSMEM, ingress/egress first.
+// Also here: the bare-geometry kernels (config 5), the ceiling probes, the host-pointer wrappers and
+// the C ABI.  Other kernels live in gl_simpson.cuh (the paper's snap + Simpson scheme),
+// gl_frontend.cuh (App. A sampling parameters), gl_gp.cuh / gl_gp_scan.cuh (GP likelihood).
 #include <cooperative_groups.h>
 #include <cuda_runtime.h>
 #include <math.h>
