@@ -689,7 +689,8 @@ transit_kernel(const double* __restrict__ params, int B,
                 // ---- evaluate the round's list: the cluster's warps take groups of exposures in
                 // turn (interleaved, so that ingress and egress are spread over every warp), each
                 // warp on its own (no block barriers)
-                const int gwarp = crank * NW + warp, gstride = csize * NW;
+                const int gwarp = warp * csize + crank, gstride = csize * NW;   // CTAs first: the early (expensive)
+                                                                            // groups land on different SMs
                 if (n_ss <= 32) {
                     // a lane takes JS consecutive sub-exposures of one exposure, a warp G = 32 / JB
                     // whole exposures (JB = blocks of JS per exposure).  Sparse lists (K2-shaped:
