@@ -35,6 +35,9 @@ N_SM, LANES = 148, 128
 # Algorithmic fp32 flop per in-transit sub-exposure (operation count of the scheme with the whole
 # outline inside the disc); limb-crossing samples need ~1050, so this undercounts.
 ALG_FLOP_PER_SUBSAMPLE = 750.0
+# dram__bytes_read.sum + dram__bytes_write.sum of ONE launch of transit_kernel<float>, from the
+# `ncu --set full` captures summarised in profiles/r01_v5.md (not measured live: ncu is not run here)
+NCU_DRAM_BYTES = {"cfg3": 232_704 + 0, "cfg4": 606_464 + 15_872}
 
 
 def make_workload(name, rank):
@@ -299,7 +302,9 @@ def main():
     alg_flop = ALG_FLOP_PER_SUBSAMPLE * n_sub_in
     achieved = alg_flop / (k_ms * 1e-3) / 1e12
     roofline = {"bound": "alu", "achieved": achieved, "peak": peak_tflops, "unit": "TFLOP/s",
-                "frac": achieved / peak_tflops, "traffic": None,
+                "frac": achieved / peak_tflops, "traffic": NCU_DRAM_BYTES.get(args.workload),
+                "traffic_unit": "bytes per launch (ncu --set full, profiles/r01_v5.md); the path is "
+                                "ALU-bound, algorithmic HBM bytes are B*96 + T*24 in, B*T*4 + B*4 out",
                 "kernel": "transit_kernel<float> (+ one-CTA baseline_kernel, overlapped by "
                           "programmatic dependent launch)", "kernel_ms": k_ms,
                 "kernel_ms_warm_l2": warm_ms,
