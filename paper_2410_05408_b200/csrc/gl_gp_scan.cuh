@@ -15,6 +15,8 @@
 #include <cuda_runtime.h>
 #include <math.h>
 
+#include "gl_gp.cuh"
+
 namespace glg {
 
 struct Elem {
@@ -88,9 +90,8 @@ __device__ __forceinline__ Trans transition(double dt, double lam, double p0, do
     t.f01 = e * dt;
     t.f10 = -e * lam * lam * dt;
     t.f11 = e * (1.0 - ld);
-    t.q00 = p0 - (t.f00 * t.f00 * p0 + t.f01 * t.f01 * p1);
-    t.q01 = -(t.f00 * t.f10 * p0 + t.f01 * t.f11 * p1);
-    t.q11 = p1 - (t.f10 * t.f10 * p0 + t.f11 * t.f11 * p1);
+    (void)p1;
+    matern32_q(ld, e * e, p0, lam, &t.q00, &t.q01, &t.q11);   // Q = Pinf - A Pinf A^T, no cancellation
     return t;
 }
 

@@ -471,3 +471,13 @@ def test_gp_serial_and_scan_filters_agree(gl, tmp_path):
     F = orc.lightcurve(w.params, t, 0.0, 1)
     ref = np.array([orc.gp_loglike_dense(obs - F[k], t, sig, *gp[k]) for k in range(6)])
     assert np.abs(scan / ref - 1.0).max() <= 1e-9
+    # a long, uniformly sampled series (config 4's 20 000 exposures: 79 steps per thread and a
+    # 13-level scan) through both filters
+    w4 = wl.config4(B=4)
+    gp4 = np.column_stack([[1e-5, 3e-5, 1e-4, 3e-4], [0.002, 0.02, 0.2, 2.0], np.full(4, 1e-5)])
+    np.savez(tmp_path / "in.npz", p=w4.params, t=w4.times, obs=w4.obs, sig=w4.sigma, gp=gp4)
+    subprocess.run([sys.executable, "-c", code], check=True, env=dict(os.environ, GL_GP_SERIAL="1"))
+    serial4 = np.load(tmp_path / "serial.npy")
+    scan4 = host(gl.gl_gp_loglike(dev(w4.params), dev(w4.times), 0.0, 1, dev(w4.obs), dev(w4.sigma),
+                                  dev(gp4), dtype="f64"))
+    assert np.all(np.isfinite(scan4)) and np.abs(scan4 / serial4 - 1.0).max() <= 1e-10
