@@ -433,6 +433,18 @@ def test_gp_likelihood(gl, dtype):
     # the filter itself, isolated from the flux precision: dense likelihood of the kernel's OWN flux
     own = np.array([orc.gp_loglike_dense(obs - flux[k], t, sig, *gp[k]) for k in good])
     assert np.abs(ll[good] / own - 1.0).max() <= 1e-9
+    # very small steps against the timescale (lambda dt ~ 1e-4 .. 1e-2): the regime in which the
+    # process noise Q = Pinf - A Pinf A^T loses its digits unless it is formed without cancellation
+    if dtype == "f64":
+        tu = -0.03 + 1e-4 * np.arange(600)
+        sgu = np.full(600, 1e-4)
+        obu = 1.0 + 1e-4 * rng.standard_normal(600) + 2e-4 * np.sin(40 * tu)
+        gpu_ = np.array([[3e-4, 1.0, 1e-5], [3e-4, 0.05, 0.0], [1e-4, 10.0, 2e-5]])
+        pu = w.params[:3]
+        Fu = orc.lightcurve(pu, tu, 0.0, 1)
+        llu = host(gl.gl_gp_loglike(dev(pu), dev(tu), 0.0, 1, dev(obu), dev(sgu), dev(gpu_), dtype="f64"))
+        refu = np.array([orc.gp_loglike_dense(obu - Fu[k], tu, sgu, *gpu_[k]) for k in range(3)])
+        assert np.abs(llu / refu - 1.0).max() <= 1e-9, np.abs(llu / refu - 1.0)
     # unsorted times and bad hyper-parameters: NaN
     tt = t.copy()
     tt[[10, 11]] = tt[[11, 10]]
