@@ -493,3 +493,21 @@ def test_gp_serial_and_scan_filters_agree(gl, tmp_path):
     scan4 = host(gl.gl_gp_loglike(dev(w4.params), dev(w4.times), 0.0, 1, dev(w4.obs), dev(w4.sigma),
                                   dev(gp4), dtype="f64"))
     assert np.all(np.isfinite(scan4)) and np.abs(scan4 / serial4 - 1.0).max() <= 1e-10
+
+
+@pytest.mark.parametrize("dtype", ["f32", "f64"])
+def test_supersampling_layouts(gl, dtype):
+    """Every lane layout of the evaluation loop: one pair per lane (sparse list), several
+    consecutive sub-exposures per lane with a ragged last block (dense list), one exposure per warp
+    (n_ss > 32)."""
+    w = wl.config3(B=3)
+    sparse_t = w.times[1700:2200]                      # 500 exposures, ~40 in the window
+    dense_t = np.linspace(-0.35, 0.35, 6000)           # almost all in the window
+    for n_ss in (1, 2, 5, 7, 16, 20, 31, 32, 33, 64):
+        for t in (sparse_t, dense_t):
+            if n_ss > 20 and t is dense_t:
+                t = dense_t[::6]
+            ref = orc.lightcurve(w.params, t, w.t_exp, n_ss)
+            out = host(gl.gl_lightcurve(dev(w.params), dev(t), w.t_exp, n_ss, dtype=dtype))
+            err = np.abs(out - ref).max()
+            assert err <= FTOL[dtype], (n_ss, t.size, err)
