@@ -95,11 +95,57 @@ __device__ __forceinline__ Trans transition(double dt, double lam, double p0, do
     return t;
 }
 
+// agg (x) (element of one filter step), using the structure of a step element instead of the general
+// combination: with f = F^T H^T = (F00, F01), the step has J = f f^T / Se, eta = f y / Se, A = (I - K H) F,
+// b = K y, C = (I - K H) Q, K = Q H^T / Se, Se = Q00 + R.  Then I + C_agg J = I + u f^T / Se with
+// u = C_agg f, whose inverse is I - u f^T / D, D = Se + f^T C_agg f (Sherman-Morrison), and
+//   A' = Ae (A - u (f^T A) / D),   b' = Ae (b + u (y - f^T b) / D) + K y,
+//   C' = Ae (C - u u^T / D) Ae^T + Ce,   eta' = eta + g (y - f^T b) / D,   J' = J + g g^T / D,   g = A^T f.
+// Two divisions and ~70 multiply-adds instead of ~140 and a 2x2 inverse.
+__device__ __forceinline__ Elem append_step(const Elem& a, const Trans& tr, double R, double y) {
+    const double f0 = tr.f00, f1 = tr.f01;
+    const double iSe = 1.0 / (tr.q00 + R), k0 = tr.q00 * iSe, k1 = tr.q01 * iSe;
+    // Ae = (I - K H) F
+    const double e00 = (1.0 - k0) * tr.f00, e01 = (1.0 - k0) * tr.f01;
+    const double e10 = tr.f10 - k1 * tr.f00, e11 = tr.f11 - k1 * tr.f01;
+    const double u0 = a.cxx * f0 + a.cxy * f1, u1 = a.cxy * f0 + a.cyy * f1;   // u = C f
+    const double iD = 1.0 / ((tr.q00 + R) + f0 * u0 + f1 * u1);
+    const double g0 = a.a00 * f0 + a.a10 * f1, g1 = a.a01 * f0 + a.a11 * f1;   // g = A^T f
+    const double nu = y - (f0 * a.b0 + f1 * a.b1);                             // y - f^T b
+    Elem o;
+    // A' = Ae (A - u g^T / D)
+    const double m00 = a.a00 - u0 * g0 * iD, m01 = a.a01 - u0 * g1 * iD;
+    const double m10 = a.a10 - u1 * g0 * iD, m11 = a.a11 - u1 * g1 * iD;
+    o.a00 = e00 * m00 + e01 * m10;
+    o.a01 = e00 * m01 + e01 * m11;
+    o.a10 = e10 * m00 + e11 * m10;
+    o.a11 = e10 * m01 + e11 * m11;
+    // b' = Ae (b + u nu / D) + K y
+    const double w0 = a.b0 + u0 * nu * iD, w1 = a.b1 + u1 * nu * iD;
+    o.b0 = e00 * w0 + e01 * w1 + k0 * y;
+    o.b1 = e10 * w0 + e11 * w1 + k1 * y;
+    // C' = Ae (C - u u^T / D) Ae^T + (I - K H) Q
+    const double n00 = a.cxx - u0 * u0 * iD, n01 = a.cxy - u0 * u1 * iD, n11 = a.cyy - u1 * u1 * iD;
+    const double r00 = e00 * n00 + e01 * n01, r01 = e00 * n01 + e01 * n11;
+    const double r10 = e10 * n00 + e11 * n01, r11 = e10 * n01 + e11 * n11;
+    o.cxx = r00 * e00 + r01 * e01 + (1.0 - k0) * tr.q00;
+    o.cxy = r00 * e10 + r01 * e11 + (1.0 - k0) * tr.q01;
+    o.cyy = r10 * e10 + r11 * e11 + (tr.q11 - k1 * tr.q01);
+    o.e0 = a.e0 + g0 * nu * iD;
+    o.e1 = a.e1 + g1 * nu * iD;
+    o.jxx = a.jxx + g0 * g0 * iD;
+    o.jxy = a.jxy + g0 * g1 * iD;
+    o.jyy = a.jyy + g1 * g1 * iD;
+    return o;
+}
+
+
 }  // namespace glg
 
 namespace glg {
 
 constexpr int GP_NT = 256;   // threads per walker
+constexpr int CH = 4;        // filter steps whose inputs are loaded together
 
 // One CTA per walker.  flux [B, T] (float or double), gp [B, 3] = (s, rho, jit), times ascending.
 template <typename T>
@@ -131,41 +177,42 @@ gp_scan_kernel(const T* __restrict__ flux, int B, const double* __restrict__ tim
     {
         Trans tr = {};
         double dtprev = -1.0;
-        for (int i = i_lo; i < i_hi; ++i) {
-            const double sg = sigma[i], R = sg * sg + jit2;
-            const double fi = (double)frow[i];
-            if (fi != fi) invalid_walker = true;
-            const double y = obs[i] - fi;
-            if (!(sg >= 0.0)) bad = true;
-            Elem e;
-            if (i == 0) {
-                // prior N(0, Pinf) updated with y_0: no dependence on an earlier state
-                const double S = p0 + R, k0 = p0 / S;
-                e = Elem{0.0, 0.0, 0.0, 0.0, k0 * y, 0.0, p0 - k0 * p0, 0.0, p1, 0.0, 0.0, 0.0, 0.0, 0.0};
-            } else {
-                const double dt = times[i] - times[i - 1];
+        // the inputs of CH steps are loaded in one batch (the loop is a dependent chain: a load
+        // inside it costs a full memory round trip per step)
+        for (int i0 = i_lo; i0 < i_hi; i0 += CH) {
+            double tv[CH + 1], sv[CH], yv[CH];
+            tv[0] = times[max(i0 - 1, 0)];
+#pragma unroll
+            for (int c = 0; c < CH; ++c) {
+                const int i = min(i0 + c, nT - 1);
+                tv[c + 1] = times[i];
+                sv[c] = sigma[i];
+                const double fi = (double)frow[i];
+                if (fi != fi && i0 + c < i_hi) invalid_walker = true;
+                yv[c] = obs[i] - fi;
+            }
+#pragma unroll
+            for (int c = 0; c < CH; ++c) {
+                const int i = i0 + c;
+                if (i >= i_hi) break;
+                const double sg = sv[c], R = sg * sg + jit2, y = yv[c];
+                if (!(sg >= 0.0)) bad = true;
+                if (i == 0) {
+                    // prior N(0, Pinf) updated with y_0: no dependence on an earlier state
+                    const double S = p0 + R, k0 = p0 / S;
+                    const Elem e = Elem{0.0, 0.0, 0.0, 0.0, k0 * y, 0.0, p0 - k0 * p0, 0.0, p1,
+                                        0.0, 0.0, 0.0, 0.0, 0.0};
+                    agg = combine(agg, e);
+                    continue;
+                }
+                const double dt = tv[c + 1] - tv[c];
                 if (dt < 0.0) bad = true;
                 if (!(fabs(dt - dtprev) <= 1e-9 * dtprev)) {
                     tr = transition(dt, lam, p0, p1);
                     dtprev = dt;
                 }
-                const double iS = 1.0 / (tr.q00 + R), k0 = tr.q00 * iS, k1 = tr.q01 * iS;
-                e.a00 = (1.0 - k0) * tr.f00;
-                e.a01 = (1.0 - k0) * tr.f01;
-                e.a10 = tr.f10 - k1 * tr.f00;
-                e.a11 = tr.f11 - k1 * tr.f01;
-                e.b0 = k0 * y;
-                e.b1 = k1 * y;
-                e.cxx = (1.0 - k0) * tr.q00;
-                e.cxy = (1.0 - k0) * tr.q01;
-                e.cyy = tr.q11 - k1 * tr.q01;
-                e.e0 = tr.f00 * y * iS;
-                e.e1 = tr.f01 * y * iS;
-                e.jxx = tr.f00 * tr.f00 * iS;
-                e.jxy = tr.f00 * tr.f01 * iS;
-                e.jyy = tr.f01 * tr.f01 * iS;
+                agg = append_step(agg, tr, R, y);
             }
-            agg = combine(agg, e);
         }
     }
     // ---- (2) inclusive scan: Hillis-Steele within the warp, the warps' totals through shared memory
@@ -196,40 +243,50 @@ gp_scan_kernel(const T* __restrict__ flux, int B, const double* __restrict__ tim
     {
         Trans tr = {};
         double dtprev = -1.0;
-        int nprod = 0;
-        for (int i = i_lo; i < i_hi; ++i) {
-            if (i > 0) {
-                const double dt = times[i] - times[i - 1];
-                if (!(fabs(dt - dtprev) <= 1e-9 * dtprev)) {
-                    tr = transition(dt, lam, p0, p1);
-                    dtprev = dt;
+        for (int i0 = i_lo; i0 < i_hi; i0 += CH) {
+            double tv[CH + 1], sv[CH], yv[CH];
+            tv[0] = times[max(i0 - 1, 0)];
+#pragma unroll
+            for (int c = 0; c < CH; ++c) {
+                const int i = min(i0 + c, nT - 1);
+                tv[c + 1] = times[i];
+                sv[c] = sigma[i];
+                yv[c] = obs[i] - (double)frow[i];
+            }
+#pragma unroll
+            for (int c = 0; c < CH; ++c) {
+                const int i = i0 + c;
+                if (i >= i_hi) break;
+                if (i > 0) {
+                    const double dt = tv[c + 1] - tv[c];
+                    if (!(fabs(dt - dtprev) <= 1e-9 * dtprev)) {
+                        tr = transition(dt, lam, p0, p1);
+                        dtprev = dt;
+                    }
+                    const double n0 = tr.f00 * m0 + tr.f01 * m1, n1 = tr.f10 * m0 + tr.f11 * m1;
+                    const double b00 = tr.f00 * P00 + tr.f01 * P01, b01 = tr.f00 * P01 + tr.f01 * P11;
+                    const double b10 = tr.f10 * P00 + tr.f11 * P01, b11 = tr.f10 * P01 + tr.f11 * P11;
+                    m0 = n0;
+                    m1 = n1;
+                    P00 = b00 * tr.f00 + b01 * tr.f01 + tr.q00;
+                    P01 = b00 * tr.f10 + b01 * tr.f11 + tr.q01;
+                    P11 = b10 * tr.f10 + b11 * tr.f11 + tr.q11;
                 }
-                const double n0 = tr.f00 * m0 + tr.f01 * m1, n1 = tr.f10 * m0 + tr.f11 * m1;
-                const double b00 = tr.f00 * P00 + tr.f01 * P01, b01 = tr.f00 * P01 + tr.f01 * P11;
-                const double b10 = tr.f10 * P00 + tr.f11 * P01, b11 = tr.f10 * P01 + tr.f11 * P11;
-                m0 = n0;
-                m1 = n1;
-                P00 = b00 * tr.f00 + b01 * tr.f01 + tr.q00;
-                P01 = b00 * tr.f10 + b01 * tr.f11 + tr.q01;
-                P11 = b10 * tr.f10 + b11 * tr.f11 + tr.q11;
+                const double sg = sv[c];
+                const double S = P00 + sg * sg + jit2;
+                if (!(S > 0.0)) bad = true;
+                const double v = yv[c] - m0, iS = 1.0 / S;
+                quad += v * v * iS;
+                prod *= S;
+                const double k0 = P00 * iS, k1 = P01 * iS;
+                m0 += k0 * v;
+                m1 += k1 * v;
+                P11 -= k1 * P01;
+                P01 -= k1 * P00;
+                P00 -= k0 * P00;
             }
-            const double sg = sigma[i];
-            const double S = P00 + sg * sg + jit2;
-            if (!(S > 0.0)) bad = true;
-            const double v = (obs[i] - (double)frow[i]) - m0, iS = 1.0 / S;
-            quad += v * v * iS;
-            prod *= S;
-            if (++nprod == 8) {
-                logdet += log(prod);
-                prod = 1.0;
-                nprod = 0;
-            }
-            const double k0 = P00 * iS, k1 = P01 * iS;
-            m0 += k0 * v;
-            m1 += k1 * v;
-            P11 -= k1 * P01;
-            P01 -= k1 * P00;
-            P00 -= k0 * P00;
+            logdet += log(prod);   // ln det K = sum ln S_i, CH factors per logarithm
+            prod = 1.0;
         }
         logdet += log(prod);
     }
