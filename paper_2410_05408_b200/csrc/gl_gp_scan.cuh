@@ -167,6 +167,9 @@ gp_scan_kernel(const T* __restrict__ flux, int B, const double* __restrict__ tim
     const T* frow = flux + (size_t)b * nT;
     const double lam = 1.7320508075688772935 / rho;
     const double p0 = s * s, p1 = lam * lam * p0, jit2 = jit * jit;
+    // launched behind the transit kernel with programmatic dependent launch: everything above ran while
+    // that kernel was still finishing; its flux rows are read only from here on
+    asm volatile("griddepcontrol.wait;" ::: "memory");
     // contiguous chunks: thread k owns steps [k len, min((k+1) len, nT))
     const int len = (nT + GP_NT - 1) / GP_NT;
     const int i_lo = min(tid * len, nT), i_hi = min(i_lo + len, nT);

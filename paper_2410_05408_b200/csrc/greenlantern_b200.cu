@@ -1173,12 +1173,22 @@ int gl_gp_loglike(const double* params, int B, const double* times, int T, doubl
         else
             glg::gp_kernel<double><<<blocks, 32, 0, st>>>((const double*)flux_work, B, times, T, obs,
                                                           sigma, gp, loglike_out);
-    } else if (dtype == GL_F32) {
-        glg::gp_scan_kernel<float><<<(unsigned)B, glg::GP_NT, 0, st>>>((const float*)flux_work, B, times, T, obs,
-                                                               sigma, gp, loglike_out);
     } else {
-        glg::gp_scan_kernel<double><<<(unsigned)B, glg::GP_NT, 0, st>>>((const double*)flux_work, B, times, T, obs,
-                                                                sigma, gp, loglike_out);
+        cudaLaunchConfig_t cfg = {};
+        cfg.gridDim = dim3((unsigned)B, 1, 1);
+        cfg.blockDim = dim3(glg::GP_NT, 1, 1);
+        cfg.stream = st;
+        cudaLaunchAttribute attr[1];
+        attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+        attr[0].val.programmaticStreamSerializationAllowed = 1;
+        cfg.attrs = attr;
+        cfg.numAttrs = 1;
+        cudaError_t el = (dtype == GL_F32)
+            ? cudaLaunchKernelEx(&cfg, glg::gp_scan_kernel<float>, (const float*)flux_work, B, times, T,
+                                 obs, sigma, gp, loglike_out)
+            : cudaLaunchKernelEx(&cfg, glg::gp_scan_kernel<double>, (const double*)flux_work, B, times, T,
+                                 obs, sigma, gp, loglike_out);
+        if (el != cudaSuccess) return cuda_fail(el, "gp_scan_kernel launch");
     }
     cudaError_t e = cudaGetLastError();
     if (e != cudaSuccess) return cuda_fail(e, "gp_kernel launch");
