@@ -74,7 +74,8 @@ constexpr double kTwoPi = 6.28318530717958647692;
 // ------------------------------------------------------------------------------------------
 struct Walker {
     // orbit (fp64: phases and Kepler's equation are always double)
-    double t0, inv_P, aR, e, omega, cosi, Mc, sq1pe, sq1me, half_win_phase, hard_phase, vmax, reach;
+    double t0, inv_P, aR, e, omega, cosi, Mc, Ec, sinEc, cosEc, sinw, cosw, sq1me2, half_win_phase,
+        hard_phase, reach;
     // projected outline: semi-axes and the rotation into the kernel frame
     double a, b, cpsi, spsi;
     // limb darkening, already divided by the disc-integrated intensity
@@ -246,8 +247,11 @@ __device__ void walker_prelude_orbit(const double* __restrict__ p, int nparams, 
         //   sin^2(phi) < [(reach/aR)^2 - cos^2 i] / sin^2 i  and cos(phi) > 0;
         // stored as a half-width in orbital phase, widened by half an exposure.
         w->cosi = b / aR;
-        w->Mc = 0.0;
-        w->sq1pe = w->sq1me = 1.0;
+        w->Mc = w->Ec = w->sinEc = 0.0;
+        w->cosEc = 1.0;
+        w->sinw = 0.0;
+        w->cosw = 1.0;
+        w->sq1me2 = 1.0;
         const R ci2 = R(w->cosi) * R(w->cosi), q = R(reach) / R(aR);
         const R S2 = (q * q - ci2) / (R(1) - ci2);
         if (S2 > R(0))
@@ -255,7 +259,6 @@ __device__ void walker_prelude_orbit(const double* __restrict__ p, int nparams, 
                               : (double)(glc::gasin(glc::gsqrt(S2)) * R(0.15915494309189535)) *
                                     (lowp ? 1.0 + 1e-5 : 1.0);
         if (hw >= 0.0) hw += 0.5 * t_exp * w->inv_P + (lowp ? 1e-9 : 1e-13);
-        w->vmax = kTwoPi * w->inv_P * aR;
         // exposures wholly inside |phase| < hard_phase keep the outline at least 0.01 inside the
         // limb (the cheap tiers of gl_fast32.cuh); the others (ingress, egress, grazing) are
         // listed FIRST so that the expensive geometries start early (scheduling only)
@@ -270,13 +273,32 @@ __device__ void walker_prelude_orbit(const double* __restrict__ p, int nparams, 
         const double nuc = 0.5 * kPi - om;
         const double s1 = sqrt(1.0 + e), s2 = sqrt(1.0 - e);
         const double Ec = 2.0 * atan2(s2 * sin(0.5 * nuc), s1 * cos(0.5 * nuc));
-        w->Mc = Ec - e * sin(Ec);
-        w->sq1pe = s1;
-        w->sq1me = s2;
-        w->cosi = (b / aR) * (1.0 + e * sin(om)) / (1.0 - e * e);
-        // largest sky-plane speed (periastron), in stellar radii per time unit: bounds how far
-        // the centre moves within half an exposure (window test of eccentric orbits)
-        w->vmax = kTwoPi * w->inv_P * aR * s1 / s2;
+        sincos(Ec, &w->sinEc, &w->cosEc);
+        sincos(om, &w->sinw, &w->cosw);
+        w->Ec = Ec;
+        w->Mc = Ec - e * w->sinEc;
+        w->sq1me2 = s1 * s2;
+        w->cosi = (b / aR) * (1.0 + e * w->sinw) / (1.0 - e * e);
+        // Transit window in phase, conservative.  With phi' = nu - nu_c the angle from conjunction,
+        // the sky distance is >= r |sin phi'| >= aR (1-e) |sin phi'|, so in transit needs
+        // |phi'| < phi_max = asin(reach / (aR (1-e))); the time to sweep phi_max is at most
+        // phi_max / min(d nu/dt), d nu/dt = n (1 + e cos nu)^2 / (1-e^2)^{3/2}, minimum taken over
+        // [nu_c - phi_max, nu_c + phi_max].  (Far from conjunction the planet is behind the star or
+        // beyond reach: those exposures get flux = 1 without a Kepler solve.)
+        const double smax = reach / (aR * (1.0 - e));
+        if (smax >= 1.0) {
+            hw = 0.5;
+        } else {
+            const double pmax = asin(smax);
+            double cmin = fmin(cos(nuc - pmax), cos(nuc + pmax));
+            double off = fmod(nuc - kPi, kTwoPi);   // does the interval contain nu = pi (apastron)?
+            if (off > kPi) off -= kTwoPi;
+            if (off < -kPi) off += kTwoPi;
+            if (fabs(off) <= pmax) cmin = -1.0;
+            const double slow = (1.0 + e * cmin) * (1.0 + e * cmin);
+            hw = pmax / kTwoPi * (1.0 - e * e) * s1 * s2 / slow * (1.0 + 1e-6) + 0.5 * t_exp * w->inv_P + 1e-9;
+            if (hw > 0.5) hw = 0.5;
+        }
         w->hard_phase = 0.0;
     }
     w->half_win_phase = hw;
@@ -361,15 +383,31 @@ __device__ bool sky_position_f64(const Walker& w, double ph, double* x0, double*
         *cphi = c;
         return c > 0.0;
     }
-    const double M = w.Mc + kTwoPi * ph;
-    const double E = kepler_E(M, w.e);
-    double sh, ch, sE, cE;
-    sincos(0.5 * E, &sh, &ch);
-    sincos(E, &sE, &cE);
-    const double nu = 2.0 * atan2(w.sq1pe * sh, w.sq1me * ch);
-    const double r = w.aR * (1.0 - w.e * cE);
-    double sp, cp;
-    sincos(nu + w.omega - 0.5 * kPi, &sp, &cp);
+    // Kepler's equation about the conjunction: E - e sin E = Mc + dM with Mc = Ec - e sin Ec, written
+    // as (E - Ec) - e (sin E - sin Ec) = dM; Newton from the second-order expansion in dM (in-window
+    // phases are close to conjunction: two or three steps), the bracketed solver as a fallback.
+    const double dM = kTwoPi * ph;
+    const double d1 = 1.0 / (1.0 - w.e * w.cosEc);
+    double E = w.Ec + dM * d1 - 0.5 * w.e * w.sinEc * dM * dM * d1 * d1 * d1;
+    double sE, cE;
+    int it = 0;
+    for (; it < 8; ++it) {
+        sincos(E, &sE, &cE);
+        const double dE = ((E - w.Ec) - w.e * (sE - w.sinEc) - dM) / (1.0 - w.e * cE);
+        E -= dE;
+        if (fabs(dE) < 1e-15) break;   // (sE, cE) then belong to E within 1e-15
+    }
+    if (it == 8) {
+        E = kepler_E(w.Mc + dM, w.e);
+        sincos(E, &sE, &cE);
+    }
+    // true anomaly and phi = nu + omega - pi/2 without inverse trigonometry:
+    //   cos nu = (cos E - e)/(1 - e cos E), sin nu = sqrt(1-e^2) sin E/(1 - e cos E),
+    //   cos phi = sin(nu + omega), sin phi = -cos(nu + omega)
+    const double q = 1.0 - w.e * cE, iq = 1.0 / q;
+    const double cnu = (cE - w.e) * iq, snu = w.sq1me2 * sE * iq;
+    const double r = w.aR * q;
+    const double cp = snu * w.cosw + cnu * w.sinw, sp = snu * w.sinw - cnu * w.cosw;
     *x0 = r * cp * w.cosi;
     *y0 = r * sp;
     *sphi = sp;
@@ -588,9 +626,7 @@ transit_kernel(const double* __restrict__ params, int B,
             acc = (double)INFINITY;
         } else {
             const WalkerT<T> v = narrow<T>(sw);
-            const bool circ = v.circular;
             const double hwin = sw.half_win_phase, hard_ph = sw.hard_phase;
-            const double reach = sw.reach + 0.5 * t_exp * sw.vmax;
             for (int round = 0; round < nrounds; ++round) {
                 const int i0 = (round * csize + crank) * tile;
                 // ---- pass 1: classify this thread's exposures of the tile against the window;
@@ -604,14 +640,8 @@ transit_kernel(const double* __restrict__ params, int B,
                     bool inwin = false, isearly = false;
                     if (i < nT) {
                         const double ph = reduced_phase(sw, times[i]);
-                        if (circ) {
-                            inwin = fabs(ph) < hwin;
-                            isearly = inwin && !(fabs(ph) < hard_ph);
-                        } else {
-                            double X, Y, sphi, cphi;
-                            sky_position_f64(sw, ph, &X, &Y, &sphi, &cphi);
-                            inwin = X * X + Y * Y < reach * reach;
-                        }
+                        inwin = fabs(ph) < hwin;
+                        isearly = inwin && !(fabs(ph) < hard_ph);
                         if (want_chi2 && !shared_base) {
                             const T r2 = residual_sq<T>(obs[i] - 1.0, T(0), sigma[i]);
                             if (!inwin) acc += (double)r2;

@@ -229,6 +229,24 @@ def test_eccentric_batch_fp32_vs_fp64(gl):
         assert np.abs(host(out) - ref).max() <= FTOL[dtype], dtype
         assert np.abs(host(chi) / chi_ref - 1.0).max() <= CTOL[dtype], dtype
     assert (ref < 1.0).sum() > 500          # the transits are really in the stretch
+    # extreme orbits: a planet skimming the star (window = the whole orbit), e = 0.8 at several
+    # arguments of periastron (Newton about the conjunction far from its starting guess), a whole
+    # orbit sampled (secondary eclipse must give exactly 1)
+    q = np.repeat(wl.config2().params, 6, axis=0)
+    q[:, 1] = 2.0
+    q[:, 2] = [1.35, 3.0, 3.0, 6.0, 6.0, 12.0]
+    q[:, 3] = [0.1, 0.4, -0.4, 0.2, 0.0, 0.5]
+    q[:, 4] = [0.1, 0.5, 0.5, 0.8, 0.8, 0.8]
+    q[:, 5] = [0.3, 1.2, 4.0, 0.5, 3.3, 5.5]
+    q[:, 6] = 0.12
+    tt = np.linspace(-1.0, 1.0, 1601)
+    ref = orc.lightcurve(q, tt, 0.002, 3)
+    for dtype in ("f32", "f64"):
+        out = host(gl.gl_lightcurve(dev(q), dev(tt), 0.002, 3, dtype=dtype))
+        err = np.abs(out - ref)
+        assert err.max() <= FTOL[dtype], (dtype, err.max(), np.unravel_index(err.argmax(), err.shape))
+        assert np.all(out[ref == 1.0] == 1.0)
+    assert all((ref[k] < 1.0).sum() > 5 for k in range(6))
 
 
 def test_bad_sigma_and_determinism(gl):
