@@ -569,12 +569,15 @@ baseline_kernel(const double* __restrict__ obs, const double* __restrict__ sigma
 }
 
 // EX = extended parameter rows (NEXT-2); the 12-column instantiation carries none of that code.
-template <typename T, bool EX>
+// SEG = the series of a walker may be split into segments taken by separate clusters (flux-only calls).
+template <typename T, bool EX, bool SEG>
 __global__ void __launch_bounds__(NT, sizeof(T) == 4 ? 8 : 2)
 transit_kernel(const double* __restrict__ params, int B,
-               const double* __restrict__ times, int nT,
+               const double* __restrict__ times_all, int nT_all,
                int tile, double t_exp, int n_ss, const double* __restrict__ obs,
-               const double* __restrict__ sigma, T* __restrict__ flux, T* chi2, int shared_base) {
+               const double* __restrict__ sigma, T* __restrict__ flux, T* chi2, int shared_base,
+               int nseg_arg, int seglen_arg) {
+    const int nseg = SEG ? nseg_arg : 1, seglen = SEG ? seglen_arg : nT_all;
     cg::cluster_group cluster = cg::this_cluster();
     const int crank = (int)cluster.block_rank(), csize = (int)cluster.num_blocks();
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
@@ -595,14 +598,13 @@ transit_kernel(const double* __restrict__ params, int B,
     const double inv_ss = 1.0 / (double)n_ss;
     const int nsub = tile / NT;   // exposures per thread and tile (<= 32: one mask bit each)
     const int round_span = csize * tile;
-    const int nrounds = (nT + round_span - 1) / round_span;
     const bool want_chi2 = (chi2 != nullptr);
     int wpar = 0;
     bool lists_live = false;   // uniform over the cluster
 
     // warm the L2 with this CTA's first tile while the prelude runs (one line = 16 doubles)
-    for (int i = crank * tile + tid * 16; i < min(nT, (crank + 1) * tile); i += NT * 16) {
-        asm volatile("prefetch.global.L2 [%0];" ::"l"(times + i));
+    for (int i = crank * tile + tid * 16; i < min(nT_all, (crank + 1) * tile); i += NT * 16) {
+        asm volatile("prefetch.global.L2 [%0];" ::"l"(times_all + i));
         if (want_chi2) {
             asm volatile("prefetch.global.L2 [%0];" ::"l"(obs + i));
             asm volatile("prefetch.global.L2 [%0];" ::"l"(sigma + i));
@@ -610,7 +612,14 @@ transit_kernel(const double* __restrict__ params, int B,
     }
 
     GL_TL(0);
-    for (int wk = blockIdx.y; wk < B; wk += gridDim.y) {
+    // A cluster works on one (walker, segment of the series); nseg > 1 only for flux-only calls with
+    // few walkers and a long series (one light curve of 1e5 exposures would otherwise use 8 CTAs of
+    // the whole GPU); chi^2 calls keep nseg = 1 (the sum over a walker's series stays in one cluster).
+    for (long long vw = blockIdx.y; vw < (long long)B * nseg; vw += gridDim.y) {
+        const int wk = (int)(vw / nseg), t_lo = (int)(vw - (long long)wk * nseg) * seglen;
+        const double* __restrict__ times = times_all + t_lo;
+        const int nT = min(seglen, nT_all - t_lo);
+        const int nrounds = (nT + round_span - 1) / round_span;
         __syncthreads();
         if (tid == 0) walker_prelude_orbit<T>(params + (size_t)wk * nparams, nparams, t_exp, &sw);
         if (tid == 32) walker_prelude_shape<T>(params + (size_t)wk * nparams, nparams, &sw);
@@ -618,7 +627,7 @@ transit_kernel(const double* __restrict__ params, int B,
         GL_TL(1);
         const bool valid = sw.valid != 0;
         double acc = 0.0;   // this thread's chi^2 terms
-        T* frow = flux ? flux + (size_t)wk * nT : nullptr;
+        T* frow = flux ? flux + (size_t)wk * nT_all + t_lo : nullptr;
 
         if (!valid) {
             if (frow)
@@ -1022,6 +1031,21 @@ int launch_transit(const double* params, int nparams, int B, const double* times
                    cudaStream_t st) {
     int C, tile;
     pick_shape(B, nT, &C, &tile);
+    // flux-only calls with few walkers and a series longer than one round: split the series into
+    // segments that separate clusters take (no reduction is needed between them)
+    int nseg = 1, seglen = nT;
+    if (chi2 == nullptr && nT > 0) {
+        const long long span = (long long)C * tile;
+        const long long rounds = (nT + span - 1) / span;
+        const long long room = (148LL * 8) / ((long long)B * C);
+        if (rounds > 1 && room > 1) {
+            nseg = (int)(rounds < room ? rounds : room);
+            const long long per = (rounds + nseg - 1) / nseg;   // rounds per segment
+            seglen = (int)(per * span);
+            nseg = (int)((nT + (long long)seglen - 1) / seglen);
+        }
+    }
+    const long long rows = (long long)B * nseg;
     // fp32 chi^2: launch-wide baseline first, the transit kernel right behind it (see baseline_kernel)
     const int shared_base = (sizeof(T) == 4 && chi2 != nullptr && nT > 0) ? 1 : 0;
     if (shared_base) {
@@ -1031,7 +1055,7 @@ int launch_transit(const double* params, int nparams, int B, const double* times
         ++tl_launches;
     }
     cudaLaunchConfig_t cfg = {};
-    cfg.gridDim = dim3((unsigned)C, (unsigned)(B < 65535 ? B : 65535), 1);
+    cfg.gridDim = dim3((unsigned)C, (unsigned)(rows < 65535 ? rows : 65535), 1);
     cfg.blockDim = dim3(NT, 1, 1);
     cfg.dynamicSmemBytes = 0;
     cfg.stream = st;
@@ -1044,20 +1068,27 @@ int launch_transit(const double* params, int nparams, int B, const double* times
     attr[1].val.programmaticStreamSerializationAllowed = 1;
     cfg.attrs = attr;
     cfg.numAttrs = shared_base ? 2 : 1;
-    cudaError_t e = (nparams == GL_NPARAMS_EX)
-            ? cudaLaunchKernelEx(&cfg, transit_kernel<T, true>, params, B, times, nT, tile, t_exp, n_ss,
-                                 obs, sigma, (T*)flux, (T*)chi2, shared_base)
-            : cudaLaunchKernelEx(&cfg, transit_kernel<T, false>, params, B, times, nT, tile, t_exp, n_ss,
-                                 obs, sigma, (T*)flux, (T*)chi2, shared_base);
+    auto launch = [&]() {
+        if (nseg > 1)   // flux-only, 12-column rows or extended ones
+            return (nparams == GL_NPARAMS_EX)
+                       ? cudaLaunchKernelEx(&cfg, transit_kernel<T, true, true>, params, B, times, nT, tile,
+                                            t_exp, n_ss, obs, sigma, (T*)flux, (T*)chi2, shared_base, nseg,
+                                            seglen)
+                       : cudaLaunchKernelEx(&cfg, transit_kernel<T, false, true>, params, B, times, nT, tile,
+                                            t_exp, n_ss, obs, sigma, (T*)flux, (T*)chi2, shared_base, nseg,
+                                            seglen);
+        return (nparams == GL_NPARAMS_EX)
+                   ? cudaLaunchKernelEx(&cfg, transit_kernel<T, true, false>, params, B, times, nT, tile,
+                                        t_exp, n_ss, obs, sigma, (T*)flux, (T*)chi2, shared_base, 1, nT)
+                   : cudaLaunchKernelEx(&cfg, transit_kernel<T, false, false>, params, B, times, nT, tile,
+                                        t_exp, n_ss, obs, sigma, (T*)flux, (T*)chi2, shared_base, 1, nT);
+    };
+    cudaError_t e = launch();
     if (e != cudaSuccess && shared_base) {
         // no early start then: plain stream order is just as correct
         (void)cudaGetLastError();
         cfg.numAttrs = 1;
-        e = (nparams == GL_NPARAMS_EX)
-                ? cudaLaunchKernelEx(&cfg, transit_kernel<T, true>, params, B, times, nT, tile, t_exp,
-                                     n_ss, obs, sigma, (T*)flux, (T*)chi2, shared_base)
-                : cudaLaunchKernelEx(&cfg, transit_kernel<T, false>, params, B, times, nT, tile, t_exp,
-                                     n_ss, obs, sigma, (T*)flux, (T*)chi2, shared_base);
+        e = launch();
     }
     if (e != cudaSuccess) return cuda_fail(e, "transit_kernel launch");
     ++tl_launches;
