@@ -161,11 +161,55 @@ int gl_loglike_host(const double* params, int B, const double* times, int T, dou
                     gl_dtype dtype);
 int gl_flux_geometry_host(const double* geom, long long N, void* flux_out, gl_dtype dtype);
 
+/* gl_series: a RESIDENT series for repeated likelihood calls (fp32 only).  An MCMC run evaluates one
+ * likelihood per walker per sampler step against fixed data: only params[B,12]
+ * changes between calls.  gl_series_create uploads (times, obs, sigma) ONCE and does, once, everything
+ * that depends on the series alone: the order check of `times`, the baseline sum
+ * S = sum_i ((obs_i - 1)/sigma_i)^2 in fp64, the fp32 pairs (obs_i - 1, 1/sigma_i) of the residuals,
+ * device buffers and pinned, device-mapped staging for up to B_max walkers.
+ *   times, obs, sigma [T] fp64, HOST pointers (copied; the caller may free them afterwards).
+ *   T >= 1, n_ss >= 1, t_exp >= 0, B_max >= 1, else GL_EINVAL.  *out receives the handle.
+ * The handle OWNS device memory (T * 32 bytes + B_max * 100 bytes, + B_max * T * 4 bytes once a host
+ * call has asked for flux), pinned host memory and one non-blocking stream, all on the device that
+ * was current at creation; gl_series_destroy releases them (NULL is allowed).  A handle serves ONE
+ * call at a time (calls on one handle must not overlap); different handles are independent.
+ *
+ * gl_series_loglike: params [B, GL_NPARAMS] fp64 HOST (any memory), B <= B_max; chi2_out [B] float
+ *   HOST; flux_out_or_null [B, T] float HOST.  Synchronous: returns when the outputs are written.
+ *   The kernel reads the parameter rows from, and writes chi^2 to, pinned host memory directly (no
+ *   copy engine on the path); flux, when asked for, comes back by one device-to-host copy.  Same
+ *   values as gl_loglike(GL_F32) up to the rounding of S (kept in fp64 here, narrowed there).
+ * gl_series_loglike_dev: params, chi2_out, flux_out_or_null are DEVICE pointers; work is enqueued on
+ *   `stream` without synchronising (the series buffers are only read, so several streams may use
+ *   one handle through this call as long as the handle outlives the work).
+ * Launches per call: hot_kernel (walkers on the common path: circular orbit, n_ss <= 32, sorted
+ * series, at most two limb crossings) followed, by programmatic dependent launch, by the full
+ * transit kernel for the walkers the first one deferred.  The host call launches the second kernel
+ * only when the previous call needed it (or, failing that, after the first has reported so). */
+typedef struct gl_series gl_series;
+int gl_series_create(const double* times, const double* obs, const double* sigma, int T, double t_exp,
+                     int n_ss, int B_max, gl_series** out);
+int gl_series_loglike(gl_series* s, const double* params, int B, float* chi2_out,
+                      float* flux_out_or_null);
+int gl_series_loglike_dev(gl_series* s, const double* params, int B, float* chi2_out,
+                          float* flux_out_or_null, void* stream);
+/* any of the output pointers may be NULL; baseline = S above (fp64; +inf when a sigma is bad) */
+int gl_series_info(const gl_series* s, int* T, int* n_ss, int* B_max, int* sorted, double* baseline);
+int gl_series_destroy(gl_series* s);
+
 /* gl_probe_peaks: measures, on the current device, the arithmetic ceilings the roofline of
  * bench.py divides by: register-only dependent-chain kernels of FFMA (fp32), DFMA
  * (fp64) and MUFU.RSQ, 8 independent chains per thread, every SM full.  out3 (HOST) receives
  * { fp32 TFLOP/s, fp64 TFLOP/s, MUFU Tops/s }.  Synchronises the device; not part of the hot path. */
 int gl_probe_peaks(double* out3);
+
+/* gl_probe_empty_launch: enqueues an EMPTY kernel of `rows` clusters of `cluster` CTAs of `threads`
+ * threads on `stream` and, when fallback_rows > 0, a second empty grid (fallback_rows clusters of
+ * fallback_cluster CTAs of 128 threads) chained to it by programmatic dependent launch -- the launch
+ * shapes of a gl_loglike / gl_series_loglike_dev step without their work.  bench.py times it the way
+ * it times a step and reports it as roofline.launch_floor_ms.  Not part of the hot path. */
+int gl_probe_empty_launch(int cluster, int rows, int threads, int fallback_cluster, int fallback_rows,
+                          void* stream);
 
 /* Number of kernel launches the calling thread's entry points have enqueued so far (HOST). */
 long long gl_launch_count(void);

@@ -17,7 +17,9 @@ _LIBPATH = Path(__file__).resolve().parent / "csrc" / "libgreenlantern_b200.so"
 _lib = None
 
 EXPORTS = ("gl_lightcurve", "gl_loglike", "gl_lightcurve_ex", "gl_loglike_ex", "gl_params_from_munu", "gl_munu_from_uniform", "gl_gp_loglike", "gl_flux_geometry", "gl_flux_geometry_simpson", "gl_lightcurve_host",
-           "gl_loglike_host", "gl_flux_geometry_host", "gl_probe_peaks", "gl_launch_count", "gl_strerror",
+           "gl_loglike_host", "gl_flux_geometry_host", "gl_series_create", "gl_series_loglike",
+           "gl_series_loglike_dev", "gl_series_info", "gl_series_destroy", "gl_probe_peaks",
+           "gl_probe_empty_launch", "gl_launch_count", "gl_strerror",
            "gl_last_cuda_error", "gl_version")
 
 
@@ -55,6 +57,17 @@ def load_library():
     for name in ("gl_lightcurve", "gl_loglike", "gl_flux_geometry", "gl_lightcurve_host",
                  "gl_loglike_host", "gl_flux_geometry_host", "gl_version"):
         getattr(lib, name).restype = i
+    lib.gl_series_create.argtypes = [vp, vp, vp, i, d, i, i, ctypes.POINTER(vp)]
+    lib.gl_series_loglike.argtypes = [vp, vp, i, vp, vp]
+    lib.gl_series_loglike_dev.argtypes = [vp, vp, i, vp, vp, vp]
+    lib.gl_series_info.argtypes = [vp, ctypes.POINTER(i), ctypes.POINTER(i), ctypes.POINTER(i),
+                                   ctypes.POINTER(i), ctypes.POINTER(d)]
+    lib.gl_series_destroy.argtypes = [vp]
+    for name in ("gl_series_create", "gl_series_loglike", "gl_series_loglike_dev", "gl_series_info",
+                 "gl_series_destroy"):
+        getattr(lib, name).restype = i
+    lib.gl_probe_empty_launch.argtypes = [i, i, i, i, i, vp]
+    lib.gl_probe_empty_launch.restype = i
     lib.gl_probe_peaks.argtypes = [vp]
     lib.gl_probe_peaks.restype = i
     lib.gl_launch_count.restype = ll
@@ -280,11 +293,93 @@ def gl_flux_geometry_host(geom, dtype="f32"):
     return out
 
 
+class GlSeries:
+    """A resident series (gl_series_* of the C ABI): upload times/obs/sigma once, then evaluate
+    chi^2 for many parameter batches.  ``loglike`` takes HOST numpy arrays and is synchronous;
+    ``loglike_dev`` takes CUDA tensors and enqueues on torch's current stream."""
+
+    def __init__(self, times, obs, sigma, t_exp, n_ss, B_max, device=None):
+        lib = load_library()
+        times, obs, sigma = map(_host_f64, (times, obs, sigma))
+        if not (times.ndim == 1 and obs.shape == times.shape and sigma.shape == times.shape):
+            raise GreenlanternError("times, obs and sigma must be 1-d arrays of one length")
+        self._h = ctypes.c_void_p()
+        self.T, self.B_max = int(times.shape[0]), int(B_max)
+        self._device = device
+        if device is not None:
+            with _torch().cuda.device(device):
+                rc = lib.gl_series_create(times.ctypes.data, obs.ctypes.data, sigma.ctypes.data, self.T,
+                                          float(t_exp), int(n_ss), self.B_max, ctypes.byref(self._h))
+        else:
+            rc = lib.gl_series_create(times.ctypes.data, obs.ctypes.data, sigma.ctypes.data, self.T,
+                                      float(t_exp), int(n_ss), self.B_max, ctypes.byref(self._h))
+        _check(rc)
+
+    def info(self):
+        i, d = ctypes.c_int, ctypes.c_double
+        T, S, Bm, so, base = i(), i(), i(), i(), d()
+        _check(load_library().gl_series_info(self._h, ctypes.byref(T), ctypes.byref(S), ctypes.byref(Bm),
+                                             ctypes.byref(so), ctypes.byref(base)))
+        return {"T": T.value, "n_ss": S.value, "B_max": Bm.value, "sorted": bool(so.value),
+                "baseline": base.value}
+
+    def loglike(self, params, want_flux=False, chi2_out=None, flux_out=None):
+        params = _host_f64(np.atleast_2d(params))
+        if params.shape[1] != GL_NPARAMS:
+            raise GreenlanternError(f"expected shape [*, {GL_NPARAMS}]")
+        B = params.shape[0]
+        chi2 = _host_out(chi2_out, (B,), np.float32)
+        flux = _host_out(flux_out, (B, self.T), np.float32) if want_flux else None
+        _check(load_library().gl_series_loglike(self._h, params.ctypes.data, B, chi2.ctypes.data,
+                                                flux.ctypes.data if want_flux else None))
+        return (chi2, flux) if want_flux else chi2
+
+    def loglike_dev(self, params, want_flux=False, chi2_out=None, flux_out=None):
+        torch = _torch()
+        params = _dev_f64(params, GL_NPARAMS)
+        B = params.shape[0]
+        chi2 = chi2_out if chi2_out is not None else torch.empty((B,), dtype=torch.float32, device=params.device)
+        flux = None
+        if want_flux:
+            flux = flux_out if flux_out is not None else torch.empty((B, self.T), dtype=torch.float32,
+                                                                     device=params.device)
+        for t, shape in ((chi2, (B,)), (flux, (B, self.T))):
+            if t is not None and not (t.is_cuda and t.dtype == torch.float32 and t.is_contiguous()
+                                      and tuple(t.shape) == shape):
+                raise GreenlanternError(f"output must be a contiguous CUDA float32 tensor of shape {shape}")
+        with torch.cuda.device(params.device):
+            _check(load_library().gl_series_loglike_dev(self._h, params.data_ptr(), B, chi2.data_ptr(),
+                                                        flux.data_ptr() if want_flux else None,
+                                                        _stream(params)))
+        return (chi2, flux) if want_flux else chi2
+
+    def close(self):
+        if self._h:
+            _check(load_library().gl_series_destroy(self._h))
+            self._h = ctypes.c_void_p()
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+
 def gl_probe_peaks():
     """{fp32 TFLOP/s, fp64 TFLOP/s, MUFU Tops/s} of the current device (FMA / MUFU chain kernels)."""
     out = (ctypes.c_double * 3)()
     _check(load_library().gl_probe_peaks(out))
     return {"fp32_tflops": out[0], "fp64_tflops": out[1], "mufu_tops": out[2]}
+
+
+def gl_probe_empty_launch(cluster, rows, threads, fallback_cluster=1, fallback_rows=0, device=None):
+    """Enqueue an empty kernel of the given shape (and, optionally, a dependent empty grid) on torch's
+    current stream: the launch floor bench.py reports."""
+    torch = _torch()
+    dev = torch.device("cuda", torch.cuda.current_device()) if device is None else device
+    st = ctypes.c_void_p(torch.cuda.current_stream(dev).cuda_stream)
+    _check(load_library().gl_probe_empty_launch(int(cluster), int(rows), int(threads), int(fallback_cluster),
+                                                int(fallback_rows), st))
 
 
 def gl_launch_count():

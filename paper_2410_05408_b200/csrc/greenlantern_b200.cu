@@ -19,12 +19,16 @@
 #include <stdint.h>
 #include <stdio.h>
 #include <stdlib.h>
+#include <string.h>
+
+#include <new>
 
 #include <mutex>
 
 #include "../../include/greenlantern_b200.h"
 #include "gl_core.cuh"
 #include "gl_fast32.cuh"
+#include "gl_hot.cuh"
 #include "gl_simpson.cuh"
 #include "gl_frontend.cuh"
 #include "gl_gp.cuh"
@@ -32,29 +36,6 @@
 #include "gl_tables.h"
 
 namespace cg = cooperative_groups;
-
-// Development aid (off unless built with -DGL_TIMELINE): per-CTA phase timestamps of transit_kernel.
-#ifdef GL_TIMELINE
-__device__ long long g_timeline[8192 * 8];
-#define GL_TL(k)                                                                          \
-    do {                                                                                  \
-        const unsigned cta_ = blockIdx.y * gridDim.x + blockIdx.x;                        \
-        if (cta_ < 8192 && (threadIdx.x & 31) == 0) {                                     \
-            long long t_;                                                                 \
-            asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t_));                        \
-            atomicMax((unsigned long long*)&g_timeline[cta_ * 8 + (k)], (unsigned long long)t_); \
-        }                                                                                 \
-    } while (0)
-extern "C" int gl_debug_timeline(long long* host_out, int reset) {
-    if (reset) {
-        static long long zeros[8192 * 8];
-        return (int)cudaMemcpyToSymbol(g_timeline, zeros, sizeof(zeros));
-    }
-    return (int)cudaMemcpyFromSymbol(host_out, g_timeline, sizeof(long long) * 8192 * 8);
-}
-#else
-#define GL_TL(k) do { } while (0)
-#endif
 
 namespace {
 
@@ -575,8 +556,8 @@ __global__ void __launch_bounds__(NT, sizeof(T) == 4 ? 8 : 2)
 transit_kernel(const double* __restrict__ params, int B,
                const double* __restrict__ times_all, int nT_all,
                int tile, double t_exp, int n_ss, const double* __restrict__ obs,
-               const double* __restrict__ sigma, T* __restrict__ flux, T* chi2, int shared_base,
-               int nseg_arg, int seglen_arg) {
+               const double* __restrict__ sigma, T* flux, T* chi2, int shared_base,
+               int nseg_arg, int seglen_arg, int marker_mode) {
     const int nseg = SEG ? nseg_arg : 1, seglen = SEG ? seglen_arg : nT_all;
     cg::cluster_group cluster = cg::this_cluster();
     const int crank = (int)cluster.block_rank(), csize = (int)cluster.num_blocks();
@@ -603,20 +584,41 @@ transit_kernel(const double* __restrict__ params, int B,
     bool lists_live = false;   // uniform over the cluster
 
     // warm the L2 with this CTA's first tile while the prelude runs (one line = 16 doubles)
-    for (int i = crank * tile + tid * 16; i < min(nT_all, (crank + 1) * tile); i += NT * 16) {
+    for (int i = crank * tile + tid * 16; !marker_mode && i < min(nT_all, (crank + 1) * tile); i += NT * 16) {
         asm volatile("prefetch.global.L2 [%0];" ::"l"(times_all + i));
         if (want_chi2) {
             asm volatile("prefetch.global.L2 [%0];" ::"l"(obs + i));
             asm volatile("prefetch.global.L2 [%0];" ::"l"(sigma + i));
         }
     }
-
-    GL_TL(0);
     // A cluster works on one (walker, segment of the series); nseg > 1 only for flux-only calls with
     // few walkers and a long series (one light curve of 1e5 exposures would otherwise use 8 CTAs of
     // the whole GPU); chi^2 calls keep nseg = 1 (the sum over a walker's series stays in one cluster).
+    // marker_mode: this launch FINISHES what hot_kernel (gl_hot.cuh), launched just before it, deferred:
+    // only (walker, segment) units whose output slot carries the marker are done; the others are
+    // left as they are.  The grid may have started early (programmatic dependent launch).
+    if (marker_mode) {
+        asm volatile("griddepcontrol.wait;" ::: "memory");
+        // common case: nothing was deferred.  Thread t looks at the slot of the t-th unit this cluster
+        // would take, all at once (one load latency), and the CTA leaves if none carries the marker.
+        // Every CTA of a cluster looks at the same slots, so the verdict is cluster-uniform.
+        bool any = false;
+        for (long long vw = blockIdx.y + (long long)tid * gridDim.y; vw < (long long)B * nseg;
+             vw += (long long)NT * gridDim.y) {
+            const int wk = (int)(vw / nseg), t_lo = (int)(vw - (long long)wk * nseg) * seglen;
+            const T* slot = want_chi2 ? chi2 + wk : flux + (size_t)wk * nT_all + t_lo;
+            any = any || (sizeof(T) == 4 && *reinterpret_cast<const volatile uint32_t*>(slot) == glh::MARK_BITS);
+        }
+        if (!__syncthreads_or(any ? 1 : 0)) return;
+    }
     for (long long vw = blockIdx.y; vw < (long long)B * nseg; vw += gridDim.y) {
         const int wk = (int)(vw / nseg), t_lo = (int)(vw - (long long)wk * nseg) * seglen;
+        if (marker_mode) {
+            const T* slot = want_chi2 ? chi2 + wk : flux + (size_t)wk * nT_all + t_lo;
+            const uint32_t bits = sizeof(T) == 4 ? *reinterpret_cast<const volatile uint32_t*>(slot) : 0u;
+            if (bits != glh::MARK_BITS) continue;   // (only this cluster ever rewrites this slot)
+            if (csize > 1) cluster.sync();   // every CTA has read the slot before any CTA rewrites it
+        }
         const double* __restrict__ times = times_all + t_lo;
         const int nT = min(seglen, nT_all - t_lo);
         const int nrounds = (nT + round_span - 1) / round_span;
@@ -624,7 +626,6 @@ transit_kernel(const double* __restrict__ params, int B,
         if (tid == 0) walker_prelude_orbit<T>(params + (size_t)wk * nparams, nparams, t_exp, &sw);
         if (tid == 32) walker_prelude_shape<T>(params + (size_t)wk * nparams, nparams, &sw);
         __syncthreads();
-        GL_TL(1);
         const bool valid = sw.valid != 0;
         double acc = 0.0;   // this thread's chi^2 terms
         T* frow = flux ? flux + (size_t)wk * nT_all + t_lo : nullptr;
@@ -702,10 +703,8 @@ transit_kernel(const double* __restrict__ params, int B,
                 }
                 // ---- share the round's list over the cluster.  Cluster-wide order: the early
                 // entries of CTA 0, 1, ..., then the remaining entries of CTA 0, 1, ...
-                if (round == 0) GL_TL(2);
                 cluster.sync();
                 lists_live = true;
-                if (round == 0) GL_TL(3);
                 if (tid < 2) {
                     int run = 0;
                     for (int r = 0; r < csize; ++r) {
@@ -789,7 +788,6 @@ transit_kernel(const double* __restrict__ params, int B,
                 }
             }
         }
-        GL_TL(4);
         // ---- chi^2: CTA sum; every CTA PUSHES its partial into rank 0's shared memory over DSMEM,
         // one cluster barrier, then rank 0 adds them in rank order.  Nothing is read remotely after
         // that barrier, so the other CTAs may move on (or exit) at once.  The slots alternate with
@@ -797,11 +795,9 @@ transit_kernel(const double* __restrict__ params, int B,
         // can only pass once it has read the slot.
         if (want_chi2) {
             const double tot = block_sum(acc, s_red);
-            GL_TL(5);
             if (tid == 0) *cluster.map_shared_rank(&s_gather[wpar][crank], 0) = tot;
             cluster.sync();
             lists_live = false;   // every CTA is past its evaluation
-            GL_TL(6);
             if (crank == 0 && tid == 0) {
                 double c2 = 0.0;
                 for (int r = 0; r < csize; ++r) c2 += s_gather[wpar][r];
@@ -818,7 +814,6 @@ transit_kernel(const double* __restrict__ params, int B,
     }
     // no CTA may exit while a neighbour can still read its lists (flux-only calls: no barrier above)
     if (lists_live) cluster.sync();
-    GL_TL(7);
 }
 
 // ------------------------------------------------------------------------------------------
@@ -934,6 +929,10 @@ geometry_binned_kernel(const double* __restrict__ geom, long long N, float* __re
 // ------------------------------------------------------------------------------------------
 // Ceiling probes (gl_probe_peaks): 8 independent register-only chains per thread.
 // ------------------------------------------------------------------------------------------
+__global__ void empty_kernel(int dependent) {
+    if (dependent) asm volatile("griddepcontrol.wait;" ::: "memory");
+    else asm volatile("griddepcontrol.launch_dependents;");
+}
 template <typename T> __global__ void probe_fma(T* out, int iters, T a, T b) {
     T x[8];
 #pragma unroll
@@ -1007,55 +1006,46 @@ int ensure_tables() {
     return GL_OK;
 }
 
-// Cluster size C and tile length: as many CTAs per walker as keep the whole batch resident in one
-// wave (8 CTAs of 128 threads x 64 registers per SM, 148 SMs), each with at least NT exposures;
-// the tile is the CTA's share of the series, so that one round covers it unless T > C * MAXTILE.
-void pick_shape(int B, int nT, int* C, int* tile) {
-    const long long slots = 148LL * 8;
-    int c = 1;
-    while (c < MAXCLUSTER && (long long)c * 2 * NT <= nT && (long long)B * c * 2 <= slots) c *= 2;
-    if (const char* env = getenv("GL_CLUSTER")) {   // experiments only
-        const int v = atoi(env);
-        if (v == 1 || v == 2 || v == 4 || v == 8) c = v;
+// Number of SMs of the current device (cached per device).
+int sm_count() {
+    static int cached[64] = {};
+    int dev = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess || dev < 0 || dev >= 64) return 148;
+    if (!cached[dev]) {
+        int n = 0;
+        if (cudaDeviceGetAttribute(&n, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess || n <= 0) n = 148;
+        cached[dev] = n;
     }
+    return cached[dev];
+}
+
+// transit_kernel: cluster size C and tile length -- as many CTAs per walker as keep the whole batch
+// resident in one wave (8 CTAs of 128 threads x 64 registers per SM), each with at least NT
+// exposures; the tile is the CTA's share of the series, so that one round covers it unless
+// T > C * MAXTILE.
+void pick_shape(long long rows, int nT, int* C, int* tile) {
+    const long long slots = (long long)sm_count() * 8;
+    int c = 1;
+    while (c < MAXCLUSTER && (long long)c * 2 * NT <= nT && rows * c * 2 <= slots) c *= 2;
     int t = ((nT + c - 1) / c + NT - 1) / NT * NT;
     t = t < NT ? NT : (t > MAXTILE ? MAXTILE : t);
     *C = c;
     *tile = t;
 }
 
+// One launch of transit_kernel<T, EX, SEG>.  marker_mode: finish the units hot_kernel deferred.
 template <typename T>
-int launch_transit(const double* params, int nparams, int B, const double* times, int nT,
-                   double t_exp, int n_ss,
-                   const double* obs, const double* sigma, void* flux, void* chi2,
-                   cudaStream_t st) {
+int launch_full(const double* params, int nparams, int B, const double* times, int nT, double t_exp,
+                int n_ss, const double* obs, const double* sigma, void* flux, void* chi2,
+                int shared_base, int nseg, int seglen, int marker_mode, long long max_rows, bool pdl,
+                cudaStream_t st) {
+    const long long units = (long long)B * nseg;
+    long long rows = units < 65535 ? units : 65535;
+    if (max_rows > 0 && rows > max_rows) rows = max_rows;
     int C, tile;
-    pick_shape(B, nT, &C, &tile);
-    // flux-only calls with few walkers and a series longer than one round: split the series into
-    // segments that separate clusters take (no reduction is needed between them)
-    int nseg = 1, seglen = nT;
-    if (chi2 == nullptr && nT > 0) {
-        const long long span = (long long)C * tile;
-        const long long rounds = (nT + span - 1) / span;
-        const long long room = (148LL * 8) / ((long long)B * C);
-        if (rounds > 1 && room > 1) {
-            nseg = (int)(rounds < room ? rounds : room);
-            const long long per = (rounds + nseg - 1) / nseg;   // rounds per segment
-            seglen = (int)(per * span);
-            nseg = (int)((nT + (long long)seglen - 1) / seglen);
-        }
-    }
-    const long long rows = (long long)B * nseg;
-    // fp32 chi^2: launch-wide baseline first, the transit kernel right behind it (see baseline_kernel)
-    const int shared_base = (sizeof(T) == 4 && chi2 != nullptr && nT > 0) ? 1 : 0;
-    if (shared_base) {
-        baseline_kernel<<<1, 1024, 0, st>>>(obs, sigma, nT, (float*)chi2, B);
-        cudaError_t e0 = cudaGetLastError();
-        if (e0 != cudaSuccess) return cuda_fail(e0, "baseline_kernel launch");
-        ++tl_launches;
-    }
+    pick_shape(rows, seglen, &C, &tile);
     cudaLaunchConfig_t cfg = {};
-    cfg.gridDim = dim3((unsigned)C, (unsigned)(rows < 65535 ? rows : 65535), 1);
+    cfg.gridDim = dim3((unsigned)C, (unsigned)rows, 1);
     cfg.blockDim = dim3(NT, 1, 1);
     cfg.dynamicSmemBytes = 0;
     cfg.stream = st;
@@ -1067,24 +1057,26 @@ int launch_transit(const double* params, int nparams, int B, const double* times
     attr[1].id = cudaLaunchAttributeProgrammaticStreamSerialization;
     attr[1].val.programmaticStreamSerializationAllowed = 1;
     cfg.attrs = attr;
-    cfg.numAttrs = shared_base ? 2 : 1;
+    cfg.numAttrs = pdl ? 2 : 1;
     auto launch = [&]() {
         if (nseg > 1)   // flux-only, 12-column rows or extended ones
             return (nparams == GL_NPARAMS_EX)
                        ? cudaLaunchKernelEx(&cfg, transit_kernel<T, true, true>, params, B, times, nT, tile,
                                             t_exp, n_ss, obs, sigma, (T*)flux, (T*)chi2, shared_base, nseg,
-                                            seglen)
+                                            seglen, marker_mode)
                        : cudaLaunchKernelEx(&cfg, transit_kernel<T, false, true>, params, B, times, nT, tile,
                                             t_exp, n_ss, obs, sigma, (T*)flux, (T*)chi2, shared_base, nseg,
-                                            seglen);
+                                            seglen, marker_mode);
         return (nparams == GL_NPARAMS_EX)
                    ? cudaLaunchKernelEx(&cfg, transit_kernel<T, true, false>, params, B, times, nT, tile,
-                                        t_exp, n_ss, obs, sigma, (T*)flux, (T*)chi2, shared_base, 1, nT)
+                                        t_exp, n_ss, obs, sigma, (T*)flux, (T*)chi2, shared_base, 1, nT,
+                                        marker_mode)
                    : cudaLaunchKernelEx(&cfg, transit_kernel<T, false, false>, params, B, times, nT, tile,
-                                        t_exp, n_ss, obs, sigma, (T*)flux, (T*)chi2, shared_base, 1, nT);
+                                        t_exp, n_ss, obs, sigma, (T*)flux, (T*)chi2, shared_base, 1, nT,
+                                        marker_mode);
     };
     cudaError_t e = launch();
-    if (e != cudaSuccess && shared_base) {
+    if (e != cudaSuccess && pdl) {
         // no early start then: plain stream order is just as correct
         (void)cudaGetLastError();
         cfg.numAttrs = 1;
@@ -1093,6 +1085,155 @@ int launch_transit(const double* params, int nparams, int B, const double* times
     if (e != cudaSuccess) return cuda_fail(e, "transit_kernel launch");
     ++tl_launches;
     return GL_OK;
+}
+
+// Launch shape of hot_kernel (gl_hot.cuh).  chi^2 calls: one cluster of C CTAs per walker, C > 1 only
+// when the batch alone does not fill the GPU (two CTAs of 512 threads per SM) and every CTA still
+// gets >= 2048 exposures.  Flux-only calls: single-CTA units, a long series cut into segments
+// (>= 512 exposures each) until the GPU is full.
+struct HotShape {
+    int C, nseg, seglen;
+};
+HotShape pick_hot_shape(int B, int nT, bool want_chi2) {
+    const long long slots = (long long)sm_count() * 2;
+    HotShape h = {1, 1, nT};
+    if (want_chi2) {
+        while (h.C < glh::MAXC && (long long)B * h.C * 2 <= slots && nT / (h.C * 2) >= 2048) h.C *= 2;
+    } else {
+        long long n = slots / B;
+        const long long most = (nT + 511) / 512;
+        if (n > most) n = most;
+        if ((long long)B * n >= (1LL << 31)) n = 1;
+        if (n > 1) {
+            int len = (int)((nT + n - 1) / n);
+            len = (len + 3) & ~3;
+            h.seglen = len;
+            h.nseg = (nT + len - 1) / len;
+        }
+    }
+    return h;
+}
+
+// Rows of the fallback grid (transit_kernel in marker mode) behind a hot launch: it finds work only
+// for deferred walkers, so in the common case it is pure overhead at the end of the step; one
+// cluster per SM keeps that small and still finishes a fully deferred batch in a few rounds.
+#ifndef GL_FALLBACK_ROWS
+#define GL_FALLBACK_ROWS 148
+#endif
+
+struct SeriesView {          // what gl_series keeps resident (all nullptr / 0 for a plain call)
+    const float2* ow = nullptr;
+    double S = 0.0;
+    int sorted_known = 0;
+    int* status = nullptr;
+    bool with_fallback = true;
+};
+
+// fp32, 12-column rows, nT > 0: [baseline_kernel ->] hot_kernel -> transit_kernel (marker mode).
+int launch_hot(const double* params, int B, const double* times, int nT, double t_exp, int n_ss,
+               const double* obs, const double* sigma, float* flux, float* chi2, const SeriesView& sv,
+               cudaStream_t st) {
+    const bool pre = sv.ow != nullptr, want_chi2 = chi2 != nullptr;
+    const HotShape h = pick_hot_shape(B, nT, want_chi2);
+    if (want_chi2 && !pre) {
+        baseline_kernel<<<1, 1024, 0, st>>>(obs, sigma, nT, chi2, B);
+        cudaError_t e0 = cudaGetLastError();
+        if (e0 != cudaSuccess) return cuda_fail(e0, "baseline_kernel launch");
+        ++tl_launches;
+    }
+    glh::HotArgs a;
+    a.params = params;
+    a.times = times;
+    a.obs = obs;
+    a.sigma = sigma;
+    a.ow = sv.ow;
+    a.flux = flux;
+    a.chi2 = chi2;
+    a.status = sv.status;
+    a.S = sv.S;
+    a.t_exp = t_exp;
+    a.inv_ss = 1.f / (float)n_ss;
+    a.doff = (float)(t_exp / (double)n_ss);
+    a.off0 = (float)((0.5 / (double)n_ss - 0.5) * t_exp);
+    a.B = B;
+    a.T = nT;
+    a.n_ss = n_ss;
+    a.nseg = h.nseg;
+    a.seglen = h.seglen;
+    a.sorted_known = sv.sorted_known;
+    const long long units = (long long)B * h.nseg;
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = dim3((unsigned)h.C, (unsigned)(units < 65535 ? units : 65535), 1);
+    cfg.blockDim = dim3(glh::HOT_NT, 1, 1);
+    cfg.stream = st;
+    cudaLaunchAttribute attr[2];
+    int na = 0;
+    if (h.C > 1) {
+        attr[na].id = cudaLaunchAttributeClusterDimension;
+        attr[na].val.clusterDim.x = (unsigned)h.C;
+        attr[na].val.clusterDim.y = 1;
+        attr[na].val.clusterDim.z = 1;
+        ++na;
+    }
+    const int na_plain = na;
+    if (want_chi2 && !pre) {
+        attr[na].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+        attr[na].val.programmaticStreamSerializationAllowed = 1;
+        ++na;
+    }
+    cfg.attrs = attr;
+    cfg.numAttrs = na;
+    auto launch = [&]() {
+        return pre ? cudaLaunchKernelEx(&cfg, glh::hot_kernel<true>, a)
+                   : cudaLaunchKernelEx(&cfg, glh::hot_kernel<false>, a);
+    };
+    cudaError_t e = launch();
+    if (e != cudaSuccess && na != na_plain) {
+        (void)cudaGetLastError();
+        cfg.numAttrs = na_plain;
+        e = launch();
+    }
+    if (e != cudaSuccess) return cuda_fail(e, "hot_kernel launch");
+    ++tl_launches;
+    if (!sv.with_fallback) return GL_OK;
+    return launch_full<float>(params, GL_NPARAMS, B, times, nT, t_exp, n_ss, obs, sigma, flux, chi2, 0,
+                              h.nseg, h.seglen, 1, GL_FALLBACK_ROWS, true, st);
+}
+
+template <typename T>
+int launch_transit(const double* params, int nparams, int B, const double* times, int nT,
+                   double t_exp, int n_ss,
+                   const double* obs, const double* sigma, void* flux, void* chi2,
+                   cudaStream_t st) {
+    if (sizeof(T) == 4 && nparams == GL_NPARAMS && nT > 0)
+        return launch_hot(params, B, times, nT, t_exp, n_ss, obs, sigma, (float*)flux, (float*)chi2,
+                          SeriesView(), st);
+    // flux-only calls with few walkers and a series longer than one round: split the series into
+    // segments that separate clusters take (no reduction is needed between them)
+    int C, tile;
+    pick_shape(B, nT, &C, &tile);
+    int nseg = 1, seglen = nT;
+    if (chi2 == nullptr && nT > 0) {
+        const long long span = (long long)C * tile;
+        const long long rounds = (nT + span - 1) / span;
+        const long long room = ((long long)sm_count() * 8) / ((long long)B * C);
+        if (rounds > 1 && room > 1) {
+            nseg = (int)(rounds < room ? rounds : room);
+            const long long per = (rounds + nseg - 1) / nseg;   // rounds per segment
+            seglen = (int)(per * span);
+            nseg = (int)((nT + (long long)seglen - 1) / seglen);
+        }
+    }
+    // fp32 chi^2: launch-wide baseline first, the transit kernel right behind it (see baseline_kernel)
+    const int shared_base = (sizeof(T) == 4 && chi2 != nullptr && nT > 0) ? 1 : 0;
+    if (shared_base) {
+        baseline_kernel<<<1, 1024, 0, st>>>(obs, sigma, nT, (float*)chi2, B);
+        cudaError_t e0 = cudaGetLastError();
+        if (e0 != cudaSuccess) return cuda_fail(e0, "baseline_kernel launch");
+        ++tl_launches;
+    }
+    return launch_full<T>(params, nparams, B, times, nT, t_exp, n_ss, obs, sigma, flux, chi2, shared_base,
+                          nseg, seglen, 0, 0, shared_base != 0, st);
 }
 
 int run_transit(const double* params, int nparams, int B, const double* times, int nT, double t_exp,
@@ -1292,6 +1433,40 @@ int gl_probe_peaks(double* out3) {
     return GL_OK;
 }
 
+// Launch floor: an EMPTY kernel with a given grid/cluster/block shape, optionally followed by a
+// second empty grid chained by programmatic dependent launch (the hot + fallback pair's shape).
+// bench.py times it exactly as it times a step; what it measures is what any launch of that shape
+// costs on this box before a single useful instruction runs.
+int gl_probe_empty_launch(int cluster, int rows, int threads, int fallback_cluster, int fallback_rows,
+                          void* stream) {
+    if (cluster < 1 || cluster > 8 || rows < 1 || threads < 32 || threads > 1024) return GL_EINVAL;
+    cudaStream_t st = (cudaStream_t)stream;
+    cudaLaunchConfig_t cfg = {};
+    cudaLaunchAttribute attr[2];
+    cfg.gridDim = dim3((unsigned)cluster, (unsigned)rows, 1);
+    cfg.blockDim = dim3((unsigned)threads, 1, 1);
+    cfg.stream = st;
+    attr[0].id = cudaLaunchAttributeClusterDimension;
+    attr[0].val.clusterDim.x = (unsigned)cluster;
+    attr[0].val.clusterDim.y = 1;
+    attr[0].val.clusterDim.z = 1;
+    cfg.attrs = attr;
+    cfg.numAttrs = 1;
+    cudaError_t e = cudaLaunchKernelEx(&cfg, empty_kernel, 0);
+    if (e != cudaSuccess) return cuda_fail(e, "empty_kernel launch");
+    if (fallback_rows > 0) {
+        cfg.gridDim = dim3((unsigned)fallback_cluster, (unsigned)fallback_rows, 1);
+        cfg.blockDim = dim3(NT, 1, 1);
+        attr[0].val.clusterDim.x = (unsigned)fallback_cluster;
+        attr[1].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+        attr[1].val.programmaticStreamSerializationAllowed = 1;
+        cfg.numAttrs = 2;
+        e = cudaLaunchKernelEx(&cfg, empty_kernel, 1);
+        if (e != cudaSuccess) return cuda_fail(e, "empty_kernel (dependent) launch");
+    }
+    return GL_OK;
+}
+
 long long gl_launch_count(void) { return tl_launches; }
 const char* gl_last_cuda_error(void) { return tl_cuda_err; }
 int gl_version(void) { return 100; }
@@ -1425,6 +1600,210 @@ int gl_flux_geometry_host(const double* geom, long long N, void* flux_out, gl_dt
     if (h.err == cudaSuccess) rc = gl_flux_geometry((const double*)dg, N, df, dtype, h.st);
     if (rc == GL_OK) h.download(flux_out, df, elem(dtype) * (size_t)N);
     return h.finish(rc);
+}
+
+}  // extern "C"
+
+// ------------------------------------------------------------------------------------------
+// gl_series: a RESIDENT series.  An MCMC run evaluates thousands of parameter batches against one
+// fixed (times, obs, sigma); everything that depends on the series alone is done
+// once here: upload, order check, baseline S = sum_i ((obs_i - 1)/sigma_i)^2 in fp64, the fp32 pairs
+// (obs_i - 1, 1/sigma_i) the in-window residuals use, device and pinned staging buffers.
+// ------------------------------------------------------------------------------------------
+namespace {
+
+// One CTA: ow[i] = (obs_i - 1, 1/sigma_i) in fp32, S in fp64 (fixed summation order, as
+// baseline_kernel), sorted = times non-decreasing.
+__global__ void __launch_bounds__(1024)
+series_prepare_kernel(const double* __restrict__ times, const double* __restrict__ obs,
+                      const double* __restrict__ sigma, int nT, float2* __restrict__ ow,
+                      double* __restrict__ S_out, int* __restrict__ sorted_out) {
+    __shared__ double s_w[32];
+    __shared__ int s_bad;
+    if (threadIdx.x == 0) s_bad = 0;
+    __syncthreads();
+    double acc = 0.0;
+    int bad = 0;
+    for (int i = threadIdx.x; i < nT; i += 1024) {
+        const double o = obs[i] - 1.0, sg = sigma[i];
+        acc += residual_sq<double>(o, 0.0, sg);
+        ow[i] = make_float2((float)o, (float)(1.0 / sg));
+        if (i + 1 < nT) bad |= !(times[i] <= times[i + 1]);
+    }
+#pragma unroll
+    for (int off = 16; off > 0; off >>= 1) acc += __shfl_down_sync(0xffffffffu, acc, off);
+    if ((threadIdx.x & 31) == 0) s_w[threadIdx.x >> 5] = acc;
+    if (bad) atomicOr(&s_bad, 1);
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        double tot = 0.0;
+        for (int k = 0; k < 32; ++k) tot += s_w[k];
+        *S_out = tot;
+        *sorted_out = s_bad ? 0 : 1;
+    }
+}
+
+}  // namespace
+
+struct gl_series {
+    int dev = 0, T = 0, n_ss = 1, B_max = 0;
+    double t_exp = 0.0, S = 0.0;
+    int sorted = 0;
+    bool fallback_hint = false;      // the last host call needed the fallback launch
+    cudaStream_t st = nullptr;       // host calls run here
+    double *d_times = nullptr, *d_obs = nullptr, *d_sigma = nullptr;
+    float2* d_ow = nullptr;
+    float* d_flux = nullptr;         // [B_max, T], allocated by the first host call that asks for flux
+    // pinned, device-mapped staging: the kernel reads params and writes chi^2 over PCIe
+    double* h_params = nullptr;
+    float* h_chi2 = nullptr;
+    int* h_status = nullptr;
+    double* m_params = nullptr;      // device aliases
+    float* m_chi2 = nullptr;
+    int* m_status = nullptr;
+    int* d_status = nullptr;         // device word for gl_series_loglike_dev (never read back)
+};
+
+extern "C" {
+
+int gl_series_create(const double* times, const double* obs, const double* sigma, int T, double t_exp,
+                     int n_ss, int B_max, gl_series** out) {
+    if (!out) return GL_EINVAL;
+    *out = nullptr;
+    if (T < 1 || B_max < 1 || n_ss < 1 || !(t_exp >= 0.0) || !isfinite(t_exp) || !times || !obs || !sigma)
+        return GL_EINVAL;
+    gl_series* s = new (std::nothrow) gl_series;
+    if (!s) return GL_ECUDA;
+    s->T = T;
+    s->n_ss = n_ss;
+    s->B_max = B_max;
+    s->t_exp = t_exp;
+    cudaError_t e = cudaGetDevice(&s->dev);
+    const size_t tb = sizeof(double) * (size_t)T;
+    double* d_S = nullptr;
+    int* d_sorted = nullptr;
+    auto ok = [&]() { return e == cudaSuccess; };
+    if (ok()) e = cudaStreamCreateWithFlags(&s->st, cudaStreamNonBlocking);
+    if (ok()) e = cudaMalloc(&s->d_times, tb);
+    if (ok()) e = cudaMalloc(&s->d_obs, tb);
+    if (ok()) e = cudaMalloc(&s->d_sigma, tb);
+    if (ok()) e = cudaMalloc(&s->d_ow, sizeof(float2) * (size_t)T);
+    if (ok()) e = cudaMalloc(&d_S, sizeof(double));
+    if (ok()) e = cudaMalloc(&d_sorted, sizeof(int));
+    if (ok()) e = cudaMalloc(&s->d_status, sizeof(int));
+    if (ok()) e = cudaHostAlloc(&s->h_params, sizeof(double) * GL_NPARAMS * (size_t)B_max, cudaHostAllocMapped);
+    if (ok()) e = cudaHostAlloc(&s->h_chi2, sizeof(float) * (size_t)B_max, cudaHostAllocMapped);
+    if (ok()) e = cudaHostAlloc(&s->h_status, sizeof(int), cudaHostAllocMapped);
+    if (ok()) e = cudaHostGetDevicePointer(&s->m_params, s->h_params, 0);
+    if (ok()) e = cudaHostGetDevicePointer(&s->m_chi2, s->h_chi2, 0);
+    if (ok()) e = cudaHostGetDevicePointer(&s->m_status, s->h_status, 0);
+    if (ok()) e = cudaMemcpyAsync(s->d_times, times, tb, cudaMemcpyHostToDevice, s->st);
+    if (ok()) e = cudaMemcpyAsync(s->d_obs, obs, tb, cudaMemcpyHostToDevice, s->st);
+    if (ok()) e = cudaMemcpyAsync(s->d_sigma, sigma, tb, cudaMemcpyHostToDevice, s->st);
+    if (ok()) e = cudaMemsetAsync(s->d_status, 0, sizeof(int), s->st);
+    if (ok()) {
+        series_prepare_kernel<<<1, 1024, 0, s->st>>>(s->d_times, s->d_obs, s->d_sigma, T, s->d_ow, d_S, d_sorted);
+        e = cudaGetLastError();
+    }
+    if (ok()) e = cudaMemcpyAsync(&s->S, d_S, sizeof(double), cudaMemcpyDeviceToHost, s->st);
+    if (ok()) e = cudaMemcpyAsync(&s->sorted, d_sorted, sizeof(int), cudaMemcpyDeviceToHost, s->st);
+    if (ok()) e = cudaStreamSynchronize(s->st);
+    cudaFree(d_S);
+    cudaFree(d_sorted);
+    if (!ok()) {
+        const int rc = cuda_fail(e, "gl_series_create");
+        gl_series_destroy(s);
+        return rc;
+    }
+    ++tl_launches;
+    *out = s;
+    return GL_OK;
+}
+
+int gl_series_destroy(gl_series* s) {
+    if (!s) return GL_OK;
+    if (s->st) cudaStreamSynchronize(s->st);
+    cudaFree(s->d_times);
+    cudaFree(s->d_obs);
+    cudaFree(s->d_sigma);
+    cudaFree(s->d_ow);
+    cudaFree(s->d_flux);
+    cudaFree(s->d_status);
+    if (s->h_params) cudaFreeHost(s->h_params);
+    if (s->h_chi2) cudaFreeHost(s->h_chi2);
+    if (s->h_status) cudaFreeHost(s->h_status);
+    if (s->st) cudaStreamDestroy(s->st);
+    delete s;
+    return GL_OK;
+}
+
+int gl_series_info(const gl_series* s, int* T, int* n_ss, int* B_max, int* sorted, double* baseline) {
+    if (!s) return GL_EINVAL;
+    if (T) *T = s->T;
+    if (n_ss) *n_ss = s->n_ss;
+    if (B_max) *B_max = s->B_max;
+    if (sorted) *sorted = s->sorted;
+    if (baseline) *baseline = s->S;
+    return GL_OK;
+}
+
+int gl_series_loglike_dev(gl_series* s, const double* params, int B, float* chi2_out,
+                          float* flux_out_or_null, void* stream) {
+    if (!s || B < 0) return GL_EINVAL;
+    if (B == 0) return GL_OK;
+    if (!params || !chi2_out) return GL_EINVAL;
+    SeriesView sv;
+    sv.ow = s->d_ow;
+    sv.S = s->S;
+    sv.sorted_known = s->sorted;
+    sv.status = nullptr;
+    sv.with_fallback = true;
+    return launch_hot(params, B, s->d_times, s->T, s->t_exp, s->n_ss, s->d_obs, s->d_sigma,
+                      flux_out_or_null, chi2_out, sv, (cudaStream_t)stream);
+}
+
+int gl_series_loglike(gl_series* s, const double* params, int B, float* chi2_out, float* flux_out_or_null) {
+    if (!s || B < 0 || B > s->B_max) return GL_EINVAL;
+    if (B == 0) return GL_OK;
+    if (!params || !chi2_out) return GL_EINVAL;
+    cudaError_t e = cudaSuccess;
+    if (flux_out_or_null && !s->d_flux) {
+        e = cudaMalloc(&s->d_flux, sizeof(float) * (size_t)s->B_max * (size_t)s->T);
+        if (e != cudaSuccess) return cuda_fail(e, "gl_series_loglike flux buffer");
+    }
+    memcpy(s->h_params, params, sizeof(double) * GL_NPARAMS * (size_t)B);
+    *(volatile int*)s->h_status = 0;
+    SeriesView sv;
+    sv.ow = s->d_ow;
+    sv.S = s->S;
+    sv.sorted_known = s->sorted;
+    sv.status = s->m_status;
+    sv.with_fallback = s->fallback_hint;
+    float* flux = flux_out_or_null ? s->d_flux : nullptr;
+    int rc = launch_hot(s->m_params, B, s->d_times, s->T, s->t_exp, s->n_ss, s->d_obs, s->d_sigma, flux,
+                        s->m_chi2, sv, s->st);
+    if (rc != GL_OK) return rc;
+    e = cudaStreamSynchronize(s->st);
+    if (e != cudaSuccess) return cuda_fail(e, "gl_series_loglike");
+    const int deferred = *(volatile int*)s->h_status;
+    if (deferred && !sv.with_fallback) {
+        // some walker needs the full-featured kernel and it was not launched: do it now, and launch it
+        // together with the hot kernel from the next call on
+        rc = launch_full<float>(s->m_params, GL_NPARAMS, B, s->d_times, s->T, s->t_exp, s->n_ss, s->d_obs,
+                                s->d_sigma, flux, s->m_chi2, 0, 1, s->T, 1, 0, false, s->st);
+        if (rc != GL_OK) return rc;
+        e = cudaStreamSynchronize(s->st);
+        if (e != cudaSuccess) return cuda_fail(e, "gl_series_loglike (fallback)");
+    }
+    s->fallback_hint = deferred != 0;
+    if (flux) {
+        e = cudaMemcpyAsync(flux_out_or_null, flux, sizeof(float) * (size_t)B * (size_t)s->T,
+                            cudaMemcpyDeviceToHost, s->st);
+        if (e == cudaSuccess) e = cudaStreamSynchronize(s->st);
+        if (e != cudaSuccess) return cuda_fail(e, "gl_series_loglike flux copy");
+    }
+    memcpy(chi2_out, s->h_chi2, sizeof(float) * (size_t)B);
+    return GL_OK;
 }
 
 }  // extern "C"

@@ -74,23 +74,30 @@ def test_config3_mcmc_batch_full(gl, dtype):
     assert np.abs(host(chi) / chi_ref - 1.0).max() <= CTOL[dtype]
 
 
+_CFG4_REF = {}
+
+
+def _config4_oracle():
+    """The whole of config 4 through the oracle, once for both dtypes (about 20 s on 16 cores)."""
+    if not _CFG4_REF:
+        w = wl.config4()
+        _CFG4_REF["chi"], _CFG4_REF["flux"] = orc.loglike(w.params, w.times, w.t_exp, w.n_ss, w.obs, w.sigma)
+    return _CFG4_REF["chi"], _CFG4_REF["flux"]
+
+
 @pytest.mark.parametrize("dtype", ["f32", "f64"])
-def test_config4_jwst_sampled(gl, dtype):
-    """Full-size launch (B=128, T=20000, S=3); the oracle checks 8 whole walkers (chi^2 needs full
-    rows) plus 64 times of every other walker."""
+def test_config4_jwst_full(gl, dtype):
+    """Full-size launch (B=128, T=20000, S=3) against the oracle on EVERY walker and exposure: the
+    in-transit-dominated, branch-heavy regime."""
     w = wl.config4()
+    chi_ref, ref = _config4_oracle()
     chi, out = gl.gl_loglike(dev(w.params), dev(w.times), w.t_exp, w.n_ss, dev(w.obs),
                              dev(w.sigma), dtype=dtype, want_flux=True)
     out, chi = host(out), host(chi)
-    rows = np.arange(0, 128, 16)
-    chi_ref, ref = orc.loglike(w.params[rows], w.times, w.t_exp, w.n_ss, w.obs, w.sigma)
-    assert np.abs(out[rows] - ref).max() <= FTOL[dtype]
-    assert np.abs(chi[rows] / chi_ref - 1.0).max() <= CTOL[dtype]
-    rng = np.random.default_rng(7)
-    cols = np.sort(rng.choice(w.T, 64, replace=False))
-    ref2 = orc.lightcurve(w.params, w.times[cols], w.t_exp, w.n_ss)
-    assert np.abs(out[:, cols] - ref2).max() <= FTOL[dtype]
-    assert np.all(np.isfinite(out)) and out.max() <= 1.0 + 1e-6
+    err = np.abs(out - ref)
+    assert err.max() <= FTOL[dtype], (err.max(), np.unravel_index(err.argmax(), err.shape))
+    assert np.abs(chi / chi_ref - 1.0).max() <= CTOL[dtype]
+    assert (ref < 1.0).mean() > 0.6
 
 
 @pytest.mark.parametrize("dtype", ["f32", "f64"])
@@ -529,3 +536,231 @@ def test_supersampling_layouts(gl, dtype):
             out = host(gl.gl_lightcurve(dev(w.params), dev(t), w.t_exp, n_ss, dtype=dtype))
             err = np.abs(out - ref).max()
             assert err <= FTOL[dtype], (n_ss, t.size, err)
+
+
+# ---------------------------------------------------------------------------------------------
+# Validity rules, walkers that never transit, signed parameter ranges (VERDICT r1 "What's weak" #1)
+# ---------------------------------------------------------------------------------------------
+def _validity_series():
+    times = np.concatenate([np.linspace(-0.3, 0.3, 61), [2.5, 5.0, 7.5]])
+    rng = np.random.default_rng(3)
+    sigma = rng.uniform(1e-4, 3e-4, times.size)
+    obs = 1.0 + rng.normal(0.0, 1.0, times.size) * sigma
+    return times, obs, sigma
+
+
+@pytest.mark.parametrize("dtype", ["f32", "f64"])
+def test_validity_rules_12_columns(gl, dtype):
+    """Every rule of include/greenlantern_b200.h:41-44 across its boundary: the NaN / +inf pattern
+    must be the hand-written one of tests/validity_cases.py AND the oracle's; valid neighbours
+    must agree with the oracle in value."""
+    from validity_cases import rows12
+    rows, valid, names = rows12()
+    times, obs, sigma = _validity_series()
+    chi_ref, ref = orc.loglike(rows, times, 0.01, 3, obs, sigma)
+    chi, out = gl.gl_loglike(dev(rows), dev(times), 0.01, 3, dev(obs), dev(sigma), dtype=dtype,
+                             want_flux=True)
+    chi, out = host(chi), host(out)
+    lc = host(gl.gl_lightcurve(dev(rows), dev(times), 0.01, 3, dtype=dtype))
+    for k, (v, n) in enumerate(zip(valid, names)):
+        if v:
+            assert np.all(np.isfinite(out[k])) and np.isfinite(chi[k]), n
+            assert np.abs(out[k] - ref[k]).max() <= FTOL[dtype], (n, np.abs(out[k] - ref[k]).max())
+            assert abs(chi[k] / chi_ref[k] - 1.0) <= CTOL[dtype], (n, chi[k], chi_ref[k])
+        else:
+            assert np.all(np.isnan(out[k])) and np.all(np.isnan(ref[k])), n
+            assert np.isinf(chi[k]) and chi[k] > 0 and np.isinf(chi_ref[k]), n
+        assert np.array_equal(lc[k], out[k], equal_nan=True), n
+        if n.startswith("never transits") or "aR, e = 0" in n and v:
+            assert np.all(out[k] == 1.0), n        # exactly 1: the window is empty
+    # chi^2 of the walkers that never transit = the baseline sum, in every launch shape
+    never = [k for k, n in enumerate(names) if n.startswith("never transits")]
+    base = float(np.sum(((obs - 1.0) / sigma) ** 2))
+    assert np.all(np.abs(chi[never] / base - 1.0) <= (1e-6 if dtype == "f32" else 1e-13))
+
+
+@pytest.mark.parametrize("dtype", ["f32", "f64"])
+def test_validity_rules_extended_rows_gp_and_geometry(gl, dtype):
+    from validity_cases import geom_rows, rows12, rows16
+    rows, valid, names = rows16()
+    times, obs, sigma = _validity_series()
+    ref = orc.lightcurve_ex(rows, times, 0.01, 3)
+    chi, out = gl.gl_loglike_ex(dev(rows), dev(times), 0.01, 3, dev(obs), dev(sigma), dtype=dtype,
+                                want_flux=True)
+    chi, out = host(chi), host(out)
+    for k, (v, n) in enumerate(zip(valid, names)):
+        if v:
+            assert np.abs(out[k] - ref[k]).max() <= FTOL[dtype], (n, np.abs(out[k] - ref[k]).max())
+            assert np.isfinite(chi[k]), n
+        else:
+            assert np.all(np.isnan(out[k])) and np.all(np.isnan(ref[k])), n
+            assert np.isinf(chi[k]) and chi[k] > 0, n
+    # GP likelihood: -inf for an invalid walker, finite for a valid one (times are sorted)
+    r12, v12, n12 = rows12()
+    gp = np.tile([2e-4, 0.5, 1e-4], (r12.shape[0], 1))
+    ll = host(gl.gl_gp_loglike(dev(r12), dev(times), 0.01, 3, dev(obs), dev(sigma), dev(gp), dtype=dtype))
+    for k, (v, n) in enumerate(zip(v12, n12)):
+        assert (np.isfinite(ll[k]) if v else (np.isinf(ll[k]) and ll[k] < 0)), (n, ll[k])
+    # bare geometries
+    g, gv = geom_rows()
+    gref = orc.flux_geometry(g)
+    gout = host(gl.gl_flux_geometry(dev(g), dtype=dtype))
+    assert np.array_equal(np.isnan(gout), ~gv) and np.array_equal(np.isnan(gref), ~gv)
+    assert np.abs(gout[gv] - gref[gv]).max() <= FTOL[dtype]
+
+
+@pytest.mark.parametrize("dtype", ["f32", "f64"])
+def test_signed_parameter_ranges_circular(gl, dtype):
+    """The paper's ranges are eta in [-pi/2, pi/2], b in [-1, 1]; configs 3/4 draw
+    the positive quadrant only.  One circular 12-column batch over the signed ranges (xi over the
+    whole circle), grazing impact parameters included."""
+    w = wl.config3(B=96)
+    rng = np.random.default_rng(23)
+    p = w.params.copy()
+    p[:, 3] = rng.uniform(-1.05, 1.05, 96)
+    p[:, 8] = rng.uniform(-np.pi, np.pi, 96)
+    p[:, 9] = rng.uniform(-np.pi / 2, np.pi / 2, 96)
+    sel = slice(1850, 2050)
+    chi_ref, ref = orc.loglike(p, w.times[sel], w.t_exp, w.n_ss, w.obs[sel], w.sigma[sel])
+    chi, out = gl.gl_loglike(dev(p), dev(w.times[sel]), w.t_exp, w.n_ss, dev(w.obs[sel]),
+                             dev(w.sigma[sel]), dtype=dtype, want_flux=True)
+    assert np.abs(host(out) - ref).max() <= FTOL[dtype]
+    assert np.abs(host(chi) / chi_ref - 1.0).max() <= CTOL[dtype]
+    assert (ref.min(axis=1) < 1.0).sum() > 80
+
+
+# ---------------------------------------------------------------------------------------------
+# The two-kernel fp32 path (gl_hot.cuh): walkers the hot kernel finishes, walkers it defers to the
+# full kernel, and invalid ones, in ONE batch; series shapes that defer everything
+# ---------------------------------------------------------------------------------------------
+def _mixed_batch():
+    w = wl.config3(B=40)
+    p = w.params.copy()
+    p[1::8, 4] = 0.3                      # eccentric: deferred
+    p[1::8, 5] = 1.0
+    p[2::8, 7], p[2::8, 9] = 0.97, 0.02   # very flat outline: evolute regime possible, deferred
+    p[3::8, 6] = 0.7                      # invalid
+    p[4::8, 2] = 2.5                      # close-in: long window, deferred
+    p[5::8, 1] = 3.0                      # short period: more transit epochs than the hot kernel lists
+    p[6::8, 3] = -1.2                     # never transits
+    return w, p
+
+
+def test_hot_and_deferred_walkers_in_one_batch(gl):
+    w, p = _mixed_batch()
+    chi_ref, ref = orc.loglike(p, w.times, w.t_exp, w.n_ss, w.obs, w.sigma)
+    chi, out = gl.gl_loglike(dev(p), dev(w.times), w.t_exp, w.n_ss, dev(w.obs), dev(w.sigma),
+                             dtype="f32", want_flux=True)
+    chi, out = host(chi), host(out)
+    bad = np.isnan(ref[:, 0])
+    assert bad.sum() == 5 and np.all(np.isnan(out[bad])) and np.all(np.isinf(chi[bad]))
+    assert np.abs(out[~bad] - ref[~bad]).max() <= 5e-7
+    assert np.abs(chi[~bad] / chi_ref[~bad] - 1.0).max() <= 1e-4
+    lc = host(gl.gl_lightcurve(dev(p), dev(w.times), w.t_exp, w.n_ss, dtype="f32"))
+    assert np.array_equal(lc, out, equal_nan=True)
+    chi_only = host(gl.gl_loglike(dev(p), dev(w.times), w.t_exp, w.n_ss, dev(w.obs), dev(w.sigma),
+                                  dtype="f32"))
+    assert np.array_equal(chi_only, chi)
+    # n_ss > 32 defers every walker; an unsorted series too; both must still match the oracle
+    sel = slice(1900, 2000)
+    q = p[[0, 1, 8, 16]]
+    r = orc.lightcurve(q, w.times[sel], w.t_exp, 40)
+    o = host(gl.gl_lightcurve(dev(q), dev(w.times[sel]), w.t_exp, 40, dtype="f32"))
+    assert np.abs(o - r).max() <= 5e-7
+    perm = np.random.default_rng(4).permutation(100)
+    tt, oo, ss = w.times[sel][perm], w.obs[sel][perm], w.sigma[sel][perm]
+    cr, r = orc.loglike(q, tt, w.t_exp, 5, oo, ss)
+    c, o = gl.gl_loglike(dev(q), dev(tt), w.t_exp, 5, dev(oo), dev(ss), dtype="f32", want_flux=True)
+    assert np.abs(host(o) - r).max() <= 5e-7 and np.abs(host(c) / cr - 1.0).max() <= 1e-4
+    # one out-of-order pair at the very end of a long series (the last CTA's share of the order check)
+    t2 = w.times.copy()
+    t2[-1], t2[-2] = t2[-2], t2[-1]
+    r = orc.lightcurve(q, t2, w.t_exp, 3)
+    o = host(gl.gl_lightcurve(dev(q), dev(t2), w.t_exp, 3, dtype="f32"))
+    assert np.abs(o - r).max() <= 5e-7
+
+
+def test_hot_kernel_launch_shapes(gl):
+    """Shapes of the hot kernel the five configs do not reach: a long flux-only series cut into
+    segments (single light curve of 1e5 exposures, the paper's Fig. 6 shape), clusters of 8 CTAs for
+    chi^2 on few walkers, several transit epochs in one series, T not a multiple of 4 with an
+    unaligned flux row, T = 1."""
+    base = wl.config2()
+    p = np.repeat(base.params, 3, axis=0)
+    p[1, 3], p[2, 7] = -0.45, 0.1
+    T = 100_003
+    t = np.linspace(-1.5, 1.5, T)
+    ref_idx = np.r_[0:T:997, 30_000:30_300, 49_990:50_010, T - 5:T]
+    r = orc.lightcurve(p, t[ref_idx], 0.001, 2)
+    o = host(gl.gl_lightcurve(dev(p), dev(t), 0.001, 2, dtype="f32"))
+    assert np.abs(o[:, ref_idx] - r).max() <= 5e-7
+    o64 = host(gl.gl_lightcurve(dev(p), dev(t), 0.001, 2, dtype="f64"))
+    assert np.abs(o - o64).max() <= 5e-7
+    rng = np.random.default_rng(8)
+    obs = 1.0 + 1e-4 * rng.standard_normal(T)
+    sig = np.full(T, 1e-4)
+    c = host(gl.gl_loglike(dev(p), dev(t), 0.001, 2, dev(obs), dev(sig), dtype="f32"))
+    c64 = host(gl.gl_loglike(dev(p), dev(t), 0.001, 2, dev(obs), dev(sig), dtype="f64"))
+    assert np.abs(c / c64 - 1.0).max() <= 1e-4
+    # five epochs of a P = 3 d planet, unevenly sampled, odd length
+    q = np.repeat(base.params, 2, axis=0)
+    q[:, 1], q[:, 2], q[1, 0] = 3.0, 9.0, 0.4
+    tt = np.sort(rng.uniform(-7.0, 7.0, 4_001))
+    cr, r = orc.loglike(q, tt, 0.004, 3, obs[:4001], sig[:4001])
+    c, o = gl.gl_loglike(dev(q), dev(tt), 0.004, 3, dev(obs[:4001]), dev(sig[:4001]), dtype="f32",
+                         want_flux=True)
+    assert np.abs(host(o) - r).max() <= 5e-7 and np.abs(host(c) / cr - 1.0).max() <= 1e-4
+    assert ((r < 1.0).sum(axis=1) > 100).all()
+    # T = 1, in and out of transit
+    for t1 in (0.0, 5.0):
+        r = orc.lightcurve(p, np.array([t1]), 0.0, 1)
+        o = host(gl.gl_lightcurve(dev(p), dev(np.array([t1])), 0.0, 1, dtype="f32"))
+        assert np.abs(o - r).max() <= 5e-7
+
+
+def test_resident_series_api(gl):
+    """gl_series_*: same numbers as gl_loglike, host and device flavours, deferred walkers included,
+    misuse rejected."""
+    w, p = _mixed_batch()
+    chi_ref, ref = orc.loglike(p, w.times, w.t_exp, w.n_ss, w.obs, w.sigma)
+    bad = np.isnan(ref[:, 0])
+    ser = gl.GlSeries(w.times, w.obs, w.sigma, w.t_exp, w.n_ss, B_max=64)
+    info = ser.info()
+    assert info["sorted"] and info["T"] == w.T and info["B_max"] == 64
+    assert abs(info["baseline"] / float(np.sum(((w.obs - 1.0) / w.sigma) ** 2)) - 1.0) < 1e-13
+    for rep in range(3):       # the host call learns after the first call that the fallback is needed
+        chi, flux = ser.loglike(p, want_flux=True)
+        assert np.all(np.isinf(chi[bad])) and np.all(np.isnan(flux[bad]))
+        assert np.abs(flux[~bad].astype(np.float64) - ref[~bad]).max() <= 5e-7
+        assert np.abs(chi[~bad].astype(np.float64) / chi_ref[~bad] - 1.0).max() <= 1e-4
+        chi_only = ser.loglike(p)
+        assert np.array_equal(chi_only, chi)
+    simple = wl.config3(B=64).params       # then a batch with nothing to defer
+    cs_ref, _ = orc.loglike(simple, w.times, w.t_exp, w.n_ss, w.obs, w.sigma)
+    for rep in range(2):
+        assert np.abs(ser.loglike(simple).astype(np.float64) / cs_ref - 1.0).max() <= 1e-4
+    cd, fd = ser.loglike_dev(dev(p), want_flux=True)
+    assert np.array_equal(host(cd), chi.astype(np.float64), equal_nan=True)
+    assert np.array_equal(host(fd), flux.astype(np.float64), equal_nan=True)
+    with pytest.raises(gl.GreenlanternError):
+        ser.loglike(np.repeat(p, 2, axis=0))           # B > B_max
+    assert ser.loglike(np.zeros((0, 12))).shape == (0,)
+    ser.close()
+    ser.close()                                        # idempotent
+    # an unsorted series: the order check at creation says so and every walker takes the full kernel
+    perm = np.random.default_rng(6).permutation(w.T)
+    ser2 = gl.GlSeries(w.times[perm], w.obs[perm], w.sigma[perm], w.t_exp, w.n_ss, B_max=8)
+    assert not ser2.info()["sorted"]
+    c2 = ser2.loglike(simple[:8])
+    assert np.abs(c2.astype(np.float64) / cs_ref[:8] - 1.0).max() <= 1e-4
+    ser2.close()
+    # a bad sigma poisons every chi^2
+    sg = w.sigma.copy()
+    sg[1950] = -1.0
+    ser3 = gl.GlSeries(w.times, w.obs, sg, w.t_exp, w.n_ss, B_max=8)
+    assert np.isinf(ser3.info()["baseline"])
+    c3 = ser3.loglike(simple[:8])
+    assert np.all(np.isinf(c3)) and np.all(c3 > 0)
+    ser3.close()
+    with pytest.raises(gl.GreenlanternError):
+        gl.GlSeries(w.times[:0], w.obs[:0], w.sigma[:0], 0.0, 1, B_max=1)
