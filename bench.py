@@ -1,13 +1,19 @@
 #!/usr/bin/env python
-"""bench.py -- throughput of the fused oblate-transit kernel on BASELINE.json's headline workload.
+"""bench.py -- throughput of the fused oblate-transit path on BASELINE.json's headline workload.
 
     python bench.py [--gpus N] [--steps K] [--warmup W] [--workload cfg3|cfg4] [--impl reference]
+                    [--no-extra] [--no-cpu-baseline] [--dry]
 
-One step = one pass of the whole hot path (prelude, Kepler/position, crossings, boundary integrals,
-exposure mean, chi^2) over one batch: gl_loglike with flux output, i.e. chi2[B] and flux[B,T].
+One step = one pass of the whole hot path (prelude, position, crossings, boundary integrals,
+exposure mean, chi^2) over one batch: chi2[B] AND flux[B,T] for B walkers against a resident series
+(gl_series_loglike_dev: the series was uploaded once, the parameter rows are resident in HBM).
 Default workload: config 3 of BASELINE.json (B=256 walkers x T=3900 x 15 sub-exposures, fp32), the
 configuration the metric's ">= 40 % of FP32 SIMT peak" is quoted on.  Prints ONE JSON line.
-See DESIGN.md "Measurement" for what every key means and how the roofline numbers are formed.
+`extra` carries the other workloads (cfg4, cfg5, cfg3 in fp64, one light curve of 1e5 exposures,
+the stateless gl_loglike call) timed the same way in the same run.
+`--gpus N` without a torchrun environment starts N ranks itself (torch.distributed.run on
+127.0.0.1); `--dry` exercises that plumbing on a CPU box with the gloo backend and no kernels.
+See DESIGN.md section 6 for what every key means and how the roofline numbers are formed.
 """
 from __future__ import annotations
 
@@ -32,12 +38,20 @@ METRIC = "oblate-transit flux evals/sec (fp32, quad LD)"
 UNIT = "flux evals/s"
 # FP32 SIMT peak of a B200: 148 SMs x 128 FP32 lanes x 2 flop (FMA) x SM clock.
 N_SM, LANES = 148, 128
-# Algorithmic fp32 flop per in-transit sub-exposure (operation count of the scheme with the whole
-# outline inside the disc); limb-crossing samples need ~1050, so this undercounts.
-ALG_FLOP_PER_SUBSAMPLE = 750.0
-# dram__bytes_read.sum + dram__bytes_write.sum of ONE launch of transit_kernel<float>, from the
-# `ncu --set full` captures summarised in profiles/r01_v5.md (not measured live: ncu is not run here)
-NCU_DRAM_BYTES = {"cfg3": 232_704 + 0, "cfg4": 606_464 + 15_872}
+# Algorithmic fp32 flop per in-transit sub-exposure: 1.0-1.1 kflop with the outline
+# inside the disc (16 f_lin nodes x 60-70 flop + ~100), 1.4-1.6 kflop when it crosses the limb (root
+# isolation + polishing + atan2).  Mid-points; the mix is counted per workload from the sky distance.
+ALG_FLOP_INSIDE, ALG_FLOP_LIMB = 1050.0, 1500.0
+NCU_FILE = ROOT / "profiles" / "r02_ncu_constants.json"
+
+
+def ncu_constants():
+    """Counters of the SHIPPED kernels from the committed ncu captures (profiles/r02_kernels.md), keyed
+    by the commit they were captured at; bench.py cannot run ncu itself."""
+    try:
+        return json.loads(NCU_FILE.read_text())
+    except (OSError, ValueError):
+        return {}
 
 
 def make_workload(name, rank):
@@ -49,18 +63,28 @@ def make_workload(name, rank):
         w = wl.config4()
         if rank:
             w.params = wl.draw_walkers(w.B, wl.SEED_CFG4_WALKERS + 1000 * rank)
-    elif name in ("cfg4ex_free", "cfg4ex_locked"):
-        # NEXT-2 context lines: config 4's batch with the extended rows of gl_loglike_ex (triaxial
-        # axes 1 : 0.9 : 1.1 x (1-f), zeta = 0.3 rad), orientation free or tidally locked
-        w = wl.config4()
-        if rank:
-            w.params = wl.draw_walkers(w.B, wl.SEED_CFG4_WALKERS + 1000 * rank)
-        ext = np.tile([0.3, 0.9, 1.1, 1.0 if name.endswith("locked") else 0.0], (w.B, 1))
-        w.params = np.concatenate([w.params, ext], axis=1)
-        w.name = w.name.replace("cfg4", name)
     else:
         raise SystemExit(f"unknown workload {name}")
     return w
+
+
+def in_transit_mix(w):
+    """(in-transit sub-exposures, of which the outline crosses the limb) for circular walkers, from the
+    sky distance of the planet centre alone (eqs. 9-10): bookkeeping for the
+    algorithmic flop count, not part of any timed path."""
+    p = w.params
+    offs = ((np.arange(w.n_ss) + 0.5) / w.n_ss - 0.5) * w.t_exp
+    n_in = n_limb = 0
+    for row in p:
+        t0, P, aR, b, rp = row[0], row[1], row[2], row[3], row[6]
+        ph = (w.times[:, None] + offs[None, :] - t0) / P
+        ph -= np.rint(ph)
+        near = np.abs(ph) < 0.25
+        phi = 2.0 * np.pi * ph[near]
+        r0 = np.hypot(b * np.cos(phi), aR * np.sin(phi))
+        n_in += int((r0 < 1.0 + rp).sum())
+        n_limb += int(((r0 < 1.0 + rp) & (r0 > 1.0 - rp)).sum())
+    return n_in, n_limb
 
 
 class ClockSampler:
@@ -108,17 +132,19 @@ class ClockSampler:
                 "reasons": sorted(reasons)}
 
 
-def oracle_timed(w, repeat=1):
-    """The CPU oracle as it stands, all host cores, on the whole workload."""
+# ---------------------------------------------------------------------------------------------
+# reference arm = the oracle (tier rules): timed as it stands on the host cores
+# ---------------------------------------------------------------------------------------------
+def oracle_timed(w, nthreads=0, rows=None):
+    """The CPU oracle as it stands on `rows` walkers of the workload (all if None)."""
     import oracle as orc
     orc.build()
+    p = w.params if rows is None else w.params[:rows]
     t0 = time.perf_counter()
-    used = 0
-    for _ in range(repeat):
-        _, _, used = orc.loglike(w.params, w.times, w.t_exp, w.n_ss, w.obs, w.sigma,
-                                 return_threads=True)
-    dt = (time.perf_counter() - t0) / repeat
-    return w.B * w.T / dt, used, dt
+    _, _, used = orc.loglike(p, w.times, w.t_exp, w.n_ss, w.obs, w.sigma, nthreads=nthreads,
+                             return_threads=True)
+    dt = time.perf_counter() - t0
+    return p.shape[0] * w.T / dt, used, dt
 
 
 def run_reference(args):
@@ -126,7 +152,8 @@ def run_reference(args):
     if rank != 0:
         return
     w = make_workload(args.workload, 0)
-    for _ in range(min(args.warmup, 1)):
+    W = min(args.warmup, 1)
+    for _ in range(W):
         oracle_timed(w)
     times = []
     used = 0
@@ -137,8 +164,9 @@ def run_reference(args):
     value = w.B * w.T / (ms * 1e-3)
     sample = f"whole workload {w.name} (B={w.B}, T={w.T}, S={w.n_ss}) per step, OpenMP over (walker,time)"
     print(json.dumps({
-        "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
-        "steps": args.steps, "warmup": min(args.warmup, 1), "ms_per_step": ms,
+        "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT,
+        "n_gpus": int(os.environ.get("WORLD_SIZE", args.gpus)),
+        "steps": args.steps, "warmup": W, "ms_per_step": ms,
         "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
         "data": "synthetic", "config": {"workload": w.name, "B": w.B, "T": w.T, "n_ss": w.n_ss},
         "cpu_baseline": {"value": value, "unit": UNIT, "cores": used, "kind": "oracle",
@@ -148,25 +176,70 @@ def run_reference(args):
     }))
 
 
+# ---------------------------------------------------------------------------------------------
+# multi-rank plumbing
+# ---------------------------------------------------------------------------------------------
+def spawn_ranks(args):
+    """--gpus N outside torchrun: start N ranks on this node (one process per GPU) and relay rank 0's
+    JSON line."""
+    port = 29500 + (os.getpid() % 2000)
+    cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", f"--nproc-per-node={args.gpus}",
+           "--master-addr", "127.0.0.1", "--master-port", str(port), str(Path(__file__).resolve()),
+           *sys.argv[1:]]
+    return subprocess.call(cmd)
+
+
+def run_dry(args, world, rank):
+    """The multi-rank code path without a GPU (tests/test_multirank_host.py): sharded walker draw,
+    barrier, max-over-ranks of a per-rank time, one JSON line from rank 0."""
+    import torch
+    import torch.distributed as dist
+    if world > 1:
+        dist.init_process_group("gloo")
+    w = make_workload(args.workload, rank)
+    t = torch.tensor([1.0 + rank], dtype=torch.float64)     # stand-in for the per-rank device time [ms]
+    shard = torch.tensor([float(w.params[:, 0].sum())], dtype=torch.float64)
+    gathered = [torch.zeros_like(shard) for _ in range(world)]
+    if world > 1:
+        dist.barrier()
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        dist.all_gather(gathered, shard)
+    else:
+        gathered = [shard]
+    if rank == 0:
+        print(json.dumps({"metric": METRIC, "dry": True, "n_gpus": world, "steps": args.steps,
+                          "ms_per_step": float(t.item()), "value": w.B * w.T * world / (float(t.item()) * 1e-3),
+                          "unit": UNIT, "scaling": "weak",
+                          "distinct_shards": len({round(float(g.item()), 9) for g in gathered}),
+                          "config": {"workload": w.name, "parallelism": f"dp{world} over walkers"}}))
+    if world > 1:
+        dist.destroy_process_group()
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
     ap.add_argument("--steps", type=int, default=50)
     ap.add_argument("--warmup", type=int, default=5)
-    ap.add_argument("--workload", default="cfg3",
-                    choices=["cfg3", "cfg4", "cfg4ex_free", "cfg4ex_locked"])
+    ap.add_argument("--workload", default="cfg3", choices=["cfg3", "cfg4"])
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-extra", action="store_true")
+    ap.add_argument("--dry", action="store_true", help="multi-rank plumbing only (gloo, no GPU)")
     args = ap.parse_args()
     if args.impl == "reference":
         return run_reference(args)
+    if "WORLD_SIZE" not in os.environ and args.gpus > 1:
+        raise SystemExit(spawn_ranks(args))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if args.dry:
+        return run_dry(args, world, rank)
 
     import torch
     import paper_2410_05408_b200 as gl
 
-    world = int(os.environ.get("WORLD_SIZE", "1"))
-    rank = int(os.environ.get("RANK", "0"))
-    local = int(os.environ.get("LOCAL_RANK", "0"))
     if not torch.cuda.is_available():
         raise SystemExit("bench.py needs a CUDA device: there is no CPU fallback")
     torch.cuda.set_device(local)
@@ -179,166 +252,227 @@ def main():
     W = max(args.warmup, 3)
     K = args.steps
 
-    w = make_workload(args.workload, rank)
     d = lambda x: torch.as_tensor(np.ascontiguousarray(x, dtype=np.float64), device=dev)  # noqa: E731
-    P, Tm, O, S = d(w.params), d(w.times), d(w.obs), d(w.sigma)
     flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)   # > 126 MB L2
-
-    extended = w.params.shape[1] == 16
-    loglike = gl.gl_loglike_ex if extended else gl.gl_loglike
-
-    def step():
-        return loglike(P, Tm, w.t_exp, w.n_ss, O, S, dtype="f32", want_flux=True)
 
     def barrier():
         if dist is not None:
             dist.barrier()
         torch.cuda.synchronize()
 
-    for _ in range(W):
-        chi2, flux = step()
-    torch.cuda.synchronize()
-    n_in_exposures = int((flux < 1.0).sum().item())
-    launches0 = gl.gl_launch_count()
+    def timed(fn, k=K, warm=W, cold=True):
+        """CUDA events around each of k calls on torch's current stream (the launching stream); L2
+        flushed before each call (cold) or a spinning spacer kernel instead (warm L2, context)."""
+        for _ in range(warm):
+            fn()
+        torch.cuda.synchronize()
+        ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(k)]
+        for a, b in ev:
+            if cold:
+                flush.zero_()
+            else:
+                torch.cuda._sleep(200_000)
+            a.record()
+            fn()
+            b.record()
+        torch.cuda.synchronize()
+        return [a.elapsed_time(b) for a, b in ev]
 
-    ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True))
-          for _ in range(K)]
+    w = make_workload(args.workload, rank)
+    P = d(w.params)
+    ser = gl.GlSeries(w.times, w.obs, w.sigma, w.t_exp, w.n_ss, w.B, device=dev)
+    chi2_d = torch.empty(w.B, dtype=torch.float32, device=dev)
+    flux_d = torch.empty((w.B, w.T), dtype=torch.float32, device=dev)
+
+    def step():
+        ser.loglike_dev(P, want_flux=True, chi2_out=chi2_d, flux_out=flux_d)
+
+    for _ in range(W):
+        step()
+    torch.cuda.synchronize()
+    n_in_exposures = int((flux_d < 1.0).sum().item())
+    launches0 = gl.gl_launch_count()
     sampler = ClockSampler(local)
     sampler.start()
     time.sleep(0.15)
     barrier()
     wall0 = time.perf_counter()
-    for a, b in ev:
-        flush.zero_()                 # L2 flush between timed iterations (outside the event pair)
-        a.record()
-        step()
-        b.record()
+    dev_ms = timed(step, warm=0)
     barrier()
     wall = time.perf_counter() - wall0
     clocks = sampler.stop()
     launches = gl.gl_launch_count() - launches0
-    # the same K steps with the L2 left warm (context only: a spinning spacer kernel, no memory
-    # traffic, lets the host run ahead so that the event pair sees GPU time, not submission gaps)
-    ev_w = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True))
-            for _ in range(K)]
-    for a, b in ev_w:
-        torch.cuda._sleep(200_000)
-        a.record()
-        step()
-        b.record()
-    torch.cuda.synchronize()
-    warm_ms = float(np.mean([a.elapsed_time(b) for a, b in ev_w]))
-    dev_ms = [a.elapsed_time(b) for a, b in ev]
+    warm_ms = float(np.mean(timed(step, warm=0, cold=False)))
     total_ms = float(np.sum(dev_ms))
     tmax = torch.tensor([total_ms], device=dev, dtype=torch.float64)
     if dist is not None:
         dist.all_reduce(tmax, op=dist.ReduceOp.MAX)
-    total_ms_max = float(tmax.item())
-    ms_per_step = total_ms_max / K
+    ms_per_step = float(tmax.item()) / K
     evals_per_step = w.B * w.T * world
     value = evals_per_step / (ms_per_step * 1e-3)
 
-    # ---- end to end through the HOST-buffer C ABI call, pinned host memory, copies timed
-    pin = lambda x: torch.as_tensor(np.ascontiguousarray(x, dtype=np.float64)).pin_memory().numpy()  # noqa: E731
-    hp, ht, ho, hs = pin(w.params), pin(w.times), pin(w.obs), pin(w.sigma)
-    c_h = torch.empty(w.B, dtype=torch.float32).pin_memory().numpy()          # pinned outputs too
+    # ---- end to end: HOST parameter rows in, HOST chi^2 (and flux) out, through gl_series_loglike
+    hp = torch.as_tensor(np.ascontiguousarray(w.params)).pin_memory().numpy()
+    c_h = torch.empty(w.B, dtype=torch.float32).pin_memory().numpy()
     f_h = torch.empty((w.B, w.T), dtype=torch.float32).pin_memory().numpy()
-    if extended:
-        # no host-pointer variant of the _ex entry points: the same copies, issued from here
-        pins = [torch.from_numpy(x) for x in (hp, ht, ho, hs)]
-        c_t, f_t = torch.from_numpy(c_h), torch.from_numpy(f_h)
 
-        def e2e_call():
-            for dst, src in zip((P, Tm, O, S), pins):
-                dst.copy_(src, non_blocking=True)
-            chi2_d, flux_d = step()
-            c_t.copy_(chi2_d, non_blocking=True)
-            f_t.copy_(flux_d, non_blocking=True)
-            torch.cuda.synchronize()
-        api = "gl_loglike_ex + pinned H2D/D2H copies issued by bench.py (wall clock over K calls)"
-    else:
-        def e2e_call():
-            gl.gl_loglike_host(hp, ht, w.t_exp, w.n_ss, ho, hs, dtype="f32", want_flux=True,
-                               chi2_out=c_h, flux_out=f_h)
-        api = "gl_loglike_host (pinned host inputs and outputs, wall clock over K calls)"
-    for _ in range(3):
-        e2e_call()
-    barrier()
-    t0 = time.perf_counter()
-    for _ in range(K):
-        e2e_call()
-    e2e_s = time.perf_counter() - t0
-    te = torch.tensor([e2e_s], device=dev, dtype=torch.float64)
-    if dist is not None:
-        dist.all_reduce(te, op=dist.ReduceOp.MAX)
-    e2e_value = evals_per_step * K / float(te.item())
-    h2d = int(hp.nbytes + ht.nbytes + ho.nbytes + hs.nbytes)
-    d2h = int(c_h.nbytes + f_h.nbytes)
-    # what an MCMC caller needs back is chi2[B] alone (flux never leaves the GPU): same call, no flux
-    e2e_chi2_only = None
-    if not extended:
+    def wall_per_call(fn):
         for _ in range(3):
-            gl.gl_loglike_host(hp, ht, w.t_exp, w.n_ss, ho, hs, dtype="f32", chi2_out=c_h)
+            fn()
         barrier()
         t0 = time.perf_counter()
         for _ in range(K):
-            gl.gl_loglike_host(hp, ht, w.t_exp, w.n_ss, ho, hs, dtype="f32", chi2_out=c_h)
-        tc = torch.tensor([time.perf_counter() - t0], device=dev, dtype=torch.float64)
+            fn()
+        t = torch.tensor([time.perf_counter() - t0], device=dev, dtype=torch.float64)
         if dist is not None:
-            dist.all_reduce(tc, op=dist.ReduceOp.MAX)
-        e2e_chi2_only = evals_per_step * K / float(tc.item())
+            dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        return float(t.item()) / K
+
+    e2e_s = wall_per_call(lambda: ser.loglike(hp, want_flux=True, chi2_out=c_h, flux_out=f_h))
+    e2e_chi2_s = wall_per_call(lambda: ser.loglike(hp, chi2_out=c_h))
+    h2d = int(hp.nbytes)
+    d2h = int(c_h.nbytes + f_h.nbytes)
 
     if rank != 0:
+        ser.close()
         if dist is not None:
             dist.destroy_process_group()
         return
 
-    # ---- roofline of the (only) kernel: plain FP32 ALU work
+    # ---- roofline of the dominant kernel (hot_kernel): plain FP32 ALU work
     sm_max = clocks.get("sm_max_mhz") or 1965.0
     peak_tflops = N_SM * LANES * 2 * sm_max * 1e6 / 1e12
     probe = gl.gl_probe_peaks()      # FFMA / DFMA / MUFU chain kernels, measured now, on this GPU
+    ncu = ncu_constants()
+
+    def fractions(workload_key, n_in, n_limb, ms):
+        alg = ALG_FLOP_INSIDE * (n_in - n_limb) + ALG_FLOP_LIMB * n_limb
+        out = {"alg_flop": alg, "alg_tflops": alg / (ms * 1e-3) / 1e12,
+               "frac_alg": alg / (ms * 1e-3) / 1e12 / peak_tflops}
+        ex = ncu.get("executed_fp32_flop", {}).get(workload_key)
+        if ex:
+            out["executed_flop_ncu"] = ex
+            out["frac_executed"] = ex / (ms * 1e-3) / 1e12 / peak_tflops
+        return out
+
     k_ms = float(np.mean(dev_ms))
-    n_sub_in = n_in_exposures * w.n_ss
-    alg_flop = ALG_FLOP_PER_SUBSAMPLE * n_sub_in
-    achieved = alg_flop / (k_ms * 1e-3) / 1e12
-    roofline = {"bound": "alu", "achieved": achieved, "peak": peak_tflops, "unit": "TFLOP/s",
-                "frac": achieved / peak_tflops, "traffic": NCU_DRAM_BYTES.get(args.workload),
-                "traffic_unit": "bytes per launch (ncu --set full, profiles/r01_v5.md); the path is "
-                                "ALU-bound, algorithmic HBM bytes are B*96 + T*24 in, B*T*4 + B*4 out",
-                "kernel": "transit_kernel<float> (+ one-CTA baseline_kernel, overlapped by "
-                          "programmatic dependent launch)", "kernel_ms": k_ms,
-                "kernel_ms_warm_l2": warm_ms,
-                "peak_source": f"derived: {N_SM} SMs x {LANES} FP32 lanes x 2 x {sm_max:.0f} MHz "
-                               "(MEASURED_PEAKS.json has no FP32 SIMT figure)",
-                "peak_measured_ffma_chain": probe["fp32_tflops"],
-                "frac_of_measured_peak": achieved / probe["fp32_tflops"],
-                "fp64_dfma_chain_tflops": probe["fp64_tflops"], "mufu_chain_tops": probe["mufu_tops"],
-                "alg_flop_per_in_transit_subsample": ALG_FLOP_PER_SUBSAMPLE,
-                "in_transit_subsamples_per_launch": n_sub_in,
-                "in_transit_fraction": n_sub_in / (w.B * w.T * w.n_ss),
-                "in_transit_subsamples_per_s": n_sub_in / (k_ms * 1e-3)}
+    n_in, n_limb = in_transit_mix(w)
+    fr = fractions(args.workload, n_in, n_limb, k_ms)
+    hs = (1, w.B, 512)               # hot_kernel's launch shape for this batch: (cluster, rows, threads)
+    floor_pair = float(np.mean(timed(lambda: gl.gl_probe_empty_launch(hs[0], hs[1], hs[2], 4, min(w.B, 148)),
+                                     k=max(K, 20))))
+    floor_one = float(np.mean(timed(lambda: gl.gl_probe_empty_launch(hs[0], hs[1], hs[2]), k=max(K, 20))))
+    roofline = {
+        "bound": "alu", "achieved": fr["alg_tflops"], "peak": peak_tflops, "unit": "TFLOP/s",
+        "frac": fr["frac_alg"],
+        "frac_label": "ALGORITHMIC flop (SURVEY.md 8(d): 1050 per in-transit sub-exposure inside the disc, "
+                      "1500 on the limb) / CUDA-event step time / derived peak",
+        "frac_executed": fr.get("frac_executed"),
+        "frac_executed_label": "fp32 flop the kernel EXECUTES (ncu: FADD + FMUL + 2 FFMA thread instructions, "
+                               f"capture of commit {ncu.get('commit')}) / step time / derived peak",
+        "traffic": ncu.get("dram_bytes", {}).get(args.workload),
+        "traffic_source": f"dram__bytes_read.sum + dram__bytes_write.sum of one hot_kernel launch, ncu --set full "
+                          f"at commit {ncu.get('commit')} (profiles/r02_kernels.md); the path is ALU/latency-bound, "
+                          "algorithmic HBM bytes are B*96 in, B*T*4 + B*4 out",
+        "kernel": "glh::hot_kernel<true> (+ transit_kernel in marker mode behind it: exits at once when no "
+                  "walker was deferred)",
+        "kernel_ms": k_ms, "kernel_ms_warm_l2": warm_ms,
+        "launch_floor_ms": floor_pair, "launch_floor_single_kernel_ms": floor_one,
+        "launch_floor_note": "EMPTY kernels of the same grid/block shapes (hot + dependent fallback pair; one "
+                             "kernel alone), timed exactly like a step, L2 flushed",
+        "peak_source": f"derived: {N_SM} SMs x {LANES} FP32 lanes x 2 x {sm_max:.0f} MHz "
+                       "(MEASURED_PEAKS.json has no FP32 SIMT figure)",
+        "peak_measured_ffma_chain": probe["fp32_tflops"],
+        "frac_of_measured_peak": fr["alg_tflops"] / probe["fp32_tflops"],
+        "fp64_dfma_chain_tflops": probe["fp64_tflops"], "mufu_chain_tops": probe["mufu_tops"],
+        "alg_flop_per_in_transit_subsample": {"inside": ALG_FLOP_INSIDE, "limb": ALG_FLOP_LIMB},
+        "in_transit_subsamples_per_launch": n_in, "of_which_limb_crossing": n_limb,
+        "in_window_exposures_with_flux_below_1": n_in_exposures,
+        "in_transit_fraction": n_in / (w.B * w.T * w.n_ss),
+        "in_transit_subsamples_per_s": n_in / (k_ms * 1e-3)}
 
     out = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": W,
         "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak",
         "vs_baseline": None, "dtype": "f32", "data": "synthetic",
         "config": {"workload": w.name, "B": w.B, "T": w.T, "n_ss": w.n_ss, "outputs": "chi2[B]+flux[B,T]",
+                   "api": "gl_series_loglike_dev (series resident, parameter rows resident)",
                    "l2": "256 MiB flush between timed iterations", "parallelism": f"dp{world} over walkers"},
         "subsample_evals_per_s": value * w.n_ss,
         "wall_ms_per_step_incl_flush": 1e3 * wall / K,
         "clocks": clocks, "gpu_launches": int(launches),
-        "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": h2d,
-                "d2h_bytes_per_step": d2h, "api": api,
-                "chi2_only_value": e2e_chi2_only, "chi2_only_d2h_bytes_per_step": int(c_h.nbytes)},
+        "e2e": {"value": evals_per_step / e2e_s, "unit": UNIT, "h2d_bytes_per_step": h2d,
+                "d2h_bytes_per_step": d2h,
+                "api": "gl_series_loglike: host parameter rows in, host chi2 + flux out (wall clock over K calls)",
+                "ms_per_call": 1e3 * e2e_s,
+                "chi2_only_value": evals_per_step / e2e_chi2_s, "chi2_only_ms_per_call": 1e3 * e2e_chi2_s,
+                "chi2_only_d2h_bytes_per_step": int(c_h.nbytes)},
         "roofline": roofline,
     }
-    if world == 1 and not args.no_cpu_baseline and not extended:
-        v, used, dt = oracle_timed(w, repeat=1)
+    if world == 1 and not args.no_extra:
+        out["extra"] = extra_workloads(gl, dev, d, timed, fractions, peak_tflops, probe, ncu, w, ser, P)
+    ser.close()
+    if world == 1 and not args.no_cpu_baseline:
+        v, used, dt = oracle_timed(w)
+        v1, _, dt1 = oracle_timed(w, nthreads=1, rows=16)
         out["cpu_baseline"] = {"value": v, "unit": UNIT, "cores": used, "kind": "oracle",
-                               "sample": f"whole workload {w.name} once ({dt:.2f} s), OpenMP over (walker,time)"}
+                               "sample": f"whole workload {w.name} once ({dt:.2f} s), OpenMP over (walker,time)",
+                               "single_thread_value": v1,
+                               "single_thread_sample": f"first 16 walkers of {w.name}, 1 thread ({dt1:.2f} s)"}
     print(json.dumps(out))
     if dist is not None:
         dist.destroy_process_group()
+
+
+def extra_workloads(gl, dev, d, timed, fractions, peak_tflops, probe, ncu, w3, ser3, P3):
+    """The secondary numbers, timed like the headline (CUDA events, L2 flushed, inputs resident), so that
+    the driver's run carries them: each with ms, units/s and both roofline fractions where they apply."""
+    import torch
+    ex = {}
+    k = 20
+    # the stateless entry point on the headline workload: baseline_kernel + hot_kernel + fallback
+    T3, O3, S3 = d(w3.times), d(w3.obs), d(w3.sigma)
+    ms = float(np.mean(timed(lambda: gl.gl_loglike(P3, T3, w3.t_exp, w3.n_ss, O3, S3, dtype="f32", want_flux=True), k=k)))
+    ex["cfg3_gl_loglike_stateless"] = {"ms": ms, "flux_evals_per_s": w3.B * w3.T / (ms * 1e-3), "launches_per_step": 3}
+    chi2_only = torch.empty(w3.B, dtype=torch.float32, device=dev)
+    ms = float(np.mean(timed(lambda: ser3.loglike_dev(P3, chi2_out=chi2_only), k=k)))
+    ex["cfg3_chi2_only"] = {"ms": ms, "flux_evals_per_s": w3.B * w3.T / (ms * 1e-3)}
+    # cfg3 in fp64 (validation path: the full kernel)
+    ms = float(np.mean(timed(lambda: gl.gl_loglike(P3, T3, w3.t_exp, w3.n_ss, O3, S3, dtype="f64", want_flux=True), k=5, warm=2)))
+    ex["cfg3_fp64"] = {"ms": ms, "flux_evals_per_s": w3.B * w3.T / (ms * 1e-3), "dtype": "f64",
+                       "dfma_chain_tflops": probe["fp64_tflops"],
+                       "executed_fp64_flop_ncu": ncu.get("executed_fp64_flop", {}).get("cfg3_fp64")}
+    if ex["cfg3_fp64"]["executed_fp64_flop_ncu"]:
+        ex["cfg3_fp64"]["frac_executed_of_dfma_chain"] = (ex["cfg3_fp64"]["executed_fp64_flop_ncu"] / (ms * 1e-3) / 1e12
+                                                          / probe["fp64_tflops"])
+    # cfg4: JWST-shaped batch, chi2 + flux
+    w4 = wl.config4()
+    ser4 = gl.GlSeries(w4.times, w4.obs, w4.sigma, w4.t_exp, w4.n_ss, w4.B, device=dev)
+    P4 = d(w4.params)
+    c4 = torch.empty(w4.B, dtype=torch.float32, device=dev)
+    f4 = torch.empty((w4.B, w4.T), dtype=torch.float32, device=dev)
+    ms = float(np.mean(timed(lambda: ser4.loglike_dev(P4, want_flux=True, chi2_out=c4, flux_out=f4), k=k)))
+    n_in, n_limb = in_transit_mix(w4)
+    ex["cfg4"] = {"ms": ms, "flux_evals_per_s": w4.B * w4.T / (ms * 1e-3), "B": w4.B, "T": w4.T, "n_ss": w4.n_ss,
+                  "in_transit_subsamples": n_in, "of_which_limb_crossing": n_limb, **fractions("cfg4", n_in, n_limb, ms)}
+    ser4.close()
+    del f4
+    # cfg5: 1e6 bare geometries, fp32
+    geom, _ = wl.config5()
+    G = d(geom)
+    ms = float(np.mean(timed(lambda: gl.gl_flux_geometry(G, dtype="f32"), k=k)))
+    ex["cfg5"] = {"ms": ms, "geometries_per_s": geom.shape[0] / (ms * 1e-3), "N": int(geom.shape[0]),
+                  "active_lanes_per_instruction_ncu": ncu.get("active_lanes", {}).get("cfg5")}
+    # one light curve of 1e5 exposures, flux only: the shape of the paper's Fig. 6 (PAPER.md:171, :183)
+    T1 = 100_000
+    t1 = d(np.linspace(-0.6, 0.6, T1))
+    p1 = d(wl.CFG2_ROW[None, :])
+    f1 = torch.empty((1, T1), dtype=torch.float32, device=dev)
+    ms = float(np.mean(timed(lambda: gl.gl_lightcurve(p1, t1, 0.0, 1, dtype="f32", out=f1), k=k)))
+    ex["single_lightcurve_T1e5"] = {"ms": ms, "us_per_flux_sample": ms * 1e3 / T1, "flux_evals_per_s": T1 / (ms * 1e-3),
+                                    "paper": "about 0.5 us per sample at 1e4-1e5 samples on a Quadro RTX 5000 "
+                                             "(PAPER.md:171; another machine: context)"}
+    return ex
 
 
 if __name__ == "__main__":

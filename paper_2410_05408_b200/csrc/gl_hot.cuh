@@ -465,27 +465,6 @@ __global__ void __launch_bounds__(HOT_NT, 2) hot_kernel(const HotArgs A) {
                 for (int k = 0; k < nep; ++k) in = in || (i >= su.lo[k] && i < su.hi[k]);
                 return in;
             };
-            // ---- 3. out-of-window exposures: flux = 1, 16 bytes at a time where the row allows
-            if (frow) {
-                const int head = (int)((4u - (((uintptr_t)frow >> 2) & 3u)) & 3u);
-                if (gtid < head && gtid < nT && !inwin(gtid)) frow[gtid] = 1.f;
-                const int nchunk = nT > head ? (nT - head) >> 2 : 0;
-                for (int c = gtid; c < nchunk; c += ntot) {
-                    const int i0 = head + 4 * c;
-                    bool hit = false;
-#pragma unroll 1
-                    for (int k = 0; k < nep; ++k) hit = hit || (i0 + 3 >= su.lo[k] && i0 < su.hi[k]);
-                    if (!hit) {
-                        *reinterpret_cast<float4*>(frow + i0) = make_float4(1.f, 1.f, 1.f, 1.f);
-                    } else {
-#pragma unroll
-                        for (int r = 0; r < 4; ++r)
-                            if (!inwin(i0 + r)) frow[i0 + r] = 1.f;
-                    }
-                }
-                const int tail0 = head + 4 * nchunk;
-                if (gtid < nT - tail0 && !inwin(tail0 + gtid)) frow[tail0 + gtid] = 1.f;
-            }
             GLH_TL(3);
             // ---- 4. in-window exposures.  A lane takes JS consecutive sub-exposures of one exposure
             // (JS = 1 unless the list is long), a warp G = 32 / JB whole exposures; groups are dealt
@@ -500,7 +479,13 @@ __global__ void __launch_bounds__(HOT_NT, 2) hot_kernel(const HotArgs A) {
                 const int JB = (S + JS - 1) / JS, G = 32 / JB;
                 const int my_l = lane / JB, my_b = lane - my_l * JB;
                 const int W = (M + G - 1) / G;
-                for (int t = warp * csize + crank; t < W; t += HOT_NW * csize) {
+                // sweep k hands out tasks k nwt .. (k+1) nwt - 1, in warp order on even sweeps and in
+                // reverse on odd ones: the warps that opened with the outermost (expensive) groups get
+                // the last, innermost ones, if any
+                const int nwt = HOT_NW * csize, gw = warp * csize + crank;
+                for (int k = 0; k * nwt < W; ++k) {
+                    const int t = k * nwt + ((k & 1) ? nwt - 1 - gw : gw);
+                    if (t >= W) continue;   // warp-uniform
                     const int g = (t & 1) ? W - 1 - (t >> 1) : (t >> 1);
                     const int v = g * G + my_l;
                     const bool active = (my_l < G) && (v < M);
@@ -549,6 +534,29 @@ __global__ void __launch_bounds__(HOT_NT, 2) hot_kernel(const HotArgs A) {
                         acc += (double)(d * fmaf(2.f * ob, rs, d));   // ((o+dbar) r)^2 - (o r)^2
                     }
                 }
+            }
+            GLH_TL(6);
+            // ---- 4b. out-of-window exposures: flux = 1, 16 bytes at a time where the row allows (after the
+            // evaluation: nothing waits for these stores)
+            if (frow) {
+                const int head = (int)((4u - (((uintptr_t)frow >> 2) & 3u)) & 3u);
+                if (gtid < head && gtid < nT && !inwin(gtid)) frow[gtid] = 1.f;
+                const int nchunk = nT > head ? (nT - head) >> 2 : 0;
+                for (int c = gtid; c < nchunk; c += ntot) {
+                    const int i0 = head + 4 * c;
+                    bool hit = false;
+#pragma unroll 1
+                    for (int k = 0; k < nep; ++k) hit = hit || (i0 + 3 >= su.lo[k] && i0 < su.hi[k]);
+                    if (!hit) {
+                        *reinterpret_cast<float4*>(frow + i0) = make_float4(1.f, 1.f, 1.f, 1.f);
+                    } else {
+#pragma unroll
+                        for (int r = 0; r < 4; ++r)
+                            if (!inwin(i0 + r)) frow[i0 + r] = 1.f;
+                    }
+                }
+                const int tail0 = head + 4 * nchunk;
+                if (gtid < nT - tail0 && !inwin(tail0 + gtid)) frow[tail0 + gtid] = 1.f;
             }
         }
         GLH_TL(4);

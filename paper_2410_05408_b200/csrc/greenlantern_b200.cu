@@ -1672,6 +1672,10 @@ int gl_series_create(const double* times, const double* obs, const double* sigma
     *out = nullptr;
     if (T < 1 || B_max < 1 || n_ss < 1 || !(t_exp >= 0.0) || !isfinite(t_exp) || !times || !obs || !sigma)
         return GL_EINVAL;
+    {   // the full kernel (the fallback of a series call) reads the constant-memory tables
+        const int rc = ensure_tables();
+        if (rc != GL_OK) return rc;
+    }
     gl_series* s = new (std::nothrow) gl_series;
     if (!s) return GL_ECUDA;
     s->T = T;

@@ -656,8 +656,13 @@ def test_hot_and_deferred_walkers_in_one_batch(gl):
     assert bad.sum() == 5 and np.all(np.isnan(out[bad])) and np.all(np.isinf(chi[bad]))
     assert np.abs(out[~bad] - ref[~bad]).max() <= 5e-7
     assert np.abs(chi[~bad] / chi_ref[~bad] - 1.0).max() <= 1e-4
+    # gl_lightcurve cuts the series into segments, so a walker with many transit epochs may be on
+    # the hot kernel there and on the full kernel here: equal to rounding, not bit for bit; walkers
+    # that are on the hot kernel both times (rows 0, 6, 7 mod 8) are bit-identical
     lc = host(gl.gl_lightcurve(dev(p), dev(w.times), w.t_exp, w.n_ss, dtype="f32"))
-    assert np.array_equal(lc, out, equal_nan=True)
+    assert np.abs(lc[~bad] - out[~bad]).max() <= 2e-7 and np.all(np.isnan(lc[bad]))
+    same = np.r_[0:40:8, 6:40:8, 7:40:8]
+    assert np.array_equal(lc[same], out[same])
     chi_only = host(gl.gl_loglike(dev(p), dev(w.times), w.t_exp, w.n_ss, dev(w.obs), dev(w.sigma),
                                   dtype="f32"))
     assert np.array_equal(chi_only, chi)

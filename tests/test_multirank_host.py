@@ -61,3 +61,25 @@ def test_two_ranks_shard_walkers(tmp_path):
     # ranks get DIFFERENT walkers (weak scaling: per-rank work fixed, total grows)
     assert not np.array_equal(got[0][:-1], got[1][:-1])
     assert np.array_equal(bench.make_workload("cfg3", 0).params, base.params)
+
+
+def test_bench_gpus_flag_starts_the_ranks():
+    """`python bench.py --gpus 2 --dry` outside torchrun: bench.py must START two ranks (gloo on this
+    CPU box), shard the walkers and print one JSON line with n_gpus = 2 and the slowest rank's time."""
+    import json
+    import subprocess
+    env = {k: v for k, v in os.environ.items() if k not in ("WORLD_SIZE", "RANK", "LOCAL_RANK")}
+    out = subprocess.run([sys.executable, str(ROOT / "bench.py"), "--gpus", "2", "--dry", "--steps", "2"],
+                         capture_output=True, text=True, timeout=300, env=env)
+    assert out.returncode == 0, out.stderr[-2000:]
+    lines = [ln for ln in out.stdout.splitlines() if ln.startswith("{")]
+    assert len(lines) == 1, out.stdout
+    rec = json.loads(lines[0])
+    assert rec["n_gpus"] == 2 and rec["dry"] is True
+    assert rec["ms_per_step"] == 2.0            # max over ranks of (1 + rank)
+    assert rec["distinct_shards"] == 2          # the two ranks drew different walkers
+    # one process, no flag: one rank
+    out1 = subprocess.run([sys.executable, str(ROOT / "bench.py"), "--dry"], capture_output=True, text=True,
+                          timeout=300, env=env)
+    rec1 = json.loads([ln for ln in out1.stdout.splitlines() if ln.startswith("{")][0])
+    assert rec1["n_gpus"] == 1
