@@ -1,30 +1,36 @@
 // gl_hot.cuh -- hot_kernel: the COMMON path of the fused fp32 transit kernel and nothing else
 // (DESIGN.md 5.4).  A walker is "simple" when its orbit is circular (eqs. 9-10 as
-// printed), n_ss <= 32, its transit window is short (|phi| <= 0.8 rad), at most MAXEP transits fall
-// inside the series, the star centre can never lie inside the outline's evolute while the outline
-// is near the limb (so the outline crosses the limb at most twice), and the series is sorted.
-// Simple walkers are finished here; every other walker is DEFERRED: the kernel leaves a marker (a
-// NaN with a payload) in the walker's output slot and the full-featured transit_kernel, launched
-// right behind with programmatic dependent launch, redoes exactly the marked walkers.  Invalid
-// walkers (NaN row, chi^2 = +inf) are finished here too.
+// printed), its transit window is short (|phi| <= 0.8 rad), at most MAXEP transits fall inside the
+// series, the star centre can never lie inside the outline's evolute while the outline is near the
+// limb (so the outline crosses the limb at most twice), and the series is sorted.  Simple walkers are
+// finished here; every other walker is DEFERRED: the kernel leaves a marker (a NaN with a payload) in
+// the walker's output slot and the full-featured transit_kernel, launched right behind with
+// programmatic dependent launch, redoes exactly the marked walkers.  Invalid walkers (NaN row,
+// chi^2 = +inf) are finished here too.
 //
 // Why a separate kernel: the full-featured kernel is ~340 KB of SASS (fp64 Kepler, the
 // four-crossing search, libm slow paths); on a K2-shaped batch (config 3) it spent its time in
 // instruction fetch and barriers, not arithmetic (profiles/r01_v5.md).  This one has no fp64
-// arithmetic beyond the time difference t_i - t_c and the chi^2 sum, no libm call, no list, and
-// one CTA (or one cluster, for long in-window ranges) per walker:
+// arithmetic beyond the epoch bookkeeping of the prelude, the time difference t_i - t_c and the
+// chi^2 sum, no libm call, no scan of the series, and one CTA (or one cluster, for long in-window
+// ranges) per walker:
 //   1. at entry every thread loads one COARSE sample of the series (every stride-th time) into
 //      shared memory and, unless the caller vouches for the order, checks its share of adjacent
-//      pairs; three threads of three warps run the walker prelude (orbit+window / outline / limb
-//      darkening) side by side;
+//      pairs; FOUR threads of four warps run the walker prelude side by side (validity + window
+//      angle / outline / limb darkening / period);
 //   2. for a sorted series the in-window exposures of transit epoch n are ONE index range
-//      [lo_n, hi_n): a warp per epoch finds it by binary search in the coarse table + one round of
-//      global loads -- no scan of the series, no ballots, no compaction, no list;
+//      [lo_n, hi_n): one warp per range end finds it by two 32-way steps in the coarse table + one
+//      round of global loads -- no scan of the series, no ballots over it, no list;
 //   3. out-of-window flux = 1 is plain 16-byte stores;
-//   4. lane = (exposure, sub-exposure): position from dt = (float)(t_i - t_c) (the fp64 phase
-//      reduction is gone: the epoch is known from the range), a3 + a4 by blocked_hot(), exposure
-//      mean by shuffles, chi^2 term in the cancellation-free form d (2 o r + d), d = dbar/sigma;
-//   5. chi^2 = S + sum of the terms, S = sum_i ((obs_i-1)/sigma_i)^2 once per series.
+//   4. SPARSE list (a K2-shaped series: all (exposure, sub-exposure) pairs of the walker fit one
+//      pass of the CTA): lane = pair, in time order, so neighbouring lanes run the same code path;
+//      pairs whose outline is near the limb (the long path: critical points, two crossings, 16-point
+//      rule) are compacted into a list and evaluated by TWO lanes each (far/near critical point,
+//      first/second crossing, even/odd quadrature nodes in parallel); exposure means through shared
+//      memory.  DENSE list (a JWST-shaped series): a thread takes whole exposures, all
+//      sub-exposures in turn, with the same arithmetic in the same order (bit-identical values);
+//   5. chi^2 = S + sum of d (2 o r + d), d = dbar/sigma (cancellation-free form of
+//      ((o + dbar)/sigma)^2 - (o/sigma)^2), S = sum_i ((obs_i-1)/sigma_i)^2 once per series.
 #pragma once
 #include <cooperative_groups.h>
 #include <cuda_runtime.h>
@@ -46,6 +52,7 @@ constexpr int HOT_NT = 512;           // threads per CTA
 constexpr int HOT_NW = HOT_NT / 32;
 constexpr int MAXEP = 8;              // transit epochs of one walker inside one series segment
 constexpr int MAXC = 8;               // CTAs per cluster (portable limit)
+constexpr int CAP = 2 * HOT_NT;       // (exposure, sub-exposure) pairs of the sparse mode
 constexpr uint32_t MARK_BITS = 0x7fc0deadu;   // "deferred": a quiet NaN no arithmetic here produces
 
 // cos, sin of pi k / 16, k = 0..15 (glf::whole_outline_lin's table), statically initialised.
@@ -134,59 +141,181 @@ __device__ __forceinline__ float asin_small(float x) {
     return fmaf(x * x2, q, x);
 }
 
-// Blocked fraction delta = k0 A_flat + k1 A_lin + k2 A_quad (R8; eqs. 21-23) for an
-// outline that crosses the limb AT MOST TWICE (the caller has excluded the evolute regime for the
-// whole walker): glf::blocked_f32 (gl_fast32.cuh) without its generic branch, with
-// the Gauss-Legendre table as immediates.  trap = shared-memory copy of c_trap16.
-__device__ __forceinline__ float blocked_hot(const glf::TrapNode* trap, float xc_in, float yc_in, float a,
-                                             float b, float ab, float e2, float k0, float k1, float k2) {
-    using namespace glf;
-    const float xc = fabsf(xc_in), yc = fabsf(yc_in);   // mirror images have the same areas
-    const float r0sq = fmaf(xc, xc, yc * yc);
+// ------------------------------------------------------------------------------------------
+// Steps a3 + a4 for an outline that crosses the limb AT MOST TWICE (the caller has
+// excluded the evolute regime for the whole walker): the arithmetic of glf::blocked_f32 without its
+// generic branch, cut into the pieces the kernel schedules separately.
+//   path_of       which rule the pair takes (0 = no overlap; 1, 2, 3 = 6 / 8 / 16 fixed nodes, outline
+//                 wholly inside and >= 0.01 from the limb; 4 = near the limb)
+//   cheap_delta   paths 1-3
+//   near_delta    path 4, by one lane (TWO = false) or by two lanes that share it (TWO = true);
+//                 both give the same bits: the one-lane version does the two lanes' parts in turn
+//                 and adds them in the same order.
+// delta = k0 A_flat + k1 A_lin + k2 A_quad (R8; eqs. 21-23).
+// ------------------------------------------------------------------------------------------
+__device__ __forceinline__ int path_of(float r0sq, float a, float* r0_out) {
     const float reach = 1.f + a;
-    if (r0sq >= reach * reach) return 0.f;
+    const float r0 = r0sq * glf::mufu_rsqrt(fmaxf(r0sq, 1e-30f));
+    *r0_out = r0;
+    if (r0sq >= reach * reach) return 0;
+    if (!(r0 + a <= 0.99f)) return 4;
+    if (fmaf(4.f, a, r0) <= 1.f || r0 + a <= 0.5f) return 1;
+    return (r0 + a + a <= 1.f || r0 + a <= 0.7f) ? 2 : 3;
+}
+
+// Part of the trapezoid sum of W(r^2) (2 f_flat) over the whole outline (glf::whole_outline_lin): the
+// blocks of four node pairs number first, first + step, ... of the nh/4 blocks; NOT yet scaled by pi/nh.
+__device__ __forceinline__ float outline_lin_part(const glf::TrapNode* trap, int nh, int first, int step,
+                                                  float xc, float yc, float a, float b, float ab, float u,
+                                                  float v) {
+    const int stride = 16 / nh;
+    float acc = 0.f;
+    for (int blk = first; blk * 4 < nh; blk += step) {
+#pragma unroll
+        for (int kk = 0; kk < 4; ++kk) {
+            const glf::TrapNode nd = trap[(blk * 4 + kk) * stride];
+            const float p = a * nd.c, q = b * nd.s;
+            const float xp = xc + p, yp = yc + q, xq = xc - p, yq = yc - q;
+            const float m2p = fmaf(-xp, xp, fmaf(-yp, yp, 1.f));
+            const float m2q = fmaf(-xq, xq, fmaf(-yq, yq, 1.f));
+            const float w = fmaf(u, nd.c, v * nd.s);
+            acc += glf::pair_term<true>(m2p, ab + w, m2q, ab - w);
+        }
+    }
+    return acc;
+}
+
+// Outline wholly inside the disc: A_flat = pi a b, A_quad = pi a b (r0^2 + (a^2 + b^2)/4) in closed
+// form, `lin` = the trapezoid sum of the f_lin weight, scaled.
+__device__ __forceinline__ float inside_delta(float lin, float a, float b, float ab, float r0sq, float k0,
+                                              float k1, float k2) {
+    const float in_flat = glf::kPiF * ab;
+    const float in_quad = in_flat * fmaf(0.25f, fmaf(a, a, b * b), r0sq);
+    return fmaf(k0, in_flat, fmaf(k1 * (1.f / 3.f), lin, k2 * in_quad));
+}
+
+// xc, yc >= 0 (already folded).  path = 1, 2 or 3.
+__device__ __forceinline__ float cheap_delta(const glf::TrapNode* trap, int path, float xc, float yc,
+                                             float r0sq, float a, float b, float ab, float k0, float k1,
+                                             float k2) {
     const float u = b * xc, v = a * yc;
-    const float r0 = r0sq * mufu_rsqrt(fmaxf(r0sq, 1e-30f));
-    int nh = 0;
-    float cf = 1.f, sf = 0.f, gfar = 0.f;
-    if (r0 + a <= 0.99f) {
-        nh = (r0 + a + a <= 1.f || r0 + a <= 0.7f) ? 4 : 8;
-        if (fmaf(4.f, a, r0) <= 1.f || r0 + a <= 0.5f) nh = 3;
+    float lin;
+    if (path == 1) {
+        lin = glf::whole_outline_lin6(xc, yc, a, b, ab, u, v);
     } else {
-        const float Aa = a * xc, Bb = b * yc;
-        const float rn = mufu_rsqrt(fmaf(Aa, Aa, Bb * Bb));
-        cf = Aa * rn;
-        sf = Bb * rn;
-        critical_point<1>(xc, yc, a, b, &cf, &sf, 1.f, 1.f);
-        const float xf = fmaf(a, cf, xc), yf = fmaf(b, sf, yc);
-        gfar = fmaf(xf, xf, fmaf(yf, yf, -1.f));
-        if (gfar <= 0.f) nh = (gfar < -0.04f) ? 8 : 16;
+        const int nh = path == 2 ? 4 : 8;
+        lin = outline_lin_part(trap, nh, 0, 1, xc, yc, a, b, ab, u, v) * (glf::kPiF / float(nh));
     }
-    if (nh) {
-        const float in_flat = kPiF * ab;
-        const float in_quad = in_flat * fmaf(0.25f, fmaf(a, a, b * b), r0sq);
-        const float lin = (nh == 3) ? whole_outline_lin6(xc, yc, a, b, ab, u, v)
-                                    : whole_outline_lin(trap, nh, xc, yc, a, b, ab, u, v);
-        return fmaf(k0, in_flat, fmaf(k1 * (1.f / 3.f), lin, k2 * in_quad));
+    return inside_delta(lin, a, b, ab, r0sq, k0, k1, k2);
+}
+
+// glf::critical_point with the sign as an argument (sgn = +1: the maximum of g in the first quadrant,
+// -1: the minimum in the third), so that two lanes can run the two searches in one instruction stream.
+__device__ __forceinline__ void critical_point_rt(float xc, float yc, float a, float b, float sgn, float* c,
+                                                  float* s) {
+    for (int it = 0; it < 12; ++it) {
+        const float x = fmaf(a, *c, xc), y = fmaf(b, *s, yc);
+        const float bc = b * *c, as = a * *s;
+        const float h = bc * y - as * x;
+        const float hp = fmaf(bc, bc, as * as) - fmaf(b * *s, y, a * *c * x);
+        float d = (sgn * hp < 0.f) ? -glf::fast_div(h, hp) : copysignf(0.5f, sgn * h);
+        d = fminf(fmaxf(d, -0.5f), 0.5f);
+        const float d2 = d * d;
+        const float sd = d * fmaf(d2, fmaf(d2, 1.f / 120.f, -1.f / 6.f), 1.f);
+        const float cd = fmaf(d2, fmaf(d2, fmaf(d2, -1.f / 720.f, 1.f / 24.f), -0.5f), 1.f);
+        float cn = *c * cd - *s * sd, sn = *s * cd + *c * sd;
+        cn = sgn * fmaxf(sgn * cn, 0.f);
+        sn = sgn * fmaxf(sgn * sn, 0.f);
+        const float rn = glf::mufu_rsqrt(fmaf(cn, cn, sn * sn));
+        *c = cn * rn;
+        *s = sn * rn;
+        if (fabsf(d) < 1e-3f) break;
     }
+}
+
+// Path 4.  xc, yc >= 0.  TWO: lanes `lane` and `lane ^ 1` of the warp hold the SAME pair; h = lane & 1
+// says which half this lane does (mask = the lanes that are in here together: whole lane pairs).
+template <bool TWO>
+__device__ __forceinline__ float near_delta(const glf::TrapNode* trap, float xc, float yc, float r0sq, float a,
+                                            float b, float ab, float e2, float k0, float k1, float k2, int h,
+                                            unsigned mask) {
+    using namespace glf;
+    const float u = b * xc, v = a * yc;
+    // ---- critical points of g = x^2 + y^2 - 1 on the outline: the farthest point from the star centre
+    // (first quadrant) and the nearest (third quadrant), both started from the direction (a xc, b yc)
+    const float Aa = a * xc, Bb = b * yc;
+    const float rn = mufu_rsqrt(fmaf(Aa, Aa, Bb * Bb));   // (r0 > 0.49 here: not both zero)
+    const float c0 = Aa * rn, s0 = Bb * rn;
+    float cf, sf, cn, sn;
+    if (TWO) {
+        const float sg = h ? -1.f : 1.f;
+        float c = sg * c0, s = sg * s0;
+        critical_point_rt(xc, yc, a, b, sg, &c, &s);
+        const float co = __shfl_xor_sync(mask, c, 1), so = __shfl_xor_sync(mask, s, 1);
+        cf = h ? co : c;
+        sf = h ? so : s;
+        cn = h ? c : co;
+        sn = h ? s : so;
+    } else {
+        cf = c0;
+        sf = s0;
+        critical_point_rt(xc, yc, a, b, 1.f, &cf, &sf);
+        cn = -c0;
+        sn = -s0;
+    }
+    const float xf = fmaf(a, cf, xc), yf = fmaf(b, sf, yc);
+    const float gfar = fmaf(xf, xf, fmaf(yf, yf, -1.f));
+    if (gfar <= 0.f) {
+        // wholly inside, close to the limb: 16 nodes, 32 within 0.02 of it; the two halves of the
+        // node blocks are summed separately (lane 0 / lane 1) and added
+        const int nh = (gfar < -0.04f) ? 8 : 16;
+        float p0, p1;
+        if (TWO) {
+            const float mine = outline_lin_part(trap, nh, h, 2, xc, yc, a, b, ab, u, v);
+            const float other = __shfl_xor_sync(mask, mine, 1);
+            p0 = h ? other : mine;
+            p1 = h ? mine : other;
+        } else {
+            p0 = outline_lin_part(trap, nh, 0, 2, xc, yc, a, b, ab, u, v);
+            p1 = outline_lin_part(trap, nh, 1, 2, xc, yc, a, b, ab, u, v);
+        }
+        return inside_delta((p0 + p1) * (kPiF / float(nh)), a, b, ab, r0sq, k0, k1, k2);
+    }
+    // ---- the outline crosses the limb twice (or misses the disc).  tau = t - t_far in [0, 2 pi).
     Arc o = {xc, yc, a, b, cf, sf};
     float tsplit = kPiF;
-    const float xo = fmaf(-a, cf, xc), yo = fmaf(-b, sf, yc);
+    const float xo = fmaf(-a, cf, xc), yo = fmaf(-b, sf, yc);   // the point opposite t_far
     float gsplit = fmaf(xo, xo, fmaf(yo, yo, -1.f));
     if (gsplit >= 0.f) {
-        float cn = -cf, sn = -sf;
-        critical_point<-1>(xc, yc, a, b, &cn, &sn, -1.f, -1.f);
+        // mostly outside: the nearest outline point and its tau
+        if (!TWO) critical_point_rt(xc, yc, a, b, -1.f, &cn, &sn);
         const float xn = fmaf(a, cn, xc), yn = fmaf(b, sn, yc);
         gsplit = fmaf(xn, xn, fmaf(yn, yn, -1.f));
         if (gsplit >= 0.f) return 0.f;
         const float dtau = atan2_fast(cf * sn - sf * cn, cf * cn + sf * sn);
         tsplit = dtau < 0.f ? dtau + kTwoPiF : dtau;
     }
+    // half-cosine model of g between its maximum and the split point (exact for a circle)
     const float mid = 0.5f * (gfar + gsplit), amp = 0.5f * (gfar - gsplit);
     const float uu = rough_acos(fminf(fmaxf(-fast_div(mid, amp), -1.f), 1.f)) * (1.f / kPiF);
-    float s1, c1, s2, c2;
-    const float t1 = crossing(o, 0.f, tsplit, uu * tsplit, false, &s1, &c1);
-    const float t2 = crossing(o, tsplit, kTwoPiF, kTwoPiF - uu * (kTwoPiF - tsplit), true, &s2, &c2);
+    float t1, s1, c1, t2, s2, c2;
+    if (TWO) {
+        float s, c;   // ONE call, the lane's half chosen by its arguments: the two lanes stay in step
+        const float t = crossing(o, h ? tsplit : 0.f, h ? kTwoPiF : tsplit,
+                                 h ? kTwoPiF - uu * (kTwoPiF - tsplit) : uu * tsplit, h != 0, &s, &c);
+        const float to = __shfl_xor_sync(mask, t, 1), so = __shfl_xor_sync(mask, s, 1),
+                    co = __shfl_xor_sync(mask, c, 1);
+        t1 = h ? to : t;
+        s1 = h ? so : s;
+        c1 = h ? co : c;
+        t2 = h ? t : to;
+        s2 = h ? s : so;
+        c2 = h ? c : co;
+    } else {
+        t1 = crossing(o, 0.f, tsplit, uu * tsplit, false, &s1, &c1);
+        t2 = crossing(o, tsplit, kTwoPiF, kTwoPiF - uu * (kTwoPiF - tsplit), true, &s2, &c2);
+    }
+    // ---- outline arc [t1, t2] (inside the disc): flat and quad in closed form
     glc::Outline<float> oo = {xc, yc, a, b, e2};
     const glc::ArcCoef<float> k = glc::arc_coefficients(oo);
     const float dt = t2 - t1;
@@ -195,14 +324,14 @@ __device__ __forceinline__ float blocked_hot(const glf::TrapNode* trap, float xc
     glc::arc_primitive(k, s2, c2, &f2, &q2);
     float Aflat = 0.5f * fmaf(k.ab, dt, f2 - f1);
     float Aquad = 0.25f * fmaf(k.k0, dt, q2 - q1);
+    // ---- f_lin: 16-point Gauss-Legendre in z, t = tm + hw (3z - z^3)/2; even node pairs (lane 0) and
+    // odd ones (lane 1) summed separately, then added
     const float hw = 0.5f * dt;
     float sm, cm;
     abs_trig(o, t1 + hw, &sm, &cm);
     constexpr float gl_phi[8] = GLH_GL_PHI, gl_om[8] = GLH_GL_OM;
-    float acc = 0.f;
-#pragma unroll
-    for (int i = 0; i < 8; ++i) {
-        const float dd = hw * gl_phi[i];   // in [0, pi]
+    auto node = [&](float phi, float om, float acc) {
+        const float dd = hw * phi;   // in [0, pi]
         const float sd = mufu_sin(dd), cd = mufu_cos(dd);
         const float cp = cm * cd - sm * sd, sp = sm * cd + cm * sd;
         const float cq = cm * cd + sm * sd, sq = sm * cd - cm * sd;
@@ -211,9 +340,23 @@ __device__ __forceinline__ float blocked_hot(const glf::TrapNode* trap, float xc
         const float m2p = fmaf(-xp, xp, fmaf(-yp, yp, 1.f));
         const float m2q = fmaf(-xq, xq, fmaf(-yq, yq, 1.f));
         const float fp = fmaf(u, cp, fmaf(v, sp, ab)), fq = fmaf(u, cq, fmaf(v, sq, ab));
-        acc = fmaf(gl_om[i], pair_term<true>(m2p, fp, m2q, fq), acc);
+        return fmaf(om, pair_term<true>(m2p, fp, m2q, fq), acc);
+    };
+    float part[2] = {0.f, 0.f};
+    if (TWO) {
+        float mine = 0.f;
+#pragma unroll
+        for (int ii = 0; ii < 4; ++ii)   // node pair 2 ii + h: the two lanes differ in constants only
+            mine = node(h ? gl_phi[2 * ii + 1] : gl_phi[2 * ii], h ? gl_om[2 * ii + 1] : gl_om[2 * ii], mine);
+        const float other = __shfl_xor_sync(mask, mine, 1);
+        part[0] = h ? other : mine;
+        part[1] = h ? mine : other;
+    } else {
+#pragma unroll
+        for (int i = 0; i < 8; ++i) part[i & 1] = node(gl_phi[i], gl_om[i], part[i & 1]);
     }
-    float Alin = (1.f / 3.f) * hw * acc;
+    float Alin = (1.f / 3.f) * hw * (part[0] + part[1]);
+    // ---- limb arc from the exit point (t2) counter-clockwise back to the entry point (t1)
     const float xa = fmaf(a, c2, xc), ya = fmaf(b, s2, yc);
     const float xb = fmaf(a, c1, xc), yb = fmaf(b, s1, yc);
     const float dl = atan2_fast(xa * yb - ya * xb, xa * xb + ya * yb);
@@ -221,6 +364,18 @@ __device__ __forceinline__ float blocked_hot(const glf::TrapNode* trap, float xc
     Alin = fmaf(1.f / 3.f, dl, Alin);
     Aquad = fmaf(0.25f, dl, Aquad);
     return fmaf(k0, Aflat, fmaf(k1, Alin, k2 * Aquad));
+}
+
+// One lane, any path: the dense mode's per-sub-exposure call.  xc_in, yc_in of any sign.
+__device__ __forceinline__ float blocked_hot(const glf::TrapNode* trap, float xc_in, float yc_in, float a,
+                                             float b, float ab, float e2, float k0, float k1, float k2) {
+    const float xc = fabsf(xc_in), yc = fabsf(yc_in);   // mirror images have the same areas
+    const float r0sq = fmaf(xc, xc, yc * yc);
+    float r0;
+    const int path = path_of(r0sq, a, &r0);
+    if (path == 0) return 0.f;
+    if (path < 4) return cheap_delta(trap, path, xc, yc, r0sq, a, b, ab, k0, k1, k2);
+    return near_delta<false>(trap, xc, yc, r0sq, a, b, ab, e2, k0, k1, k2, 0, 0xffffffffu);
 }
 
 // ------------------------------------------------------------------------------------------
@@ -240,6 +395,7 @@ struct HotArgs {
     double S;               // PRE: baseline sum_i ((obs_i - 1)/sigma_i)^2
     double t_exp;
     float inv_ss, doff, off0;   // 1/n_ss, t_exp/n_ss, (0.5/n_ss - 0.5) t_exp: sub-exposure j sits at off0 + j doff (R18)
+    unsigned ss_magic;      // ceil(2^32 / n_ss): pair / n_ss = umulhi(pair, ss_magic) for pair < 2^16 (n_ss > 1)
     int B, T, n_ss, nseg, seglen;   // B * nseg < 2^31
     int sorted_known;       // the caller vouches that times is non-decreasing (gl_series checked it)
 };
@@ -247,89 +403,46 @@ struct HotArgs {
 enum { CLS_SIMPLE = 0, CLS_INVALID = 1, CLS_DEFER = 2 };
 
 struct Unit {
-    double tc[MAXEP];             // conjunction time of each listed transit epoch
-    double qlo[MAXEP], qhi[MAXEP];   // its window [qlo, qhi) in time
-    int lo[MAXEP], hi[MAXEP];     // ... and in index (relative to the segment)
-    int nep;
-    int cls_orbit, defer_shape;
+    // written by the four prelude threads
+    double t0, P, x1, x2, hx;     // x1, x2 = (t_first - t0)/P, (t_last - t0)/P; hx = t_exp/(2P) + 1e-9
+    float phimax;                 // half-angle of the window [rad], widened
     float w, aR, bimp, a, b, cpsi, spsi, k0, k1, k2;
+    int cls_win, defer_shape, bad_ld, bad_period, never;
+    // written by the search warps
+    double tc[MAXEP];             // conjunction time of each transit epoch that touches the segment
+    int lo[MAXEP], hi[MAXEP];     // its in-window index range [lo, hi) (relative to the segment)
 };
 
-// Orbit half of the prelude (one thread): validity, window, transit epochs inside [tfirst, tlast].
-// e != 0 (or NaN) is deferred without looking further: the full kernel owns those rules.
-__device__ __forceinline__ void hot_prelude_orbit(const double* p, double t_exp, int n_ss,
-                                                  double tfirst, double tlast, Unit* u) {
-    const double t0 = p[0], P = p[1], aR = p[2], b = p[3], e = p[4];
-    const double Rp = p[6], f = p[7], u1 = p[10], u2 = p[11];
-    u->nep = 0;
-    if (!(e == 0.0) || n_ss > 32) {
-        u->cls_orbit = CLS_DEFER;
-        return;
-    }
-    bool ok = true;
-#pragma unroll
-    for (int k = 0; k < 12; ++k) ok = ok && (fabs(p[k]) <= 1.79769313486231570e308);   // finite
-    ok = ok && (P > 0.0) && (Rp > 0.0) && (Rp < 0.5) && (f >= 0.0) && (f < 1.0) && (aR > 1.0) &&
-         (1.0 - u1 / 3.0 - u2 / 6.0 > 0.0) && (fabs(b) <= aR);
-    if (!ok) {
-        u->cls_orbit = CLS_INVALID;
-        return;
-    }
-    // PAPER.md:85-87 eqs. 9-10: the centre is within `reach` of the star centre iff
-    // sin^2(phi) < [(reach/aR)^2 - cos^2 i] / sin^2 i (and cos(phi) > 0)
+// Prelude, thread 1 of 4: validity (the limb-darkening norm is checked by hot_prelude_ld) and the
+// half-angle of the transit window.  fin = every entry of the row is finite (voted by the warp).
+// PAPER.md:85-87 eqs. 9-10: the centre is within `reach` of the star centre iff
+// sin^2(phi) < [(reach/aR)^2 - cos^2 i] / sin^2 i (and cos(phi) > 0).
+// e != 0 (or NaN) is deferred whatever else the row holds: the full kernel owns those rules.
+__device__ __forceinline__ void hot_prelude_window(const double* p, bool fin, Unit* u) {
+    const double P = p[1], aR = p[2], b = p[3], e = p[4], Rp = p[6], f = p[7];
+    const bool ok = fin & (P > 0.0) & (Rp > 0.0) & (Rp < 0.5) & (f >= 0.0) & (f < 1.0) & (aR > 1.0) &
+                    (fabs(b) <= aR);
     const float aRf = (float)aR, bf = (float)b;
     const float iaR = rcp_nr(aRf);
     const float cosi = bf * iaR, ci2 = cosi * cosi;
     const float reach = (1.f + (float)Rp) * (1.f + 1e-5f);
     const float q = reach * iaR;
     const float S2 = glf::fast_div(q * q - ci2, 1.f - ci2);
-    // 1/P in fp64 by Newton from the MUFU reciprocal (P must be in fp32's range for that)
-    if (!(P > 1e-30 && P < 1e30)) {
-        u->cls_orbit = CLS_DEFER;
-        return;
-    }
-    double inv_P = (double)glf::mufu_rcp((float)P);
-    inv_P = inv_P * fma(-P, inv_P, 2.0);
-    inv_P = inv_P * fma(-P, inv_P, 2.0);
-    const float w = (float)(6.28318530717958647692 * inv_P);
-    u->w = w;
+    u->phimax = asin_small(glf::mufu_sqrt(fminf(fmaxf(S2, 0.f), 0.25f)) * (1.f + 1e-6f)) * (1.f + 1e-5f);
     u->aR = aRf;
     u->bimp = bf;
-    u->cls_orbit = CLS_SIMPLE;
-    if (S2 <= 0.f) return;   // never transits: nep = 0, flux = 1 everywhere
-    if (!(S2 <= 0.25f)) {    // long window (or NaN: face-on orbit): not the common path
-        u->cls_orbit = CLS_DEFER;
-        return;
-    }
-    const float phimax = asin_small(glf::mufu_sqrt(S2) * (1.f + 1e-6f)) * (1.f + 1e-5f);
-    if (!(phimax + w * (float)t_exp <= 0.8f)) {   // small_sincos's range
-        u->cls_orbit = CLS_DEFER;
-        return;
-    }
-    const double hw = (double)phimax * P * 0.15915494309189535 + 0.5 * t_exp + 1e-9 * P;
-    const double nlo = ceil((tfirst - hw - t0) * inv_P - 1e-9);
-    const double nhi = floor((tlast + hw - t0) * inv_P + 1e-9);
-    const double cnt = nhi - nlo + 1.0;
-    if (!(cnt <= (double)MAXEP)) {   // also NaN / infinite time stamps
-        u->cls_orbit = CLS_DEFER;
-        return;
-    }
-    const int nep = cnt > 0.0 ? (int)cnt : 0;
-    for (int k = 0; k < nep; ++k) {
-        const double tc = fma(nlo + (double)k, P, t0);
-        u->tc[k] = tc;
-        u->qlo[k] = tc - hw;
-        u->qhi[k] = tc + hw;
-    }
-    u->nep = nep;
+    const bool never = (S2 <= 0.f);   // no transit at all
+    u->never = never;
+    // S2 > 1/4 is a long window (a NaN S2 -- face-on orbit grazing the reach -- fails both tests): deferred
+    u->cls_win = !(e == 0.0) ? CLS_DEFER : (!ok ? CLS_INVALID : ((never | (S2 <= 0.25f)) ? CLS_SIMPLE : CLS_DEFER));
 }
 
-// Outline half (one thread): the oblate spheroid's projected outline in closed form -- semi-major
-// axis Rp along (sin xi, cos xi), semi-minor Rp sqrt(1 - f(2-f) cos^2 eta) (eqs. 6, 11-13 with
-// a = Rp(1-f), b = c = Rp, zeta = 0: SURVEY.md 8(c) "equation checks"; tests compare with the
-// general eigen-axes of the full kernel) -- and the evolute exclusion: a second pair of critical
-// points of g needs a xc < e2 and b yc < e2 (gl_core.cuh), i.e. r0 < e2 sqrt(1/a^2 + 1/b^2); if
-// that is below 0.99 - a, blocked_hot's near-limb branch (r0 + a > 0.99) can never see one.
+// Thread 2 of 4: the oblate spheroid's projected outline in closed form -- semi-major axis Rp along
+// (sin xi, cos xi), semi-minor Rp sqrt(1 - f(2-f) cos^2 eta) (eqs. 6, 11-13 with a = Rp(1-f),
+// b = c = Rp, zeta = 0: SURVEY.md 8(c) "equation checks"; the parity tests compare with the general
+// eigen-axes of the full kernel) -- and the evolute exclusion: a second pair of critical points of g
+// needs a xc < e2 and b yc < e2 (gl_core.cuh), i.e. r0 < e2 sqrt(1/a^2 + 1/b^2); if that is below
+// 0.99 - a, the near-limb path (r0 + a > 0.99) can never see one.
 __device__ __forceinline__ void hot_prelude_shape(const double* p, Unit* u) {
     const float Rp = (float)p[6], f = (float)p[7];
     float sx, cx, se, ce;
@@ -347,33 +460,53 @@ __device__ __forceinline__ void hot_prelude_shape(const double* p, Unit* u) {
     u->defer_shape = !(rmax <= (0.99f - a) * 0.98f);   // NaN (b = 0) defers too
 }
 
+// Thread 3 of 4: c0, c1, c2 of R8 over pi (1 - u1/3 - u2/6), and that norm's sign.
 __device__ __forceinline__ void hot_prelude_ld(const double* p, Unit* u) {
     const double u1 = p[10], u2 = p[11];
-    const float pn = (float)(3.14159265358979323846 * (1.0 - u1 / 3.0 - u2 / 6.0));
-    const float ipn = rcp_nr(pn);
+    const double norm = 1.0 - u1 / 3.0 - u2 / 6.0;
+    const float ipn = rcp_nr((float)(3.14159265358979323846 * norm));
     u->k0 = (float)(1.0 - u1 - 2.0 * u2) * ipn;
     u->k1 = (float)(u1 + 2.0 * u2) * ipn;
     u->k2 = (float)u2 * ipn;
+    u->bad_ld = !(norm > 0.0);
 }
 
-// #{i in [0, n) : seg[i] < q} for a non-decreasing segment, by the 16 lanes of a half-warp (all 32
-// lanes of the warp call this; `hl` = lane & 15).  coarse[k] = seg[k stride], k < nc.
-__device__ __forceinline__ int lower_bound_half(const double* __restrict__ seg, int n,
-                                                const double* coarse, int nc, int stride, double q,
-                                                int hl) {
-    int lo = 0, hi = nc;
-    while (lo < hi) {   // identical in every lane
-        const int mid = (lo + hi) >> 1;
-        if (coarse[mid] < q) lo = mid + 1; else hi = mid;
-    }
-    // (no early exit: the two halves of the warp meet again at the shuffles below)
-    const bool none = (lo == 0);
-    const int base = none ? 0 : (lo - 1) * stride, end = none ? 0 : min(lo * stride, n);
+// Thread 4 of 4: 1/P in fp64 by Newton from the MUFU reciprocal (P must be in fp32's range for that),
+// the angular velocity, and the segment's ends in units of the period.
+__device__ __forceinline__ void hot_prelude_period(const double* p, double t_exp, double tfirst, double tlast,
+                                                   Unit* u) {
+    const double t0 = p[0], P = p[1];
+    double inv_P = (double)glf::mufu_rcp((float)P);
+    inv_P = inv_P * fma(-P, inv_P, 2.0);
+    inv_P = inv_P * fma(-P, inv_P, 2.0);
+    u->t0 = t0;
+    u->P = P;
+    u->w = (float)(6.28318530717958647692 * inv_P);
+    u->x1 = (tfirst - t0) * inv_P;
+    u->x2 = (tlast - t0) * inv_P;
+    u->hx = 0.5 * t_exp * inv_P + 1e-9;
+    u->bad_period = !((P > 1e-30) & (P < 1e30));
+}
+
+// #{i in [0, n) : seg[i] < q} for a non-decreasing segment, by ONE WARP (every lane calls this with
+// the same arguments and gets the same answer).  coarse[k] = seg[k stride] for k stride < n, +inf
+// beyond, HOT_NT = 512 entries: two 32-way steps (16 entries apart, then 1 apart) find how many
+// coarse samples lie below q, one round of global loads (stride - 1 candidates) does the rest.  On a
+// segment that is NOT sorted the answer is meaningless but still in [0, n].
+__device__ __forceinline__ int lower_bound_warp(const double* __restrict__ seg, int n, const double* coarse,
+                                                int stride, double q, int lane) {
+    const int j1 = __popc(__ballot_sync(0xffffffffu, coarse[lane * 16] < q));
+    if (j1 == 0) return 0;   // warp-uniform
+    const int blk = (j1 - 1) * 16;
+    const int j2 = __popc(__ballot_sync(0xffffffffu, lane < 16 && coarse[blk + (lane & 15)] < q));
+    const int lo = blk + max(j2, 1);                  // coarse samples below q (>= 1)
+    const int base = (lo - 1) * stride, end = min(lo * stride, n);
     int cnt = 0;
-    for (int m = base + 1 + hl; m < end; m += 16) cnt += (seg[m] < q) ? 1 : 0;
-#pragma unroll
-    for (int off = 8; off > 0; off >>= 1) cnt += __shfl_xor_sync(0xffffffffu, cnt, off);
-    return none ? 0 : base + 1 + cnt;
+    for (int m0 = base + 1; m0 < end; m0 += 32) {      // warp-uniform trip count
+        const int m = m0 + lane;
+        cnt += __popc(__ballot_sync(0xffffffffu, m < end && seg[m] < q));
+    }
+    return min(base + 1 + cnt, n);
 }
 
 template <bool PRE>
@@ -384,11 +517,17 @@ __global__ void __launch_bounds__(HOT_NT, 2) hot_kernel(const HotArgs A) {
     cg::cluster_group cluster = cg::this_cluster();
 
     __shared__ Unit su;
-    __shared__ double s_coarse[HOT_NT];
+    __shared__ double s_row[4][12];
+    __shared__ double s_coarse[HOT_NT];    // every stride-th time of the segment (+inf beyond its end)
     __shared__ double s_red[HOT_NW];
     __shared__ double s_gather[2][MAXC];   // rank 0's copy collects the cluster's chi^2 partials
-    __shared__ int s_gflag[2][MAXC];       // ... and their "my share of the series is unsorted" flags
-    __shared__ double s_row[3][12];
+    __shared__ int s_gflag[2][MAXC];       // ... and their "my share of the series is out of order" flags
+    __shared__ int s_cnt[2][HOT_NW];       // near-limb pairs per (pair slot, warp)
+    __shared__ float s_px[CAP], s_py[CAP]; // sparse mode: folded kernel-frame centre of a near-limb pair
+    __shared__ float s_d[CAP];             // ... blocked fraction of every pair
+    __shared__ unsigned short s_np[CAP];   // ... the near-limb pairs, in pair order
+    __shared__ int s_li[CAP];              // ... index in the segment of in-window exposure e
+    __shared__ float2 s_ow[CAP];           // ... its (obs - 1, 1/sigma)
     __shared__ glf::TrapNode s_trap[16];
     if (tid < 16) s_trap[tid] = glf::TrapNode{c_trap16[tid].x, c_trap16[tid].y};
 
@@ -396,6 +535,7 @@ __global__ void __launch_bounds__(HOT_NT, 2) hot_kernel(const HotArgs A) {
     const float inv_ss = A.inv_ss, doff = A.doff, off0 = A.off0;
     const bool want_chi2 = A.chi2 != nullptr, want_flux = A.flux != nullptr;
     const int ntot = csize * HOT_NT, gtid = crank * HOT_NT + tid;
+    const unsigned lt_mask = (1u << lane) - 1u;
     int wpar = 0;
     // no CTA may write into rank 0's shared memory before rank 0 runs: arrive now, wait before the
     // first push
@@ -408,141 +548,131 @@ __global__ void __launch_bounds__(HOT_NT, 2) hot_kernel(const HotArgs A) {
         const int t_lo = (int)(un - (unsigned)wk * (unsigned)A.nseg) * A.seglen;
         const double* __restrict__ seg = A.times + t_lo;
         const int nT = min(A.seglen, A.T - t_lo);
-        const int stride = (nT + HOT_NT - 1) / HOT_NT;
-        const int nc = (nT + stride - 1) / stride;
         const double* __restrict__ p = A.params + (size_t)wk * 12;
         float* frow = want_flux ? A.flux + (size_t)wk * A.T + t_lo : nullptr;
+        const int stride = (nT + HOT_NT - 1) / HOT_NT;   // coarse table: every stride-th time
 
         __syncthreads();   // the previous unit's shared data is dead
         GLH_TL(0);
-        // ---- 1. coarse samples, order check (this CTA's share of the adjacent pairs, incl. the pair
-        // that straddles into the next segment), prelude
-        if (tid < nc) s_coarse[tid] = seg[(size_t)tid * stride];
+        // ---- 1. coarse samples of the series; order check (this CTA's share of the adjacent pairs,
+        // incl. the pair that straddles into the next segment) unless the caller vouches for the order;
+        // prelude on four threads of four warps.  The parameter row is ONE coalesced 96-byte request
+        // per prelude warp (it may sit in host memory read over PCIe: gl_series_loglike).
+        {
+            const long long ci = (long long)tid * stride;
+            s_coarse[tid] = ci < nT ? seg[ci] : __longlong_as_double(0x7ff0000000000000LL);
+        }
         int unsorted = 0;
         if (!A.sorted_known) {
             const int npairs = min(nT, A.T - t_lo - 1);
             for (int i = gtid; i < npairs; i += ntot) unsorted |= !(seg[i] <= seg[i + 1]);
         }
-        // the parameter row: ONE coalesced 96-byte request per prelude warp (it may sit in host memory
-        // that the device reads over PCIe: gl_series_loglike), handed to lane 0 through shared memory
-        if (warp < 3) {
-            if (lane < 12) s_row[warp][lane] = p[lane];
+        if (warp < 4) {
+            const double v = lane < 12 ? p[lane] : 0.0;
+            if (lane < 12) s_row[warp][lane] = v;
+            const bool fin = __all_sync(0xffffffffu, fabs(v) <= 1.79769313486231570e308);
             __syncwarp();
-            if (tid == 0) hot_prelude_orbit(s_row[0], A.t_exp, S, seg[0], seg[nT - 1], &su);
+            if (tid == 0) hot_prelude_window(s_row[0], fin, &su);
             if (tid == 32) hot_prelude_shape(s_row[1], &su);
             if (tid == 64) hot_prelude_ld(s_row[2], &su);
+            if (tid == 96) hot_prelude_period(s_row[3], A.t_exp, seg[0], seg[nT - 1], &su);
         }
         unsorted = __syncthreads_or(unsorted);
         GLH_TL(1);
+        // every thread: the transit epochs n whose window [t0 + n P - hw, t0 + n P + hw) can touch the
+        // segment (hw = half-width of the window in time, hwp in units of the period), and the verdict
+        const double P = su.P, t0 = su.t0;
+        const double hwp = (double)su.phimax * 0.15915494309189535 + su.hx;
+        const double nlo = ceil(su.x1 - hwp - 1e-9);
+        const double cnt = floor(su.x2 + hwp + 1e-9) - nlo + 1.0;
+        const bool few = (cnt <= (double)MAXEP);   // false for NaN / infinite time stamps too
+        int cls = su.cls_win;
+        if (cls != CLS_DEFER && su.bad_ld) cls = CLS_INVALID;
+        if (cls == CLS_SIMPLE && !su.never &&
+            (su.bad_period || su.defer_shape || !few || !(su.phimax + su.w * (float)A.t_exp <= 0.8f)))
+            cls = CLS_DEFER;   // (0.8 rad: small_sincos's range)
+        if (cls == CLS_SIMPLE && unsorted && csize == 1) cls = CLS_DEFER;   // (clusters: decided at the end)
+        const int nep = (cls == CLS_SIMPLE && !su.never && cnt > 0.0) ? (int)cnt : 0;
 
-        int cls = su.cls_orbit;
-        if (cls == CLS_SIMPLE && su.defer_shape) cls = CLS_DEFER;
-        const int nep = (cls == CLS_SIMPLE) ? su.nep : 0;
-
-        // ---- 2. index range of every listed epoch: warp = epoch, half-warp = end of the window
-        if (warp < nep) {
-            const int half = lane >> 4;
-            const double q = half ? su.qhi[warp] : su.qlo[warp];
-            const int idx = lower_bound_half(seg, nT, s_coarse, nc, stride, q, lane & 15);
-            if ((lane & 15) == 0) (half ? su.hi : su.lo)[warp] = idx;
+        // ---- 2. for a sorted series the in-window exposures of an epoch are ONE index range: warp
+        // 2 k finds where epoch k's window starts, warp 2 k + 1 where it ends
+        if (warp < 2 * nep) {
+            const double tc = fma(nlo + (double)(warp >> 1), P, t0);
+            const double q = (warp & 1) ? tc + hwp * P : tc - hwp * P;
+            const int idx = lower_bound_warp(seg, nT, s_coarse, stride, q, lane);
+            if (lane == 0) {
+                if (warp & 1) {
+                    su.hi[warp >> 1] = idx;
+                } else {
+                    su.lo[warp >> 1] = idx;
+                    su.tc[warp >> 1] = tc;
+                }
+            }
         }
         __syncthreads();
         GLH_TL(2);
 
-        double acc = 0.0;   // this lane's chi^2 terms
+        double acc = 0.0;   // this thread's chi^2 terms
         if (cls == CLS_INVALID) {
             if (frow)
                 for (int i = gtid; i < nT; i += ntot) frow[i] = __int_as_float(0x7fc00000);
         } else if (cls == CLS_SIMPLE) {
-            // index ranges are read from shared memory where they are needed (broadcast reads; nep is 1
+            const float w = su.w, aR = su.aR, bimp = su.bimp, a = su.a, b = su.b;
+            const float cpsi = su.cpsi, spsi = su.spsi, k0 = su.k0, k1 = su.k1, k2 = su.k2;
+            const float ab = a * b, e2 = (a - b) * (a + b);
+            // the ranges are read from shared memory where they are needed (broadcast reads; nep is 1
             // for a single-transit series): len_k = max(hi_k - lo_k, 0) -- an unsorted share of the
             // series may give anything, the unit is then redone by the fallback kernel
-            int M = 0;
+            int M = 0;   // in-window exposures of the unit (the whole cluster's)
             for (int k = 0; k < nep; ++k) M += max(su.hi[k] - su.lo[k], 0);
-            auto inwin = [&](int i) {
-                bool in = false;
+            // v-th in-window exposure of the unit -> its index in the segment and its time from the
+            // centre of its transit, (float)(t - t_c): the fp64 phase reduction is gone
+            auto entry = [&](int v, int* idx) {
+                int n = 0, run = 0, i = su.lo[0] + v;
 #pragma unroll 1
-                for (int k = 0; k < nep; ++k) in = in || (i >= su.lo[k] && i < su.hi[k]);
-                return in;
-            };
-            GLH_TL(3);
-            // ---- 4. in-window exposures.  A lane takes JS consecutive sub-exposures of one exposure
-            // (JS = 1 unless the list is long), a warp G = 32 / JB whole exposures; groups are dealt
-            // from both ends of the list inwards, so that ingress and egress -- the long code path --
-            // start first and sit in warps of their own.
-            if (M > 0) {
-                const float w = su.w, aR = su.aR, bimp = su.bimp, a = su.a, b = su.b;
-                const float cpsi = su.cpsi, spsi = su.spsi, k0 = su.k0, k1 = su.k1, k2 = su.k2;
-                const float ab = a * b, e2 = (a - b) * (a + b);
-                const long long pairs = (long long)M * S;
-                const int JS = (int)min((long long)S, max(1LL, pairs / (4LL * ntot)));
-                const int JB = (S + JS - 1) / JS, G = 32 / JB;
-                const int my_l = lane / JB, my_b = lane - my_l * JB;
-                const int W = (M + G - 1) / G;
-                // sweep k hands out tasks k nwt .. (k+1) nwt - 1, in warp order on even sweeps and in
-                // reverse on odd ones: the warps that opened with the outermost (expensive) groups get
-                // the last, innermost ones, if any
-                const int nwt = HOT_NW * csize, gw = warp * csize + crank;
-                for (int k = 0; k * nwt < W; ++k) {
-                    const int t = k * nwt + ((k & 1) ? nwt - 1 - gw : gw);
-                    if (t >= W) continue;   // warp-uniform
-                    const int g = (t & 1) ? W - 1 - (t >> 1) : (t >> 1);
-                    const int v = g * G + my_l;
-                    const bool active = (my_l < G) && (v < M);
-                    int i = 0;
-                    float delta = 0.f, ob = 0.f, rs = 0.f;
-                    if (active) {
-                        int n = 0, run = 0;
-                        i = su.lo[0] + v;
-#pragma unroll 1
-                        for (int k = 0; k < nep; ++k) {   // which epoch's range holds list entry v
-                            if (v >= run) {
-                                n = k;
-                                i = su.lo[k] + (v - run);
-                            }
-                            run += max(su.hi[k] - su.lo[k], 0);
-                        }
-                        const float dtc = (float)(seg[i] - su.tc[n]);
-                        if (want_chi2 && my_b == 0) {
-                            if (PRE) {
-                                const float2 o2 = A.ow[t_lo + i];
-                                ob = o2.x;
-                                rs = o2.y;
-                            } else {
-                                ob = (float)(A.obs[t_lo + i] - 1.0);
-                                const float sf = (float)A.sigma[t_lo + i];
-                                rs = glf::mufu_rcp(sf);
-                                rs = rs * fmaf(-sf, rs, 2.f);
-                            }
-                        }
-                        const int j1 = min(S, (my_b + 1) * JS);
-                        for (int j = my_b * JS; j < j1; ++j) {
-                            const float phi = w * (dtc + fmaf((float)j, doff, off0));
-                            float s, c;
-                            small_sincos(phi, &s, &c);
-                            const float x0 = bimp * c, y0 = aR * s;   // eqs. 9-10, d sin(beta) = b
-                            delta += blocked_hot(s_trap, fmaf(cpsi, x0, spsi * y0), fmaf(cpsi, y0, -spsi * x0),
-                                                 a, b, ab, e2, k0, k1, k2);
-                        }
-                    }
-                    float sum = 0.f;   // exposure mean, blocks in sub-exposure order (R18)
-                    for (int bb = 0; bb < JB; ++bb) sum += __shfl_sync(0xffffffffu, delta, (lane + bb) & 31);
-                    if (active && my_b == 0) {
-                        const float dbar = sum * inv_ss;
-                        if (frow) frow[i] = 1.f - dbar;
-                        const float d = dbar * rs;
-                        acc += (double)(d * fmaf(2.f * ob, rs, d));   // ((o+dbar) r)^2 - (o r)^2
+                for (int k = 1; k < nep; ++k) {
+                    run += max(su.hi[k - 1] - su.lo[k - 1], 0);
+                    if (v >= run) {
+                        n = k;
+                        i = su.lo[k] + (v - run);
                     }
                 }
-            }
-            GLH_TL(6);
-            // ---- 4b. out-of-window exposures: flux = 1, 16 bytes at a time where the row allows (after the
-            // evaluation: nothing waits for these stores)
-            if (frow) {
+                *idx = i;
+                return (float)(seg[i] - su.tc[n]);
+            };
+            // folded kernel-frame position of sub-exposure j of an exposure (eqs. 9-10
+            // with d sin(beta) = b; phi = 2 pi dt / P, |phi| <= 0.8)
+            auto position = [&](float dtc, int j, float* xc, float* yc) {
+                float s, c;
+                small_sincos(w * (dtc + fmaf((float)j, doff, off0)), &s, &c);
+                const float x0 = bimp * c, y0 = aR * s;
+                *xc = fabsf(fmaf(cpsi, x0, spsi * y0));
+                *yc = fabsf(fmaf(cpsi, y0, -spsi * x0));
+            };
+            auto obs_of = [&](int i) {   // (obs - 1, 1/sigma) of exposure i in fp32
+                if (PRE) return A.ow[t_lo + i];
+                const float sf = (float)A.sigma[t_lo + i];
+                float rs = glf::mufu_rcp(sf);
+                rs = rs * fmaf(-sf, rs, 2.f);
+                return make_float2((float)(A.obs[t_lo + i] - 1.0), rs);
+            };
+            auto finish = [&](int i, float dbar, float2 o2) {   // exposure i is done: flux, chi^2 term
+                if (frow) frow[i] = 1.f - dbar;
+                const float d = dbar * o2.y;
+                acc += (double)(d * fmaf(2.f * o2.x, o2.y, d));   // ((o + dbar) r)^2 - (o r)^2
+            };
+            // out-of-window exposures: flux = 1, 16 bytes at a time where the row allows; thread ft of nft
+            auto fill = [&](int ft, int nft) {
+                auto inwin = [&](int i) {
+                    bool in = false;
+#pragma unroll 1
+                    for (int k = 0; k < nep; ++k) in = in || (i >= su.lo[k] && i < su.hi[k]);
+                    return in;
+                };
                 const int head = (int)((4u - (((uintptr_t)frow >> 2) & 3u)) & 3u);
-                if (gtid < head && gtid < nT && !inwin(gtid)) frow[gtid] = 1.f;
+                if (ft < head && ft < nT && !inwin(ft)) frow[ft] = 1.f;
                 const int nchunk = nT > head ? (nT - head) >> 2 : 0;
-                for (int c = gtid; c < nchunk; c += ntot) {
+                for (int c = ft; c < nchunk; c += nft) {
                     const int i0 = head + 4 * c;
                     bool hit = false;
 #pragma unroll 1
@@ -550,19 +680,119 @@ __global__ void __launch_bounds__(HOT_NT, 2) hot_kernel(const HotArgs A) {
                     if (!hit) {
                         *reinterpret_cast<float4*>(frow + i0) = make_float4(1.f, 1.f, 1.f, 1.f);
                     } else {
-#pragma unroll
+#pragma unroll 1
                         for (int r = 0; r < 4; ++r)
                             if (!inwin(i0 + r)) frow[i0 + r] = 1.f;
                     }
                 }
                 const int tail0 = head + 4 * nchunk;
-                if (gtid < nT - tail0 && !inwin(tail0 + gtid)) frow[tail0 + gtid] = 1.f;
+                if (ft < nT - tail0 && !inwin(tail0 + ft)) frow[tail0 + ft] = 1.f;
+            };
+            const long long pairs = (long long)M * S;
+            if (csize == 1 && pairs <= CAP) {
+                // ---- 3a. SPARSE list: lane = (exposure, sub-exposure) pair, in time order.  Pairs on the
+                // short paths (outline wholly inside the disc, away from the limb) are finished at once;
+                // the near-limb ones are listed (deterministic order: pair slot, warp, lane).
+                const int np = (int)pairs;
+                int rank0 = -1, rank1 = -1;
+#pragma unroll
+                for (int sl = 0; sl < 2; ++sl) {   // (unrolled: the two slots' loads and chains overlap)
+                    const int pr = tid + sl * HOT_NT;
+                    bool near = false;
+                    if (pr < np) {
+                        const int e = S == 1 ? pr : (int)__umulhi((unsigned)pr, A.ss_magic);
+                        const int j = pr - e * S;
+                        int i;
+                        const float dtc = entry(e, &i);
+                        if (j == 0) {
+                            s_li[e] = i;
+                            if (want_chi2) s_ow[e] = obs_of(i);
+                        }
+                        float xc, yc, r0;
+                        position(dtc, j, &xc, &yc);
+                        const float r0sq = fmaf(xc, xc, yc * yc);
+                        const int path = path_of(r0sq, a, &r0);
+                        near = (path == 4);
+                        if (near) {
+                            s_px[pr] = xc;
+                            s_py[pr] = yc;
+                        } else {
+                            s_d[pr] = path == 0 ? 0.f : cheap_delta(s_trap, path, xc, yc, r0sq, a, b, ab, k0, k1, k2);
+                        }
+                    }
+                    const unsigned bal = __ballot_sync(0xffffffffu, near);
+                    if (lane == 0) s_cnt[sl][warp] = __popc(bal);
+                    const int rk = near ? __popc(bal & lt_mask) : -1;
+                    if (sl == 0) rank0 = rk; else rank1 = rk;
+                }
+                __syncthreads();
+                // position of (slot, warp) in the list: scan of the 32 counts by every warp for itself
+                int L;
+                {
+                    const int c = s_cnt[lane >> 4][lane & 15];
+                    int incl = c;
+#pragma unroll
+                    for (int off = 1; off < 32; off <<= 1) {
+                        const int v = __shfl_up_sync(0xffffffffu, incl, off);
+                        if (lane >= off) incl += v;
+                    }
+                    L = __shfl_sync(0xffffffffu, incl, 31);
+                    const int b0 = __shfl_sync(0xffffffffu, incl - c, warp);
+                    const int b1 = __shfl_sync(0xffffffffu, incl - c, 16 + warp);
+                    if (rank0 >= 0) s_np[b0 + rank0] = (unsigned short)tid;
+                    if (rank1 >= 0) s_np[b1 + rank1] = (unsigned short)(tid + HOT_NT);
+                }
+                __syncthreads();
+                GLH_TL(3);
+                // ---- near-limb pairs: TWO lanes each (16 pairs per warp); the warps that have none fill
+                // the out-of-window part of the flux row meanwhile
+                const int nearwarps = min((L + 15) >> 4, HOT_NW);
+                if (frow && warp >= nearwarps) fill(tid - nearwarps * 32, (HOT_NW - nearwarps) * 32);
+                for (int q0 = 0; q0 < L; q0 += HOT_NT / 2) {
+                    const int q = q0 + (tid >> 1);
+                    if (q < L) {
+                        const int pr = s_np[q];
+                        const float xc = s_px[pr], yc = s_py[pr];
+                        const float d = near_delta<true>(s_trap, xc, yc, fmaf(xc, xc, yc * yc), a, b, ab, e2, k0,
+                                                         k1, k2, lane & 1, 3u << (lane & 30));
+                        if ((lane & 1) == 0) s_d[pr] = d;
+                    }
+                }
+                if (frow && nearwarps == HOT_NW) fill(tid, HOT_NT);
+                __syncthreads();
+                GLH_TL(6);
+                // exposure means, in sub-exposure order (R18)
+                for (int e = tid; e < M; e += HOT_NT) {
+                    float sum = 0.f;
+#pragma unroll 4
+                    for (int j = 0; j < S; ++j) sum += s_d[e * S + j];
+                    finish(s_li[e], sum * inv_ss, want_chi2 ? s_ow[e] : make_float2(0.f, 0.f));
+                }
+                GLH_TL(7);
+            } else {
+                // ---- 3b. DENSE list (a JWST-shaped series): thread v takes the v-th, (v + ntot)-th, ...
+                // in-window exposure, all its sub-exposures in turn; neighbouring lanes hold neighbouring
+                // exposures, i.e. nearly the same geometry and code path
+                GLH_TL(3);
+                for (int v = gtid; v < M; v += ntot) {
+                    int i;
+                    const float dtc = entry(v, &i);
+                    const float2 o2 = want_chi2 ? obs_of(i) : make_float2(0.f, 0.f);
+                    float sum = 0.f;
+                    for (int j = 0; j < S; ++j) {
+                        float xc, yc;
+                        position(dtc, j, &xc, &yc);
+                        sum += blocked_hot(s_trap, xc, yc, a, b, ab, e2, k0, k1, k2);
+                    }
+                    finish(i, sum * inv_ss, o2);
+                }
+                GLH_TL(6);
+                if (frow) fill(gtid, ntot);
             }
         }
         GLH_TL(4);
-        // ---- 5. chi^2 (and the cluster's verdict on the order of the series): CTA sum, partials
-        // pushed into rank 0's shared memory, one cluster barrier, rank 0 adds them in rank order
-        bool defer = (cls == CLS_DEFER);
+        // ---- 4. chi^2: CTA sum in fixed order, partials pushed into rank 0's shared memory, one
+        // cluster barrier, rank 0 adds them in rank order
         if (want_chi2) {
 #pragma unroll
             for (int off = 16; off > 0; off >>= 1) acc += __shfl_down_sync(0xffffffffu, acc, off);
@@ -580,7 +810,7 @@ __global__ void __launch_bounds__(HOT_NT, 2) hot_kernel(const HotArgs A) {
                     *cluster.map_shared_rank(&s_gflag[wpar][crank], 0) = unsorted;
                 } else {
                     s_gather[wpar][0] = tot;
-                    s_gflag[wpar][0] = unsorted;
+                    s_gflag[wpar][0] = 0;   // (a single CTA has already deferred an unsorted unit)
                 }
             }
             if (csize > 1) cluster.sync();
@@ -591,14 +821,14 @@ __global__ void __launch_bounds__(HOT_NT, 2) hot_kernel(const HotArgs A) {
                     d2 += s_gather[wpar][r];
                     uns |= s_gflag[wpar][r];
                 }
-                defer = defer || (uns != 0 && cls != CLS_INVALID);
+                if (uns && cls == CLS_SIMPLE) cls = CLS_DEFER;   // some CTA's share of the series is out of order
                 // raw series: baseline_kernel, launched before this grid (which may have started early:
                 // programmatic dependent launch), writes S into chi2[0..B): wait before touching chi2
                 if (!PRE) asm volatile("griddepcontrol.wait;" ::: "memory");
                 float out;
                 if (cls == CLS_INVALID) {
                     out = __int_as_float(0x7f800000);
-                } else if (defer) {
+                } else if (cls == CLS_DEFER) {
                     out = __uint_as_float(MARK_BITS);
                 } else {
                     double Sb = A.S;
@@ -606,15 +836,13 @@ __global__ void __launch_bounds__(HOT_NT, 2) hot_kernel(const HotArgs A) {
                     out = (Sb > 1.79769313486231570e308) ? (float)Sb : (float)(Sb + d2);
                 }
                 A.chi2[wk] = out;
-                if (defer && A.status) *A.status = 1;
+                if (cls == CLS_DEFER && A.status) *A.status = 1;
             }
             GLH_TL(5);
             wpar ^= 1;
-        } else if (frow) {
+        } else if (frow && cls == CLS_DEFER) {
             // flux-only units are single CTAs; the marker goes where this segment's row starts
-            defer = defer || (unsorted != 0 && cls != CLS_INVALID);
-            __syncthreads();   // every other store of this CTA to frow[0] is behind us
-            if (tid == 0 && defer) {
+            if (tid == 0) {
                 frow[0] = __uint_as_float(MARK_BITS);
                 if (A.status) *A.status = 1;
             }
