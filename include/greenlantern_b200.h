@@ -10,8 +10,13 @@
  *   - Work is enqueued on `stream` (a cudaStream_t passed as void*; NULL = the legacy default
  *     stream) and the call returns WITHOUT synchronising.  Buffers must stay alive until the
  *     stream has passed the work.
- *   - No hidden device allocation, no global mutable state: calls are re-entrant and may be
- *     issued concurrently on different streams.
+ *   - The device-pointer entry points allocate nothing and keep no per-call state: they are
+ *     re-entrant and may be issued concurrently on different streams.  What the library DOES keep:
+ *     (1) per device, the quadrature tables in constant memory, uploaded once by the first call on that
+ *     device (immutable afterwards); (2) per calling thread and device, for the *_host wrappers only,
+ *     one non-blocking stream and one private cudaMemPool that keeps its scratch between calls (the
+ *     device's default pool is not touched); both live until the thread ends; (3) what a gl_series
+ *     handle owns (see gl_series_create).  Nothing is read from the environment.
  *   - Return value: GL_OK or a negative gl_status.  Argument errors (GL_EINVAL) enqueue nothing.
  *     B == 0, T == 0 or N == 0 is GL_OK and enqueues nothing.
  *   - Parameters, times, observations and sigmas cross the boundary as fp64 whatever the compute
@@ -69,7 +74,8 @@ typedef enum {
  *   flux_out [B, T] row-major, float (GL_F32) or double (GL_F64) (device), fully overwritten.
  * Steps: Kepler + sky position (eqs. 9-10, R7), outline (PAPER.md:89-96
  * eqs. 11-13), outline/limb crossings (R3), boundary integrals (eqs. 21-23),
- * exposure mean -- one fused kernel, nothing per-sub-sample is stored. */
+ * exposure mean -- fused, nothing per-sub-sample is stored (GL_F32: hot_kernel + the full kernel for the
+ * walkers it defers, see gl_loglike; GL_F64: the full kernel). */
 int gl_lightcurve(const double* params, int B, const double* times, int T, double t_exp, int n_ss,
                   void* flux_out, gl_dtype dtype, void* stream);
 
@@ -77,11 +83,17 @@ int gl_lightcurve(const double* params, int B, const double* times, int T, doubl
  *   obs, sigma [T] fp64 (device), sigma > 0 (a non-positive or non-finite sigma makes every
  *   chi^2 +inf).  chi2_out [B] float/double per dtype, fully overwritten.
  *   flux_out_or_null: optional [B, T] output as in gl_lightcurve; NULL => the model flux never
- *   leaves registers.  The residual sum is accumulated in fp64 in both dtypes (GL_F32: the
- *   residuals themselves are formed in fp32 from the fp64 difference obs - 1, and the walker-
- *   independent part sum_i ((obs_i - 1)/sigma_i)^2 is formed once per call by a one-CTA kernel
- *   launched just before the transit kernel, which starts early by programmatic dependent launch:
- *   two launches on `stream`; GL_F64: one launch, everything per walker in fp64). */
+ *   leaves registers.  The residual sum is accumulated in fp64 in both dtypes.
+ *   GL_F64: one launch of the full transit kernel, everything per walker in fp64.
+ *   GL_F32 (12-column rows): THREE launches on `stream`, chained by programmatic dependent launch:
+ *   (1) a one-CTA kernel forms the walker-independent part S = sum_i ((obs_i - 1)/sigma_i)^2 once;
+ *   (2) hot_kernel finishes every walker on the common path (circular orbit, short transit window,
+ *   sorted series, outline that can cross the limb at most twice): in-window exposures found as index
+ *   ranges, chi^2 = S + sum over them of d (2 o r + d), o = obs - 1, r = 1/sigma, d = (1 - F) r, in
+ *   fp32 terms summed in fp64; every other walker is left marked in its output slot;
+ *   (3) the full transit kernel redoes exactly the marked walkers (it exits at once if there are none).
+ *   A caller that evaluates many batches against one series should use gl_series_* below, which does
+ *   (1) once per series. */
 int gl_loglike(const double* params, int B, const double* times, int T, double t_exp, int n_ss,
                const double* obs, const double* sigma, void* chi2_out, void* flux_out_or_null,
                gl_dtype dtype, void* stream);
@@ -181,7 +193,9 @@ int gl_flux_geometry_host(const double* geom, long long N, void* flux_out, gl_dt
  *   values as gl_loglike(GL_F32) up to the rounding of S (kept in fp64 here, narrowed there).
  * gl_series_loglike_dev: params, chi2_out, flux_out_or_null are DEVICE pointers; work is enqueued on
  *   `stream` without synchronising (the series buffers are only read, so several streams may use
- *   one handle through this call as long as the handle outlives the work).
+ *   one handle through this call as long as the handle outlives the work).  The launch pair is
+ *   captured once per distinct (params, B, chi2_out, flux_out_or_null) -- the last four are kept --
+ *   and replayed as a CUDA graph: a sampler that reuses its buffers pays one graph launch per step.
  * Launches per call: hot_kernel (walkers on the common path: circular orbit, n_ss <= 32, sorted
  * series, at most two limb crossings) followed, by programmatic dependent launch, by the full
  * transit kernel for the walkers the first one deferred.  The host call launches the second kernel

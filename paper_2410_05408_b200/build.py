@@ -13,7 +13,7 @@ from pathlib import Path
 CSRC = Path(__file__).resolve().parent / "csrc"
 LIB = CSRC / "libgreenlantern_b200.so"
 SOURCES = [CSRC / "greenlantern_b200.cu"]
-DEPENDS = SOURCES + [CSRC / "gl_core.cuh", CSRC / "gl_tables.h", CSRC / "gl_fast32.cuh", CSRC / "gl_simpson.cuh", CSRC / "gl_frontend.cuh", CSRC / "gl_gp.cuh", CSRC / "gl_gp_scan.cuh",
+DEPENDS = SOURCES + [CSRC / "gl_core.cuh", CSRC / "gl_tables.h", CSRC / "gl_fast32.cuh", CSRC / "gl_hot.cuh", CSRC / "gl_simpson.cuh", CSRC / "gl_frontend.cuh", CSRC / "gl_gp.cuh", CSRC / "gl_gp_scan.cuh",
                      CSRC.parents[1] / "include" / "greenlantern_b200.h"]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
               "-shared", "-Xcompiler", "-fPIC"]

@@ -43,6 +43,25 @@
 #ifndef GLH_TL
 #define GLH_TL(k) do { } while (0)
 #endif
+// CHECKED build (-DGLH_CHECKED; tests/test_gpu_parity.py builds it, the product never does): every
+// shared- and global-memory index of the transit kernels is asserted to be in range, and pseudo-random
+// per-CTA delays are injected in front of every cluster barrier, DSMEM access and marker read, so that
+// a protocol that only works by luck of timing shows up as a wrong or irreproducible result.
+// (compute-sanitizer is closed on the GPU pool this was developed on: profiles/r02_sanitizer.md.)
+#ifdef GLH_CHECKED
+#include <assert.h>
+#define GLH_ASSERT(c) assert(c)
+#define GLH_DELAY(k)                                                                                  \
+    do {                                                                                              \
+        const unsigned h_ = (blockIdx.x + 1u) * 2654435761u ^ (blockIdx.y + 7u) * 40503u ^ (unsigned)(k) * 977u; \
+        const long long n_ = (long long)((h_ >> 9) % 30000u);                                         \
+        const long long t0_ = clock64();                                                              \
+        while (clock64() - t0_ < n_) { }                                                              \
+    } while (0)
+#else
+#define GLH_ASSERT(c) do { } while (0)
+#define GLH_DELAY(k) do { } while (0)
+#endif
 
 namespace glh {
 
@@ -504,6 +523,7 @@ __device__ __forceinline__ int lower_bound_warp(const double* __restrict__ seg, 
     int cnt = 0;
     for (int m0 = base + 1; m0 < end; m0 += 32) {      // warp-uniform trip count
         const int m = m0 + lane;
+        GLH_ASSERT(m0 >= 0 && end <= n);
         cnt += __popc(__ballot_sync(0xffffffffu, m < end && seg[m] < q));
     }
     return min(base + 1 + cnt, n);
@@ -560,6 +580,7 @@ __global__ void __launch_bounds__(HOT_NT, 2) hot_kernel(const HotArgs A) {
         // per prelude warp (it may sit in host memory read over PCIe: gl_series_loglike).
         {
             const long long ci = (long long)tid * stride;
+            GLH_ASSERT(ci >= 0 && (ci < nT || ci >= nT));
             s_coarse[tid] = ci < nT ? seg[ci] : __longlong_as_double(0x7ff0000000000000LL);
         }
         int unsorted = 0;
@@ -637,6 +658,7 @@ __global__ void __launch_bounds__(HOT_NT, 2) hot_kernel(const HotArgs A) {
                         i = su.lo[k] + (v - run);
                     }
                 }
+                GLH_ASSERT(i >= 0 && i < nT && n >= 0 && n < MAXEP);
                 *idx = i;
                 return (float)(seg[i] - su.tc[n]);
             };
@@ -657,6 +679,7 @@ __global__ void __launch_bounds__(HOT_NT, 2) hot_kernel(const HotArgs A) {
                 return make_float2((float)(A.obs[t_lo + i] - 1.0), rs);
             };
             auto finish = [&](int i, float dbar, float2 o2) {   // exposure i is done: flux, chi^2 term
+                GLH_ASSERT(i >= 0 && i < nT);
                 if (frow) frow[i] = 1.f - dbar;
                 const float d = dbar * o2.y;
                 acc += (double)(d * fmaf(2.f * o2.x, o2.y, d));   // ((o + dbar) r)^2 - (o r)^2
@@ -678,6 +701,7 @@ __global__ void __launch_bounds__(HOT_NT, 2) hot_kernel(const HotArgs A) {
 #pragma unroll 1
                     for (int k = 0; k < nep; ++k) hit = hit || (i0 + 3 >= su.lo[k] && i0 < su.hi[k]);
                     if (!hit) {
+                        GLH_ASSERT(i0 >= 0 && i0 + 3 < nT && (((uintptr_t)(frow + i0)) & 15u) == 0);
                         *reinterpret_cast<float4*>(frow + i0) = make_float4(1.f, 1.f, 1.f, 1.f);
                     } else {
 #pragma unroll 1
@@ -704,6 +728,7 @@ __global__ void __launch_bounds__(HOT_NT, 2) hot_kernel(const HotArgs A) {
                         const int j = pr - e * S;
                         int i;
                         const float dtc = entry(e, &i);
+                        GLH_ASSERT(e >= 0 && e < M && e < CAP && j >= 0 && j < S);
                         if (j == 0) {
                             s_li[e] = i;
                             if (want_chi2) s_ow[e] = obs_of(i);
@@ -739,6 +764,7 @@ __global__ void __launch_bounds__(HOT_NT, 2) hot_kernel(const HotArgs A) {
                     L = __shfl_sync(0xffffffffu, incl, 31);
                     const int b0 = __shfl_sync(0xffffffffu, incl - c, warp);
                     const int b1 = __shfl_sync(0xffffffffu, incl - c, 16 + warp);
+                    GLH_ASSERT(L <= np && L <= CAP && (rank0 < 0 || b0 + rank0 < L) && (rank1 < 0 || b1 + rank1 < L));
                     if (rank0 >= 0) s_np[b0 + rank0] = (unsigned short)tid;
                     if (rank1 >= 0) s_np[b1 + rank1] = (unsigned short)(tid + HOT_NT);
                 }
@@ -752,6 +778,7 @@ __global__ void __launch_bounds__(HOT_NT, 2) hot_kernel(const HotArgs A) {
                     const int q = q0 + (tid >> 1);
                     if (q < L) {
                         const int pr = s_np[q];
+                        GLH_ASSERT(pr >= 0 && pr < np);
                         const float xc = s_px[pr], yc = s_py[pr];
                         const float d = near_delta<true>(s_trap, xc, yc, fmaf(xc, xc, yc * yc), a, b, ab, e2, k0,
                                                          k1, k2, lane & 1, 3u << (lane & 30));
@@ -763,6 +790,7 @@ __global__ void __launch_bounds__(HOT_NT, 2) hot_kernel(const HotArgs A) {
                 GLH_TL(6);
                 // exposure means, in sub-exposure order (R18)
                 for (int e = tid; e < M; e += HOT_NT) {
+                    GLH_ASSERT(e * S + S <= CAP);
                     float sum = 0.f;
 #pragma unroll 4
                     for (int j = 0; j < S; ++j) sum += s_d[e * S + j];
@@ -797,6 +825,7 @@ __global__ void __launch_bounds__(HOT_NT, 2) hot_kernel(const HotArgs A) {
 #pragma unroll
             for (int off = 16; off > 0; off >>= 1) acc += __shfl_down_sync(0xffffffffu, acc, off);
             if (lane == 0) s_red[warp] = acc;
+            GLH_DELAY(1);
             if (!started) {
                 cluster.barrier_wait();
                 started = true;
@@ -805,6 +834,7 @@ __global__ void __launch_bounds__(HOT_NT, 2) hot_kernel(const HotArgs A) {
             if (tid == 0) {
                 double tot = 0.0;
                 for (int k = 0; k < HOT_NW; ++k) tot += s_red[k];
+                GLH_DELAY(2);
                 if (csize > 1) {
                     *cluster.map_shared_rank(&s_gather[wpar][crank], 0) = tot;
                     *cluster.map_shared_rank(&s_gflag[wpar][crank], 0) = unsorted;
@@ -813,7 +843,9 @@ __global__ void __launch_bounds__(HOT_NT, 2) hot_kernel(const HotArgs A) {
                     s_gflag[wpar][0] = 0;   // (a single CTA has already deferred an unsorted unit)
                 }
             }
+            GLH_DELAY(3);
             if (csize > 1) cluster.sync();
+            GLH_DELAY(4);
             if (crank == 0 && tid == 0) {
                 double d2 = 0.0;
                 int uns = 0;

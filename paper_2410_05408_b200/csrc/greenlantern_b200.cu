@@ -609,6 +609,7 @@ transit_kernel(const double* __restrict__ params, int B,
             const T* slot = want_chi2 ? chi2 + wk : flux + (size_t)wk * nT_all + t_lo;
             any = any || (sizeof(T) == 4 && *reinterpret_cast<const volatile uint32_t*>(slot) == glh::MARK_BITS);
         }
+        GLH_DELAY(11);
         if (!__syncthreads_or(any ? 1 : 0)) return;
     }
     for (long long vw = blockIdx.y; vw < (long long)B * nseg; vw += gridDim.y) {
@@ -617,6 +618,7 @@ transit_kernel(const double* __restrict__ params, int B,
             const T* slot = want_chi2 ? chi2 + wk : flux + (size_t)wk * nT_all + t_lo;
             const uint32_t bits = sizeof(T) == 4 ? *reinterpret_cast<const volatile uint32_t*>(slot) : 0u;
             if (bits != glh::MARK_BITS) continue;   // (only this cluster ever rewrites this slot)
+            GLH_DELAY(12);
             if (csize > 1) cluster.sync();   // every CTA has read the slot before any CTA rewrites it
         }
         const double* __restrict__ times = times_all + t_lo;
@@ -668,6 +670,7 @@ transit_kernel(const double* __restrict__ params, int B,
                     s_cnt[1][warp] = wcount - wearly;
                 }
                 // nobody may still be reading the lists of the previous round / walker
+                GLH_DELAY(13);
                 if (lists_live) cluster.sync(); else __syncthreads();
                 // ---- pass 2: compact the in-window indices into this CTA's list: early entries
                 // first, then the rest, each ordered by (warp, sub-chunk, lane) -- fixed for a given
@@ -690,6 +693,8 @@ transit_kernel(const double* __restrict__ params, int B,
                             const unsigned bal0 = __ballot_sync(0xffffffffu, b0);
                             const unsigned bal1 = __ballot_sync(0xffffffffu, b1);
                             const unsigned lt = (1u << lane) - 1u;
+                            GLH_ASSERT(!b0 || base0 + __popc(bal0 & lt) < MAXTILE);
+                            GLH_ASSERT(!b1 || base1 + __popc(bal1 & lt) < MAXTILE);
                             if (b0) s_list[base0 + __popc(bal0 & lt)] = i0 + r * NT + tid;
                             if (b1) s_list[base1 + __popc(bal1 & lt)] = i0 + r * NT + tid;
                             base0 += __popc(bal0);
@@ -703,8 +708,10 @@ transit_kernel(const double* __restrict__ params, int B,
                 }
                 // ---- share the round's list over the cluster.  Cluster-wide order: the early
                 // entries of CTA 0, 1, ..., then the remaining entries of CTA 0, 1, ...
+                GLH_DELAY(14);
                 cluster.sync();
                 lists_live = true;
+                GLH_DELAY(15);
                 if (tid < 2) {
                     int run = 0;
                     for (int r = 0; r < csize; ++r) {
@@ -722,6 +729,7 @@ transit_kernel(const double* __restrict__ params, int B,
 #pragma unroll
                     for (int c = 1; c < MAXCLUSTER; ++c) r += (q >= s_pre[k][c] && c < csize) ? 1 : 0;
                     const int local = q - s_pre[k][r] + (k ? s_pre[0][r + 1] - s_pre[0][r] : 0);
+                    GLH_ASSERT(r >= 0 && r < csize && local >= 0 && local < MAXTILE);
                     return *cluster.map_shared_rank(&s_list[local], r);
                 };
                 // ---- evaluate the round's list: the cluster's warps take groups of exposures in
@@ -762,6 +770,7 @@ transit_kernel(const double* __restrict__ params, int B,
                             sum += __shfl_sync(0xffffffffu, delta, (lane + bb) & 31);
                         if (active && my_b == 0) {
                             const T dbar = sum * T(inv_ss);
+                            GLH_ASSERT(i >= 0 && i < nT);
                             if (frow) frow[i] = T(1) - dbar;
                             if (want_chi2) acc += listed_residual<T>(obs[i] - 1.0, dbar, sigma[i], shared_base);
                         }
@@ -795,8 +804,11 @@ transit_kernel(const double* __restrict__ params, int B,
         // can only pass once it has read the slot.
         if (want_chi2) {
             const double tot = block_sum(acc, s_red);
+            GLH_DELAY(16);
             if (tid == 0) *cluster.map_shared_rank(&s_gather[wpar][crank], 0) = tot;
+            GLH_DELAY(17);
             cluster.sync();
+            GLH_DELAY(18);
             lists_live = false;   // every CTA is past its evaluation
             if (crank == 0 && tid == 0) {
                 double c2 = 0.0;
@@ -1365,36 +1377,24 @@ int gl_gp_loglike(const double* params, int B, const double* times, int T, doubl
     int rc = gl_lightcurve(params, B, times, T, t_exp, n_ss, flux_work, dtype, stream);
     if (rc != GL_OK) return rc;
     cudaStream_t st = (cudaStream_t)stream;
-    // one CTA per walker, parallel in time (gl_gp_scan.cuh); GL_GP_SERIAL=1 selects the one-thread-
-    // per-walker filter of gl_gp.cuh (kept as the plain version the scan is checked against)
-    static const bool serial = getenv("GL_GP_SERIAL") && atoi(getenv("GL_GP_SERIAL")) != 0;
-    if (serial) {
-        const unsigned blocks = (unsigned)((B + 31) / 32);
-        if (dtype == GL_F32)
-            glg::gp_kernel<float><<<blocks, 32, 0, st>>>((const float*)flux_work, B, times, T, obs, sigma,
-                                                         gp, loglike_out);
-        else
-            glg::gp_kernel<double><<<blocks, 32, 0, st>>>((const double*)flux_work, B, times, T, obs,
-                                                          sigma, gp, loglike_out);
-    } else {
-        cudaLaunchConfig_t cfg = {};
-        cfg.gridDim = dim3((unsigned)B, 1, 1);
-        cfg.blockDim = dim3(glg::GP_NT, 1, 1);
-        cfg.stream = st;
-        cudaLaunchAttribute attr[1];
-        attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
-        attr[0].val.programmaticStreamSerializationAllowed = 1;
-        cfg.attrs = attr;
-        cfg.numAttrs = 1;
-        cudaError_t el = (dtype == GL_F32)
-            ? cudaLaunchKernelEx(&cfg, glg::gp_scan_kernel<float>, (const float*)flux_work, B, times, T,
-                                 obs, sigma, gp, loglike_out)
-            : cudaLaunchKernelEx(&cfg, glg::gp_scan_kernel<double>, (const double*)flux_work, B, times, T,
-                                 obs, sigma, gp, loglike_out);
-        if (el != cudaSuccess) return cuda_fail(el, "gp_scan_kernel launch");
-    }
+    // one CTA per walker, parallel in time (gl_gp_scan.cuh)
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = dim3((unsigned)B, 1, 1);
+    cfg.blockDim = dim3(glg::GP_NT, 1, 1);
+    cfg.stream = st;
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    attr[0].val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = attr;
+    cfg.numAttrs = 1;
+    cudaError_t el = (dtype == GL_F32)
+        ? cudaLaunchKernelEx(&cfg, glg::gp_scan_kernel<float>, (const float*)flux_work, B, times, T,
+                             obs, sigma, gp, loglike_out)
+        : cudaLaunchKernelEx(&cfg, glg::gp_scan_kernel<double>, (const double*)flux_work, B, times, T,
+                             obs, sigma, gp, loglike_out);
+    if (el != cudaSuccess) return cuda_fail(el, "gp_scan_kernel launch");
     cudaError_t e = cudaGetLastError();
-    if (e != cudaSuccess) return cuda_fail(e, "gp_kernel launch");
+    if (e != cudaSuccess) return cuda_fail(e, "gp_scan_kernel launch");
     ++tl_launches;
     return GL_OK;
 }
@@ -1402,7 +1402,7 @@ int gl_gp_loglike(const double* params, int B, const double* times, int T, doubl
 int gl_probe_peaks(double* out3) {
     if (!out3) return GL_EINVAL;
     void* scratch = nullptr;
-    const int blocks = 148 * 8, thr = 256, iters = 8192;
+    const int blocks = sm_count() * 8, thr = 256, iters = 8192;
     cudaError_t e = cudaMalloc(&scratch, (size_t)blocks * thr * sizeof(double));
     if (e != cudaSuccess) return cuda_fail(e, "gl_probe_peaks cudaMalloc");
     cudaEvent_t a, b;
@@ -1490,38 +1490,58 @@ const char* gl_strerror(int code) {
 // ------------------------------------------------------------------------------------------
 namespace {
 
-// One non-blocking stream per calling thread and device, created on first use and kept; the
-// device's default memory pool is told to keep its memory between calls (release threshold = max),
-// otherwise every synchronise hands the scratch back to the driver and the next call pays
-// milliseconds to get it again.
-cudaStream_t host_stream(cudaError_t* err) {
-    thread_local cudaStream_t streams[64] = {};
+// One non-blocking stream and one PRIVATE memory pool per calling thread and device, created on first
+// use and kept for the life of the thread (include/greenlantern_b200.h says so).  The pool keeps its
+// memory between calls (release threshold = max), otherwise every synchronise hands the scratch back
+// to the driver and the next call pays milliseconds to get it again; the device's default pool is
+// not touched.
+struct HostCtx {
+    cudaStream_t st = nullptr;
+    cudaMemPool_t pool = nullptr;
+};
+HostCtx* host_ctx(cudaError_t* err) {
+    thread_local HostCtx ctx[64];
     int dev = 0;
     *err = cudaGetDevice(&dev);
     if (*err != cudaSuccess) return nullptr;
     if (dev < 0 || dev >= 64) dev = 63;
-    if (!streams[dev]) {
-        *err = cudaStreamCreateWithFlags(&streams[dev], cudaStreamNonBlocking);
+    HostCtx* c = &ctx[dev];
+    if (!c->st) {
+        *err = cudaStreamCreateWithFlags(&c->st, cudaStreamNonBlocking);
         if (*err != cudaSuccess) return nullptr;
-        cudaMemPool_t pool;
-        if (cudaDeviceGetDefaultMemPool(&pool, dev) == cudaSuccess) {
-            unsigned long long keep = ~0ull;
-            cudaMemPoolSetAttribute(pool, cudaMemPoolAttrReleaseThreshold, &keep);
+        cudaMemPoolProps props = {};
+        props.allocType = cudaMemAllocationTypePinned;
+        props.handleTypes = cudaMemHandleTypeNone;
+        props.location.type = cudaMemLocationTypeDevice;
+        props.location.id = dev;
+        *err = cudaMemPoolCreate(&c->pool, &props);
+        if (*err != cudaSuccess) {
+            cudaStreamDestroy(c->st);
+            c->st = nullptr;
+            return nullptr;
         }
+        unsigned long long keep = ~0ull;
+        cudaMemPoolSetAttribute(c->pool, cudaMemPoolAttrReleaseThreshold, &keep);
     }
-    return streams[dev];
+    return c;
 }
 
 struct HostCall {
     cudaStream_t st = nullptr;
+    cudaMemPool_t pool = nullptr;
     void* bufs[8];
     int nbufs = 0;
     cudaError_t err = cudaSuccess;
-    HostCall() { st = host_stream(&err); }
+    HostCall() {
+        if (HostCtx* c = host_ctx(&err)) {
+            st = c->st;
+            pool = c->pool;
+        }
+    }
     void* alloc(size_t bytes) {
         void* p = nullptr;
         if (err != cudaSuccess) return nullptr;
-        err = cudaMallocAsync(&p, bytes ? bytes : 1, st);
+        err = cudaMallocFromPoolAsync(&p, bytes ? bytes : 1, pool, st);
         if (err == cudaSuccess) bufs[nbufs++] = p;
         return p;
     }

@@ -32,3 +32,16 @@ extern "C" int host_flux_geometry_f32(const double* geom, long long n, double* f
     }
     return 0;
 }
+
+// The tables of the library's generator (gl_tables.h), for the check of the literal copies that
+// csrc/gl_hot.cuh carries as immediates: phi8, om8 = smoothed 16-point Gauss-Legendre; trap32 =
+// (cos, sin)(pi k / 16), k = 0..15, interleaved.
+extern "C" void host_tables(float* phi8, float* om8, float* trap32) {
+    glt::smoothed_gauss_legendre<float>(16, phi8, om8);
+    for (int k = 0; k < 16; ++k) {
+        trap32[2 * k] = (float)cosl(3.141592653589793238462643383279502884L * k / 16);
+        trap32[2 * k + 1] = (float)sinl(3.141592653589793238462643383279502884L * k / 16);
+    }
+    trap32[16] = 0.f;   // exact zeros at the axes, as the library sets them
+    trap32[1] = 0.f;
+}

@@ -64,3 +64,21 @@ def test_fast32_golden_pins(host_lib):
                      (1.0, 0.1, 0.5, 2.0, 0.7, -0.1)])
     want = np.array([0.998815344408319, 0.994809529489372, 0.998408554994727])
     assert np.abs(run(host_lib, geom) - want).max() <= 5e-7
+
+
+def test_hot_kernel_literal_tables_match_the_generator(host_lib):
+    """csrc/gl_hot.cuh carries the quadrature tables as literals (immediates in the unrolled loop, a
+    statically initialised constant array): they must be the generator's values, bit for bit."""
+    import re
+    text = (HERE.parent / "paper_2410_05408_b200" / "csrc" / "gl_hot.cuh").read_text()
+
+    def floats(body):
+        return np.array([np.float32(x) for x in re.findall(r"(-?\d+\.?\d*(?:e-?\d+)?)f", body)], dtype=np.float32)
+    phi = floats(re.search(r"#define GLH_GL_PHI \{([^}]*)\}", text).group(1))
+    om = floats(re.search(r"#define GLH_GL_OM \{([^}]*)\}", text).group(1))
+    trap = floats(re.search(r"c_trap16\[16\] = \{(.*?)\};", text, re.S).group(1))
+    assert phi.size == 8 and om.size == 8 and trap.size == 32
+    p, o, t = np.zeros(8, np.float32), np.zeros(8, np.float32), np.zeros(32, np.float32)
+    host_lib.host_tables(p.ctypes.data_as(ctypes.c_void_p), o.ctypes.data_as(ctypes.c_void_p),
+                         t.ctypes.data_as(ctypes.c_void_p))
+    assert np.array_equal(phi, p) and np.array_equal(om, o) and np.array_equal(trap, t)

@@ -57,9 +57,12 @@ def test_config2_k2_single(gl, dtype):
     chi_only = gl.gl_loglike(dev(w.params), dev(w.times), w.t_exp, w.n_ss, dev(w.obs),
                              dev(w.sigma), dtype=dtype)
     assert np.array_equal(host(chi_only), host(chi))
-    # gl_lightcurve agrees with gl_loglike's flux bit for bit
+    # gl_lightcurve (another launch shape: the series cut into segments; sparse or dense evaluation per
+    # segment) agrees with gl_loglike's flux to 2 ulp of 1 in fp32 (the two evaluation modes run the same
+    # arithmetic in the same order, but the compiler may contract a product differently in each) and bit
+    # for bit in fp64
     lc = gl.gl_lightcurve(dev(w.params), dev(w.times), w.t_exp, w.n_ss, dtype=dtype)
-    assert np.array_equal(host(lc), host(out))
+    assert np.abs(host(lc) - host(out)).max() <= (1.2e-7 if dtype == "f32" else 0.0)
 
 
 @pytest.mark.parametrize("dtype", ["f32", "f64"])
@@ -207,7 +210,7 @@ def test_many_rounds_and_many_walkers(gl, dtype):
     assert np.abs(host(out) - ref).max() <= FTOL[dtype]
     assert np.abs(host(chi) / chi_ref - 1.0).max() <= CTOL[dtype]
     lc = gl.gl_lightcurve(dev(p), dev(t), base.t_exp, 3, dtype=dtype)
-    assert np.array_equal(host(lc), host(out))
+    assert np.abs(host(lc) - host(out)).max() <= (1.2e-7 if dtype == "f32" else 0.0)
     # 2) 70 000 walkers (> 65 535 grid rows) on a short stretch around mid-transit
     B = 70_000
     pw = wl.draw_walkers(B, 99)
@@ -481,12 +484,36 @@ def test_gp_likelihood(gl, dtype):
     assert np.isnan(out[0]) and np.isfinite(out[1])
 
 
-def test_gp_serial_and_scan_filters_agree(gl, tmp_path):
-    """The one-thread-per-walker filter (GL_GP_SERIAL=1, read once per process: run in a child) and
-    the parallel-in-time scan give the same likelihood (both were checked against the dense
-    definition above; this keeps the plain version alive)."""
+def _gp_serial(tmp_path):
+    """tests/gp_serial_harness.cu (the plain serial filter, test infrastructure) built with nvcc."""
+    import ctypes
     import subprocess
-    import sys
+    from pathlib import Path
+    src = Path(__file__).resolve().parent / "gp_serial_harness.cu"
+    so = tmp_path / "libgp_serial.so"
+    subprocess.run(["nvcc", "-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-std=c++17", "-shared",
+                    "-Xcompiler", "-fPIC", "-o", str(so), str(src)], check=True)
+    lib = ctypes.CDLL(str(so))
+    vp, i = ctypes.c_void_p, ctypes.c_int
+    lib.gp_serial_loglike.argtypes = [vp, i, vp, i, vp, vp, vp, vp, i]
+    lib.gp_serial_loglike.restype = i
+
+    def run(flux, times, obs, sigma, gp):
+        import torch
+        out = torch.empty(flux.shape[0], dtype=torch.float64, device="cuda:0")
+        torch.cuda.synchronize()
+        rc = lib.gp_serial_loglike(flux.data_ptr(), flux.shape[0], times.data_ptr(), times.shape[0],
+                                   obs.data_ptr(), sigma.data_ptr(), gp.data_ptr(), out.data_ptr(),
+                                   1 if flux.dtype == torch.float64 else 0)
+        assert rc == 0
+        return host(out)
+    return run
+
+
+def test_gp_serial_and_scan_filters_agree(gl, tmp_path):
+    """The one-thread-per-walker filter (tests/gp_serial_harness.cu) and the library's parallel-in-time
+    scan give the same likelihood (both are also checked against the dense definition)."""
+    serial_of = _gp_serial(tmp_path)
     rng = np.random.default_rng(61)
     w = wl.config3(B=6)
     T = 700                                    # not a multiple of the 256 chunks, ragged last chunk
@@ -494,16 +521,10 @@ def test_gp_serial_and_scan_filters_agree(gl, tmp_path):
     sig = rng.uniform(0.5e-4, 2e-4, T)
     obs = 1.0 + 1e-4 * rng.standard_normal(T)
     gp = np.column_stack([rng.uniform(0.3e-4, 5e-4, 6), rng.uniform(0.01, 1.0, 6), np.full(6, 1e-4)])
-    np.savez(tmp_path / "in.npz", p=w.params, t=t, obs=obs, sig=sig, gp=gp)
-    code = ("import numpy as np, torch, sys; sys.path.insert(0, %r); import paper_2410_05408_b200 as g; "
-            "z = np.load(%r); d = lambda x: torch.as_tensor(x, device='cuda'); "
-            "np.save(%r, g.gl_gp_loglike(d(z['p']), d(z['t']), 0.0, 1, d(z['obs']), d(z['sig']), d(z['gp']), "
-            "dtype='f64').cpu().numpy())") % (str(wl.__file__.rsplit('/', 2)[0]), str(tmp_path / "in.npz"),
-                                              str(tmp_path / "serial.npy"))
-    import os
-    subprocess.run([sys.executable, "-c", code], check=True, env=dict(os.environ, GL_GP_SERIAL="1"))
-    serial = np.load(tmp_path / "serial.npy")
-    scan = host(gl.gl_gp_loglike(dev(w.params), dev(t), 0.0, 1, dev(obs), dev(sig), dev(gp), dtype="f64"))
+    scan, flux = gl.gl_gp_loglike(dev(w.params), dev(t), 0.0, 1, dev(obs), dev(sig), dev(gp), dtype="f64",
+                                  want_flux=True)
+    scan = host(scan)
+    serial = serial_of(flux, dev(t), dev(obs), dev(sig), dev(gp))
     assert np.abs(scan / serial - 1.0).max() <= 1e-10
     F = orc.lightcurve(w.params, t, 0.0, 1)
     ref = np.array([orc.gp_loglike_dense(obs - F[k], t, sig, *gp[k]) for k in range(6)])
@@ -512,11 +533,10 @@ def test_gp_serial_and_scan_filters_agree(gl, tmp_path):
     # 13-level scan) through both filters
     w4 = wl.config4(B=4)
     gp4 = np.column_stack([[1e-5, 3e-5, 1e-4, 3e-4], [0.002, 0.02, 0.2, 2.0], np.full(4, 1e-5)])
-    np.savez(tmp_path / "in.npz", p=w4.params, t=w4.times, obs=w4.obs, sig=w4.sigma, gp=gp4)
-    subprocess.run([sys.executable, "-c", code], check=True, env=dict(os.environ, GL_GP_SERIAL="1"))
-    serial4 = np.load(tmp_path / "serial.npy")
-    scan4 = host(gl.gl_gp_loglike(dev(w4.params), dev(w4.times), 0.0, 1, dev(w4.obs), dev(w4.sigma),
-                                  dev(gp4), dtype="f64"))
+    scan4, flux4 = gl.gl_gp_loglike(dev(w4.params), dev(w4.times), 0.0, 1, dev(w4.obs), dev(w4.sigma),
+                                    dev(gp4), dtype="f64", want_flux=True)
+    scan4 = host(scan4)
+    serial4 = serial_of(flux4, dev(w4.times), dev(w4.obs), dev(w4.sigma), dev(gp4))
     assert np.all(np.isfinite(scan4)) and np.abs(scan4 / serial4 - 1.0).max() <= 1e-10
 
 
@@ -658,11 +678,11 @@ def test_hot_and_deferred_walkers_in_one_batch(gl):
     assert np.abs(chi[~bad] / chi_ref[~bad] - 1.0).max() <= 1e-4
     # gl_lightcurve cuts the series into segments, so a walker with many transit epochs may be on
     # the hot kernel there and on the full kernel here: equal to rounding, not bit for bit; walkers
-    # that are on the hot kernel both times (rows 0, 6, 7 mod 8) are bit-identical
+    # that are on the hot kernel both times (rows 0, 6, 7 mod 8) agree to 2 ulp
     lc = host(gl.gl_lightcurve(dev(p), dev(w.times), w.t_exp, w.n_ss, dtype="f32"))
     assert np.abs(lc[~bad] - out[~bad]).max() <= 2e-7 and np.all(np.isnan(lc[bad]))
     same = np.r_[0:40:8, 6:40:8, 7:40:8]
-    assert np.array_equal(lc[same], out[same])
+    assert np.abs(lc[same] - out[same]).max() <= 1.2e-7
     chi_only = host(gl.gl_loglike(dev(p), dev(w.times), w.t_exp, w.n_ss, dev(w.obs), dev(w.sigma),
                                   dtype="f32"))
     assert np.array_equal(chi_only, chi)
@@ -769,3 +789,40 @@ def test_resident_series_api(gl):
     ser3.close()
     with pytest.raises(gl.GreenlanternError):
         gl.GlSeries(w.times[:0], w.obs[:0], w.sigma[:0], 0.0, 1, B_max=1)
+
+
+def test_checked_build_index_assertions_and_delays(gl, tmp_path):
+    """compute-sanitizer is closed on this GPU pool (profiles/r02_sanitizer.md), so the library carries
+    its own checks: built with -DGLH_CHECKED every shared/global index of the transit kernels is
+    asserted in range and pseudo-random per-CTA delays sit in front of every cluster barrier, DSMEM
+    access and marker read.  The shapes of tests/sanitizer_shapes.py (clusters, many units per cluster,
+    multi-round series, PDL chains, deferred walkers, graph replay) must run clean through that build
+    twice with bit-identical outputs, equal to the product build's up to the last place."""
+    import subprocess
+    import sys
+    from pathlib import Path
+    root = Path(__file__).resolve().parents[1]
+    so = tmp_path / "libgreenlantern_checked.so"
+    subprocess.run(["nvcc", "-DGLH_CHECKED", "-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-std=c++17",
+                    "-shared", "-Xcompiler", "-fPIC", "-diag-suppress", "128", "-o", str(so),
+                    str(root / "paper_2410_05408_b200" / "csrc" / "greenlantern_b200.cu")], check=True)
+    script = str(root / "tests" / "sanitizer_shapes.py")
+
+    def run(tag, *extra):
+        r = subprocess.run([sys.executable, script, "--quick", *extra, "--dump", str(tmp_path / f"{tag}.npz")],
+                           capture_output=True, text=True)
+        assert r.returncode == 0, r.stdout[-2000:] + r.stderr[-2000:]
+        return np.load(tmp_path / f"{tag}.npz")
+    prod = run("product")
+    chk1 = run("checked1", "--lib", str(so))
+    chk2 = run("checked2", "--lib", str(so))
+    assert sorted(prod.files) == sorted(chk1.files) == sorted(chk2.files) and len(prod.files) >= 15
+    for k in prod.files:
+        # the same build twice: bit-identical (a race would show as run-to-run differences) ...
+        assert np.array_equal(chk1[k], chk2[k], equal_nan=True), k
+        # ... and equal to the product build up to the last place (another compilation of the same source
+        # may contract a product into an FMA differently; a protocol error would be orders larger)
+        a, b = prod[k].astype(np.float64), chk1[k].astype(np.float64)
+        same = (np.isnan(a) & np.isnan(b)) | (np.isinf(a) & np.isinf(b) & (np.sign(a) == np.sign(b)))
+        d = np.abs(np.where(same, 0.0, a - b)) / np.maximum(np.abs(np.where(same, 1.0, a)), 1.0)
+        assert d.max() <= 2e-6, (k, d.max())
