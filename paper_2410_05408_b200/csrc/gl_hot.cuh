@@ -252,6 +252,11 @@ __device__ __forceinline__ void critical_point_rt(float xc, float yc, float a, f
     }
 }
 
+template <bool TWO>
+__device__ __forceinline__ float near_rest(const glf::TrapNode* trap, float xc, float yc, float r0sq, float a,
+                                           float b, float ab, float e2, float k0, float k1, float k2, float cf,
+                                           float sf, float cn, float sn, int h, unsigned mask);
+
 // Path 4.  xc, yc >= 0.  TWO: lanes `lane` and `lane ^ 1` of the warp hold the SAME pair; h = lane & 1
 // says which half this lane does (mask = the lanes that are in here together: whole lane pairs).
 template <bool TWO>
@@ -259,7 +264,6 @@ __device__ __forceinline__ float near_delta(const glf::TrapNode* trap, float xc,
                                             float b, float ab, float e2, float k0, float k1, float k2, int h,
                                             unsigned mask) {
     using namespace glf;
-    const float u = b * xc, v = a * yc;
     // ---- critical points of g = x^2 + y^2 - 1 on the outline: the farthest point from the star centre
     // (first quadrant) and the nearest (third quadrant), both started from the direction (a xc, b yc)
     const float Aa = a * xc, Bb = b * yc;
@@ -282,6 +286,17 @@ __device__ __forceinline__ float near_delta(const glf::TrapNode* trap, float xc,
         cn = -c0;
         sn = -s0;
     }
+    return near_rest<TWO>(trap, xc, yc, r0sq, a, b, ab, e2, k0, k1, k2, cf, sf, cn, sn, h, mask);
+}
+
+// The rest of path 4 once the farthest point (cf, sf) is known; (cn, sn) = the nearest point (TWO) or
+// the starting direction of its search (one lane: it is searched here, only if needed).
+template <bool TWO>
+__device__ __forceinline__ float near_rest(const glf::TrapNode* trap, float xc, float yc, float r0sq, float a,
+                                           float b, float ab, float e2, float k0, float k1, float k2, float cf,
+                                           float sf, float cn, float sn, int h, unsigned mask) {
+    using namespace glf;
+    const float u = b * xc, v = a * yc;
     const float xf = fmaf(a, cf, xc), yf = fmaf(b, sf, yc);
     const float gfar = fmaf(xf, xf, fmaf(yf, yf, -1.f));
     if (gfar <= 0.f) {

@@ -614,9 +614,9 @@ transit_kernel(const double* __restrict__ params, int B,
     }
     for (long long vw = blockIdx.y; vw < (long long)B * nseg; vw += gridDim.y) {
         const int wk = (int)(vw / nseg), t_lo = (int)(vw - (long long)wk * nseg) * seglen;
-        if (marker_mode) {
+        if (sizeof(T) == 4 && marker_mode) {   // (markers are an fp32 affair: hot_kernel has no fp64 flavour)
             const T* slot = want_chi2 ? chi2 + wk : flux + (size_t)wk * nT_all + t_lo;
-            const uint32_t bits = sizeof(T) == 4 ? *reinterpret_cast<const volatile uint32_t*>(slot) : 0u;
+            const uint32_t bits = *reinterpret_cast<const volatile uint32_t*>(slot);
             if (bits != glh::MARK_BITS) continue;   // (only this cluster ever rewrites this slot)
             GLH_DELAY(12);
             if (csize > 1) cluster.sync();   // every CTA has read the slot before any CTA rewrites it
@@ -840,7 +840,9 @@ geometry_kernel(const double* __restrict__ geom, long long N, T* __restrict__ ou
     if (threadIdx.x < 16)
         s_trap[threadIdx.x] = glf::TrapNode{glf::c_trap_cos[threadIdx.x], glf::c_trap_sin[threadIdx.x]};
     __syncthreads();
-    const long long k = (long long)blockIdx.x * NT + threadIdx.x;
+    // blocks of 32 rows dealt round-robin to the CTAs (a stretch of expensive rows -- config 5 ends with
+    // 100 000 forced ones -- is spread over the grid; see geometry_sorted_kernel)
+    const long long k = ((long long)(threadIdx.x >> 5) * gridDim.x + blockIdx.x) * 32 + (threadIdx.x & 31);
     if (k >= N) return;
     const double* g = geom + k * GL_NGEOM;
     const double d = g[0], Rp = g[1], fp = g[2], pa = g[3], u1 = g[4], u2 = g[5];
@@ -861,32 +863,47 @@ geometry_kernel(const double* __restrict__ geom, long long N, T* __restrict__ ou
     out[k] = T(1) - delta;
 }
 
-// fp32 production version of the above: the same arithmetic (glf::blocked_f32), but a CTA first
-// SORTS its GEO_ROWS rows by the code path they will take, so that the lanes of a warp run the same
-// path.  Bare geometries arrive in random order (config 5: 76 % inside the disc, 14 % crossing the
-// limb, 10 % outside), and with one row per thread in input order a warp executed every path for a
-// few lanes each (ncu: 7.8 of 32 lanes active per instruction).  Bins, in list order: outlines deep
-// inside (6 immediate nodes); inside with 8 or 16 table nodes; everything that needs the farthest
-// point first (near the limb, crossing it, or the evolute case).  Rows that are invalid or do not
-// overlap the disc are finished in the first pass.  Outputs do not depend on the bin order.
+// fp32 production version of the above.  Bare geometries arrive in random order (config 5: 76 % inside
+// the disc, 14 % crossing the limb, 10 % outside, plus forced tangent / grazing / four-crossing rows),
+// and with one row per thread in input order a warp executed every code path for a few lanes each
+// (7.8 of 32 lanes active per instruction; a three-bin ordering per CTA reached 16.8: round 1).  Here a
+// CTA takes GEO_ROWS rows and SORTS them by the code path they will really take, in two stages:
+//   stage 1  validity, kernel-frame centre, path_of() (gl_hot.cuh): no overlap -> done; 6 / 8 / 16 fixed
+//            nodes -> three lists; near the limb -> a fourth list
+//   stage 2  the three fixed-node lists, one after the other, full warps (glh::cheap_delta)
+//   stage 3  near-limb rows: evolute test (only rows whose star centre may lie inside the outline's
+//            evolute take the generic bracketed search) and the farthest point; what comes out -- inside
+//            with 16 or 32 nodes, two crossings, evolute -- is listed again
+//   stage 4  those three lists, full warps each (glh::near_rest, glc::overlap_areas)
+// Outputs go to fixed slots, so the order inside a list (atomics) does not matter.
 constexpr int GEO_NT = 256, GEO_PER = 4, GEO_ROWS = GEO_NT * GEO_PER;
 __global__ void __launch_bounds__(GEO_NT)
-geometry_binned_kernel(const double* __restrict__ geom, long long N, float* __restrict__ out) {
+geometry_sorted_kernel(const double* __restrict__ geom, long long N, float* __restrict__ out) {
     __shared__ glf::TrapNode s_trap[16];
-    __shared__ float s_par[7][GEO_ROWS];   // xc, yc, a, b, k0, k1, k2 of the CTA's rows
-    __shared__ short s_order[GEO_ROWS];    // local row numbers, bin after bin
-    __shared__ int s_count[3], s_start[3];
+    __shared__ float s_par[7][GEO_ROWS];        // xc, yc (folded), a, b, k0, k1, k2 of the CTA's rows
+    __shared__ float s_far[2][GEO_ROWS];        // near-limb rows: farthest outline point (cos, sin)
+    __shared__ unsigned short s_ord[GEO_ROWS];  // stage-1 lists: paths 4, 3, 2, 1 one after the other
+    __shared__ unsigned short s_ord2[GEO_ROWS]; // stage-3 lists: crossing, inside near the limb, evolute
+    __shared__ int s_count[4], s_start[5], s_count2[3], s_start2[4];
     const int tid = threadIdx.x;
-    if (tid < 16) s_trap[tid] = glf::TrapNode{glf::c_trap_cos[tid], glf::c_trap_sin[tid]};
-    if (tid < 3) s_count[tid] = 0;
+    asm volatile("griddepcontrol.launch_dependents;");   // geometry_evolute_kernel may become resident
+    if (tid < 16) s_trap[tid] = glf::TrapNode{glh::c_trap16[tid].x, glh::c_trap16[tid].y};
+    if (tid < 4) s_count[tid] = 0;
+    if (tid < 3) s_count2[tid] = 0;
     __syncthreads();
-    const long long base = (long long)blockIdx.x * GEO_ROWS;
-    int bin[GEO_PER], slot[GEO_PER];
+    // rows are dealt to the CTAs in blocks of 32 (one coalesced 1.5 KB read per warp), ROUND-ROBIN: local
+    // row loc sits in block (loc / 32) gridDim.x + blockIdx.x.  A stretch of the input full of one
+    // expensive kind of geometry (config 5 ends with 100 000 forced rows) is thereby spread over the
+    // whole grid instead of landing on a few CTAs that finish long after the others.
+    auto row_of = [&](int loc) {
+        return ((long long)(loc >> 5) * gridDim.x + blockIdx.x) * 32 + (loc & 31);
+    };
+    int path[GEO_PER], slot[GEO_PER];
 #pragma unroll
     for (int q = 0; q < GEO_PER; ++q) {
         const int loc = q * GEO_NT + tid;
-        const long long k = base + loc;
-        bin[q] = -1;
+        const long long k = row_of(loc);
+        path[q] = 0;
         slot[q] = 0;
         if (k >= N) continue;
         const double* g = geom + k * GL_NGEOM;
@@ -900,41 +917,158 @@ geometry_binned_kernel(const double* __restrict__ geom, long long N, float* __re
             continue;
         }
         float s, c;
-        sincosf((float)pa, &s, &c);
+        glh::angle_sincos(pa, &s, &c);
         const float a = (float)Rp, b = (float)(Rp * (1.0 - fp)), r0 = (float)d;
-        if (r0 >= 1.f + a) {   // no overlap (blocked_f32's own first test)
+        const float xc = fabsf(r0 * c), yc = fabsf(r0 * s);
+        float r0r;
+        path[q] = glh::path_of(fmaf(xc, xc, yc * yc), a, &r0r);
+        if (path[q] == 0) {   // no overlap
             out[k] = 1.f;
             continue;
         }
-        const double pn = kPi * norm;
-        s_par[0][loc] = r0 * c;
-        s_par[1][loc] = -r0 * s;
+        const float ipn = glh::rcp_nr((float)(kPi * norm));
+        s_par[0][loc] = xc;
+        s_par[1][loc] = yc;
         s_par[2][loc] = a;
         s_par[3][loc] = b;
-        s_par[4][loc] = (float)((1.0 - u1 - 2.0 * u2) / pn);
-        s_par[5][loc] = (float)((u1 + 2.0 * u2) / pn);
-        s_par[6][loc] = (float)(u2 / pn);
-        // the tiers of glf::blocked_f32 (it decides again by itself; this only orders the work)
-        bin[q] = (r0 + a > 0.99f) ? 2 : ((fmaf(4.f, a, r0) <= 1.f || r0 + a <= 0.5f) ? 0 : 1);
-        slot[q] = atomicAdd(&s_count[bin[q]], 1);
+        s_par[4][loc] = (float)(1.0 - u1 - 2.0 * u2) * ipn;
+        s_par[5][loc] = (float)(u1 + 2.0 * u2) * ipn;
+        s_par[6][loc] = (float)u2 * ipn;
+        slot[q] = atomicAdd(&s_count[4 - path[q]], 1);   // list 0 = path 4 (the long one first)
     }
     __syncthreads();
     if (tid == 0) {
-        s_start[0] = 0;
-        s_start[1] = s_count[0];
-        s_start[2] = s_count[0] + s_count[1];
+        int run = 0;
+        for (int l = 0; l < 4; ++l) {
+            s_start[l] = run;
+            run += s_count[l];
+        }
+        s_start[4] = run;
     }
     __syncthreads();
 #pragma unroll
     for (int q = 0; q < GEO_PER; ++q)
-        if (bin[q] >= 0) s_order[s_start[bin[q]] + slot[q]] = (short)(q * GEO_NT + tid);
+        if (path[q] > 0) s_ord[s_start[4 - path[q]] + slot[q]] = (unsigned short)(q * GEO_NT + tid);
     __syncthreads();
-    const int total = s_start[2] + s_count[2];
-    for (int j = tid; j < total; j += GEO_NT) {
-        const int loc = s_order[j];
-        const float delta = glf::blocked_f32<true>(s_trap, s_par[0][loc], s_par[1][loc], s_par[2][loc],
-                                             s_par[3][loc], s_par[4][loc], s_par[5][loc], s_par[6][loc]);
-        out[base + loc] = 1.f - delta;
+    const int n_near = s_start[1], n_all = s_start[4];
+    // ---- stage 2: fixed-node rules (lists 1..3 = paths 3, 2, 1)
+    for (int j = n_near + tid; j < n_all; j += GEO_NT) {
+        const int loc = s_ord[j];
+        const int pth = j < s_start[2] ? 3 : (j < s_start[3] ? 2 : 1);
+        const float xc = s_par[0][loc], yc = s_par[1][loc], a = s_par[2][loc], b = s_par[3][loc];
+        const float delta = glh::cheap_delta(s_trap, pth, xc, yc, fmaf(xc, xc, yc * yc), a, b, a * b, s_par[4][loc],
+                                             s_par[5][loc], s_par[6][loc]);
+        out[row_of(loc)] = 1.f - delta;
+    }
+    // ---- stage 3: near-limb rows: which of them need the generic search, farthest point of the others
+    for (int j = tid; j < n_near; j += GEO_NT) {
+        const int loc = s_ord[j];
+        const float xc = s_par[0][loc], yc = s_par[1][loc], a = s_par[2][loc], b = s_par[3][loc];
+        const float e2 = (a - b) * (a + b), Aa = a * xc, Bb = b * yc;
+        int lst;
+        if (Aa < e2 && Bb < e2 && glf::evolute_inside(Aa, Bb, e2)) {
+            // the generic bracketed search is ~10x longer than anything else here: left to
+            // geometry_evolute_kernel, which gathers these rows from the whole grid into full warps
+            out[row_of(loc)] = __uint_as_float(glh::MARK_BITS);
+            s_ord2[j] = 0xffffu;
+            continue;
+        } else {
+            const float rn = glf::mufu_rsqrt(fmaf(Aa, Aa, Bb * Bb));
+            float cf = Aa * rn, sf = Bb * rn;
+            glh::critical_point_rt(xc, yc, a, b, 1.f, &cf, &sf);
+            s_far[0][loc] = cf;
+            s_far[1][loc] = sf;
+            const float xf = fmaf(a, cf, xc), yf = fmaf(b, sf, yc);
+            lst = fmaf(xf, xf, fmaf(yf, yf, -1.f)) <= 0.f ? 1 : 0;
+        }
+        const int sl = atomicAdd(&s_count2[lst], 1);
+        // (positions inside a list are final only after the counts are: keep (list, slot) in s_ord2 for now)
+        s_ord2[j] = (unsigned short)((lst << 12) | sl);
+    }
+    __syncthreads();
+    if (tid == 0) {
+        s_start2[0] = 0;
+        s_start2[1] = s_count2[0];
+        s_start2[2] = s_count2[0] + s_count2[1];
+        s_start2[3] = s_count2[0] + s_count2[1] + s_count2[2];
+    }
+    __syncthreads();
+    // scatter the row numbers to their final positions (through registers: s_ord2 is rewritten in place)
+    {
+        int locs[GEO_PER], poss[GEO_PER];
+#pragma unroll
+        for (int q = 0; q < GEO_PER; ++q) {
+            const int j = q * GEO_NT + tid;
+            poss[q] = -1;
+            locs[q] = 0;
+            if (j < n_near && s_ord2[j] != 0xffffu) {
+                const int code = s_ord2[j];
+                poss[q] = s_start2[code >> 12] + (code & 0xfff);
+                locs[q] = s_ord[j];
+            }
+        }
+        __syncthreads();
+#pragma unroll
+        for (int q = 0; q < GEO_PER; ++q)
+            if (poss[q] >= 0) s_ord2[poss[q]] = (unsigned short)locs[q];
+    }
+    __syncthreads();
+    // ---- stage 4: two crossings / inside near the limb (evolute rows: geometry_evolute_kernel)
+    const int n_stage4 = s_start2[2];
+    for (int j = tid; j < n_stage4; j += GEO_NT) {
+        const int loc = s_ord2[j];
+        const float xc = s_par[0][loc], yc = s_par[1][loc], a = s_par[2][loc], b = s_par[3][loc];
+        const float Aa = a * xc, Bb = b * yc;
+        const float rn = glf::mufu_rsqrt(fmaf(Aa, Aa, Bb * Bb));
+        const float delta = glh::near_rest<false>(s_trap, xc, yc, fmaf(xc, xc, yc * yc), a, b, a * b,
+                                                  (a - b) * (a + b), s_par[4][loc], s_par[5][loc], s_par[6][loc],
+                                                  s_far[0][loc], s_far[1][loc], -(Aa * rn), -(Bb * rn), 0,
+                                                  0xffffffffu);
+        out[row_of(loc)] = 1.f - delta;
+    }
+}
+
+// Second launch of the fp32 bare-geometry call (programmatic dependent launch behind
+// geometry_sorted_kernel): the rows that kernel marked -- star centre possibly inside the outline's
+// evolute: up to four crossings, generic bracketed search (gl_core.cuh) -- gathered from EVO_ROWS rows of
+// the output into one list per CTA and evaluated with full warps.
+constexpr int EVO_NT = 256, EVO_ROWS = 2048;   // rows looked at per round of a CTA
+__global__ void __launch_bounds__(EVO_NT)
+geometry_evolute_kernel(const double* __restrict__ geom, long long N, float* out) {
+    __shared__ long long s_rows[EVO_ROWS];
+    __shared__ int s_n;
+    const int tid = threadIdx.x;
+    asm volatile("griddepcontrol.wait;" ::: "memory");
+    // blocks of 32 rows, round-robin over the CTAs (see geometry_sorted_kernel); a CTA looks at EVO_ROWS
+    // rows per round, lists the marked ones and evaluates them
+    const long long nblocks = (N + 31) / 32;
+    for (long long b0 = blockIdx.x; b0 < nblocks; b0 += (long long)gridDim.x * (EVO_ROWS / 32)) {
+        __syncthreads();
+        if (tid == 0) s_n = 0;
+        __syncthreads();
+        for (int r = tid; r < EVO_ROWS; r += EVO_NT) {
+            const long long blk = b0 + (long long)(r >> 5) * gridDim.x;
+            const long long k = blk * 32 + (r & 31);
+            if (blk < nblocks && k < N && *reinterpret_cast<const volatile uint32_t*>(out + k) == glh::MARK_BITS)
+                s_rows[atomicAdd(&s_n, 1)] = k;
+        }
+        __syncthreads();
+        const int n = s_n;
+        for (int j = tid; j < n; j += EVO_NT) {
+            const long long k = s_rows[j];
+            const double* g = geom + k * GL_NGEOM;
+            const double d = g[0], Rp = g[1], fp = g[2], pa = g[3], u1 = g[4], u2 = g[5];
+            float s, c;
+            glh::angle_sincos(pa, &s, &c);   // (the same preparation as geometry_sorted_kernel)
+            const float a = (float)Rp, b = (float)(Rp * (1.0 - fp)), r0 = (float)d;
+            const float ipn = glh::rcp_nr((float)(kPi * (1.0 - u1 / 3.0 - u2 / 6.0)));
+            float A[3];
+            float delta = 0.f;
+            if (glc::overlap_areas<float, 16, true>(fabsf(r0 * c), fabsf(r0 * s), a, b, glf::c_gl_phi, glf::c_gl_om, A))
+                delta = fmaf((float)(1.0 - u1 - 2.0 * u2) * ipn, A[0],
+                             fmaf((float)(u1 + 2.0 * u2) * ipn, A[1], (float)u2 * ipn * A[2]));
+            out[k] = 1.f - delta;
+        }
     }
 }
 
@@ -1311,10 +1445,27 @@ int gl_flux_geometry(const double* geom, long long N, void* flux_out, gl_dtype d
     if (rc != GL_OK) return rc;
     const unsigned blocks = (unsigned)((N + NT - 1) / NT);
     cudaStream_t st = (cudaStream_t)stream;
-    if (dtype == GL_F32)
-        geometry_binned_kernel<<<(unsigned)((N + GEO_ROWS - 1) / GEO_ROWS), GEO_NT, 0, st>>>(
+    if (dtype == GL_F32) {
+        geometry_sorted_kernel<<<(unsigned)((N + GEO_ROWS - 1) / GEO_ROWS), GEO_NT, 0, st>>>(
             geom, N, (float*)flux_out);
-    else
+        cudaError_t e1 = cudaGetLastError();
+        if (e1 != cudaSuccess) return cuda_fail(e1, "geometry_sorted_kernel launch");
+        ++tl_launches;
+        cudaLaunchConfig_t cfg = {};
+        {   // as many CTAs as keep every SM busy, but no more than there are rounds of EVO_ROWS rows
+            const long long want = (N + EVO_ROWS - 1) / EVO_ROWS, room = (long long)sm_count() * 4;
+            cfg.gridDim = dim3((unsigned)(want < room ? want : room), 1, 1);
+        }
+        cfg.blockDim = dim3(EVO_NT, 1, 1);
+        cfg.stream = st;
+        cudaLaunchAttribute attr[1];
+        attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+        attr[0].val.programmaticStreamSerializationAllowed = 1;
+        cfg.attrs = attr;
+        cfg.numAttrs = 1;
+        e1 = cudaLaunchKernelEx(&cfg, geometry_evolute_kernel, geom, N, (float*)flux_out);
+        if (e1 != cudaSuccess) return cuda_fail(e1, "geometry_evolute_kernel launch");
+    } else
         geometry_kernel<double><<<blocks, NT, 0, st>>>(geom, N, (double*)flux_out);
     cudaError_t e = cudaGetLastError();
     if (e != cudaSuccess) return cuda_fail(e, "geometry_kernel launch");
