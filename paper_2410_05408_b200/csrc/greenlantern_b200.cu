@@ -840,9 +840,7 @@ geometry_kernel(const double* __restrict__ geom, long long N, T* __restrict__ ou
     if (threadIdx.x < 16)
         s_trap[threadIdx.x] = glf::TrapNode{glf::c_trap_cos[threadIdx.x], glf::c_trap_sin[threadIdx.x]};
     __syncthreads();
-    // blocks of 32 rows dealt round-robin to the CTAs (a stretch of expensive rows -- config 5 ends with
-    // 100 000 forced ones -- is spread over the grid; see geometry_sorted_kernel)
-    const long long k = ((long long)(threadIdx.x >> 5) * gridDim.x + blockIdx.x) * 32 + (threadIdx.x & 31);
+    const long long k = (long long)blockIdx.x * NT + threadIdx.x;
     if (k >= N) return;
     const double* g = geom + k * GL_NGEOM;
     const double d = g[0], Rp = g[1], fp = g[2], pa = g[3], u1 = g[4], u2 = g[5];
