@@ -100,7 +100,7 @@ class ClockSampler:
         try:
             self.proc = subprocess.Popen(
                 ["nvidia-smi", f"--id={self.index}", f"--query-gpu={self.Q}",
-                 "--format=csv,noheader,nounits", "-lms", "50"],
+                 "--format=csv,noheader,nounits", "-lms", "100"],
                 stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
             self.thread = threading.Thread(target=self._read, daemon=True)
             self.thread.start()
@@ -226,9 +226,12 @@ def main():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-extra", action="store_true")
     ap.add_argument("--dry", action="store_true", help="multi-rank plumbing only (gloo, no GPU)")
+    ap.add_argument("--profile", default=None, help="run one named call five times and exit (for ncu)")
     args = ap.parse_args()
     if args.impl == "reference":
         return run_reference(args)
+    if args.profile:
+        return run_profile(args)
     if "WORLD_SIZE" not in os.environ and args.gpus > 1:
         raise SystemExit(spawn_ranks(args))
     world = int(os.environ.get("WORLD_SIZE", "1"))
@@ -264,6 +267,8 @@ def main():
         """CUDA events around each of k calls on torch's current stream (the launching stream); L2
         flushed before each call (cold) or a spinning spacer kernel instead (warm L2, context)."""
         for _ in range(warm):
+            if cold:
+                flush.zero_()
             fn()
         torch.cuda.synchronize()
         ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(k)]
@@ -287,14 +292,17 @@ def main():
     def step():
         ser.loglike_dev(P, want_flux=True, chi2_out=chi2_d, flux_out=flux_d)
 
-    for _ in range(W):
-        step()
+    step()
     torch.cuda.synchronize()
     n_in_exposures = int((flux_d < 1.0).sum().item())
-    launches0 = gl.gl_launch_count()
     sampler = ClockSampler(local)
     sampler.start()
-    time.sleep(0.15)
+    time.sleep(0.5)                # nvidia-smi is up and sampling before anything is timed
+    for _ in range(W):             # W untimed warm-up steps, in the timed loop's own rhythm (flush, step)
+        flush.zero_()
+        step()
+    torch.cuda.synchronize()
+    launches0 = gl.gl_launch_count()
     barrier()
     wall0 = time.perf_counter()
     dev_ms = timed(step, warm=0)
@@ -399,6 +407,8 @@ def main():
                    "api": "gl_series_loglike_dev (series resident, parameter rows resident)",
                    "l2": "256 MiB flush between timed iterations", "parallelism": f"dp{world} over walkers"},
         "subsample_evals_per_s": value * w.n_ss,
+        "ms_per_step_median": float(np.median(dev_ms)), "ms_per_step_min": float(np.min(dev_ms)),
+        "ms_per_step_max": float(np.max(dev_ms)),
         "wall_ms_per_step_incl_flush": 1e3 * wall / K,
         "clocks": clocks, "gpu_launches": int(launches),
         "e2e": {"value": evals_per_step / e2e_s, "unit": UNIT, "h2d_bytes_per_step": h2d,
@@ -424,55 +434,91 @@ def main():
         dist.destroy_process_group()
 
 
-def extra_workloads(gl, dev, d, timed, fractions, peak_tflops, probe, ncu, w3, ser3, P3):
-    """The secondary numbers, timed like the headline (CUDA events, L2 flushed, inputs resident), so that
-    the driver's run carries them: each with ms, units/s and both roofline fractions where they apply."""
+def secondary_calls(gl, dev, d, w3, ser3, P3):
+    """name -> (callable that enqueues one call, units per call, unit name, keep-alive objects) for the
+    workloads beside the headline: used by `extra` (timed) and by --profile (run a few times under ncu)."""
     import torch
-    ex = {}
-    k = 20
-    # the stateless entry point on the headline workload: baseline_kernel + hot_kernel + fallback
+    calls = {}
     T3, O3, S3 = d(w3.times), d(w3.obs), d(w3.sigma)
-    ms = float(np.mean(timed(lambda: gl.gl_loglike(P3, T3, w3.t_exp, w3.n_ss, O3, S3, dtype="f32", want_flux=True), k=k)))
-    ex["cfg3_gl_loglike_stateless"] = {"ms": ms, "flux_evals_per_s": w3.B * w3.T / (ms * 1e-3), "launches_per_step": 3}
     chi2_only = torch.empty(w3.B, dtype=torch.float32, device=dev)
-    ms = float(np.mean(timed(lambda: ser3.loglike_dev(P3, chi2_out=chi2_only), k=k)))
-    ex["cfg3_chi2_only"] = {"ms": ms, "flux_evals_per_s": w3.B * w3.T / (ms * 1e-3)}
-    # cfg3 in fp64 (validation path: the full kernel)
-    ms = float(np.mean(timed(lambda: gl.gl_loglike(P3, T3, w3.t_exp, w3.n_ss, O3, S3, dtype="f64", want_flux=True), k=5, warm=2)))
-    ex["cfg3_fp64"] = {"ms": ms, "flux_evals_per_s": w3.B * w3.T / (ms * 1e-3), "dtype": "f64",
-                       "dfma_chain_tflops": probe["fp64_tflops"],
-                       "executed_fp64_flop_ncu": ncu.get("executed_fp64_flop", {}).get("cfg3_fp64")}
-    if ex["cfg3_fp64"]["executed_fp64_flop_ncu"]:
-        ex["cfg3_fp64"]["frac_executed_of_dfma_chain"] = (ex["cfg3_fp64"]["executed_fp64_flop_ncu"] / (ms * 1e-3) / 1e12
-                                                          / probe["fp64_tflops"])
-    # cfg4: JWST-shaped batch, chi2 + flux
+    calls["cfg3_gl_loglike_stateless"] = (
+        lambda: gl.gl_loglike(P3, T3, w3.t_exp, w3.n_ss, O3, S3, dtype="f32", want_flux=True), w3.B * w3.T, "flux_evals")
+    calls["cfg3_chi2_only"] = (lambda: ser3.loglike_dev(P3, chi2_out=chi2_only), w3.B * w3.T, "flux_evals")
+    calls["cfg3_fp64"] = (
+        lambda: gl.gl_loglike(P3, T3, w3.t_exp, w3.n_ss, O3, S3, dtype="f64", want_flux=True), w3.B * w3.T, "flux_evals")
+    gp3 = d(np.tile([2e-4, 0.5, 1e-4], (w3.B, 1)))
+    calls["cfg3_gp_loglike"] = (
+        lambda: gl.gl_gp_loglike(P3, T3, w3.t_exp, w3.n_ss, O3, S3, gp3, dtype="f32"), w3.B * w3.T, "flux_evals")
     w4 = wl.config4()
     ser4 = gl.GlSeries(w4.times, w4.obs, w4.sigma, w4.t_exp, w4.n_ss, w4.B, device=dev)
     P4 = d(w4.params)
     c4 = torch.empty(w4.B, dtype=torch.float32, device=dev)
     f4 = torch.empty((w4.B, w4.T), dtype=torch.float32, device=dev)
-    ms = float(np.mean(timed(lambda: ser4.loglike_dev(P4, want_flux=True, chi2_out=c4, flux_out=f4), k=k)))
-    n_in, n_limb = in_transit_mix(w4)
-    ex["cfg4"] = {"ms": ms, "flux_evals_per_s": w4.B * w4.T / (ms * 1e-3), "B": w4.B, "T": w4.T, "n_ss": w4.n_ss,
-                  "in_transit_subsamples": n_in, "of_which_limb_crossing": n_limb, **fractions("cfg4", n_in, n_limb, ms)}
-    ser4.close()
-    del f4
-    # cfg5: 1e6 bare geometries, fp32
+    calls["cfg4"] = (lambda: ser4.loglike_dev(P4, want_flux=True, chi2_out=c4, flux_out=f4), w4.B * w4.T, "flux_evals")
     geom, _ = wl.config5()
     G = d(geom)
-    ms = float(np.mean(timed(lambda: gl.gl_flux_geometry(G, dtype="f32"), k=k)))
-    ex["cfg5"] = {"ms": ms, "geometries_per_s": geom.shape[0] / (ms * 1e-3), "N": int(geom.shape[0]),
-                  "active_lanes_per_instruction_ncu": ncu.get("active_lanes", {}).get("cfg5")}
-    # one light curve of 1e5 exposures, flux only: the shape of the paper's Fig. 6 (PAPER.md:171, :183)
+    calls["cfg5"] = (lambda: gl.gl_flux_geometry(G, dtype="f32"), geom.shape[0], "geometries")
+    G1 = d(geom[-200_000:])          # (the last 10^5 of these are the forced rows)
+    calls["cfg5_fp64_200k"] = (lambda: gl.gl_flux_geometry(G1, dtype="f64"), 200_000, "geometries")
+    G2 = d(geom[:20_000])
+    calls["simpson_fp32_20k_x4096"] = (lambda: gl.gl_flux_geometry_simpson(G2, 4096, dtype="f32"), 20_000, "geometries")
     T1 = 100_000
     t1 = d(np.linspace(-0.6, 0.6, T1))
     p1 = d(wl.CFG2_ROW[None, :])
     f1 = torch.empty((1, T1), dtype=torch.float32, device=dev)
-    ms = float(np.mean(timed(lambda: gl.gl_lightcurve(p1, t1, 0.0, 1, dtype="f32", out=f1), k=k)))
-    ex["single_lightcurve_T1e5"] = {"ms": ms, "us_per_flux_sample": ms * 1e3 / T1, "flux_evals_per_s": T1 / (ms * 1e-3),
-                                    "paper": "about 0.5 us per sample at 1e4-1e5 samples on a Quadro RTX 5000 "
-                                             "(PAPER.md:171; another machine: context)"}
+    calls["single_lightcurve_T1e5"] = (lambda: gl.gl_lightcurve(p1, t1, 0.0, 1, dtype="f32", out=f1), T1, "flux_evals")
+    return calls, {"w4": w4, "ser4": ser4}
+
+
+def extra_workloads(gl, dev, d, timed, fractions, peak_tflops, probe, ncu, w3, ser3, P3):
+    """The secondary numbers, timed like the headline (CUDA events, L2 flushed, inputs resident), so that
+    the driver's run carries them: each with ms, units/s and both roofline fractions where they apply."""
+    calls, keep = secondary_calls(gl, dev, d, w3, ser3, P3)
+    ex = {}
+    for name, (fn, units, unit) in calls.items():
+        slow = name in ("cfg3_fp64", "cfg5_fp64_200k", "simpson_fp32_20k_x4096")
+        ms = float(np.mean(timed(fn, k=5 if slow else 20, warm=2 if slow else 3)))
+        ex[name] = {"ms": ms, f"{unit}_per_s": units / (ms * 1e-3)}
+    ex["cfg3_gl_loglike_stateless"]["launches_per_step"] = 3
+    ex["cfg3_fp64"].update({"dtype": "f64", "dfma_chain_tflops": probe["fp64_tflops"]})
+    exf = ncu.get("executed_fp64_flop", {}).get("cfg3_fp64")
+    if exf:
+        ex["cfg3_fp64"]["executed_fp64_flop_ncu"] = exf
+        ex["cfg3_fp64"]["frac_executed_of_dfma_chain"] = exf / (ex["cfg3_fp64"]["ms"] * 1e-3) / 1e12 / probe["fp64_tflops"]
+    w4 = keep["w4"]
+    n_in, n_limb = in_transit_mix(w4)
+    ex["cfg4"].update({"B": w4.B, "T": w4.T, "n_ss": w4.n_ss, "in_transit_subsamples": n_in,
+                       "of_which_limb_crossing": n_limb, **fractions("cfg4", n_in, n_limb, ex["cfg4"]["ms"])})
+    ex["cfg5"]["active_lanes_per_instruction_ncu"] = ncu.get("active_lanes", {}).get("cfg5")
+    ex["single_lightcurve_T1e5"].update({
+        "us_per_flux_sample": ex["single_lightcurve_T1e5"]["ms"] * 1e3 / 100_000,
+        "paper": "about 0.5 us per sample at 1e4-1e5 samples on a Quadro RTX 5000 (PAPER.md:171; another "
+                 "machine: context)"})
+    keep["ser4"].close()
     return ex
+
+
+def run_profile(args):
+    """--profile NAME: the named call five times and nothing else (a short command for ncu)."""
+    import torch
+    import paper_2410_05408_b200 as gl
+    dev = torch.device("cuda", 0)
+    torch.cuda.set_device(0)
+    gl.load_library()
+    d = lambda x: torch.as_tensor(np.ascontiguousarray(x, dtype=np.float64), device=dev)  # noqa: E731
+    w = make_workload("cfg3", 0)
+    P = d(w.params)
+    ser = gl.GlSeries(w.times, w.obs, w.sigma, w.t_exp, w.n_ss, w.B, device=dev)
+    chi2_d = torch.empty(w.B, dtype=torch.float32, device=dev)
+    flux_d = torch.empty((w.B, w.T), dtype=torch.float32, device=dev)
+    calls, keep = secondary_calls(gl, dev, d, w, ser, P)
+    calls["cfg3"] = (lambda: ser.loglike_dev(P, want_flux=True, chi2_out=chi2_d, flux_out=flux_d), w.B * w.T, "flux_evals")
+    if args.profile not in calls:
+        raise SystemExit(f"--profile: one of {sorted(calls)}")
+    for _ in range(5):
+        calls[args.profile][0]()
+    torch.cuda.synchronize()
+    print(json.dumps({"profile": args.profile, "calls": 5}))
 
 
 if __name__ == "__main__":
