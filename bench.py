@@ -367,9 +367,8 @@ def main():
     n_in, n_limb = in_transit_mix(w)
     fr = fractions(args.workload, n_in, n_limb, k_ms)
     hs = (1, w.B, 512)               # hot_kernel's launch shape for this batch: (cluster, rows, threads)
-    floor_pair = float(np.mean(timed(lambda: gl.gl_probe_empty_launch(hs[0], hs[1], hs[2], 4, min(w.B, 148)),
-                                     k=max(K, 20))))
-    floor_one = float(np.mean(timed(lambda: gl.gl_probe_empty_launch(hs[0], hs[1], hs[2]), k=max(K, 20))))
+    floor_graph = float(np.mean(timed(lambda: gl.gl_probe_empty_graph(hs[0], hs[1], hs[2]), k=max(K, 20))))
+    floor_stream = float(np.mean(timed(lambda: gl.gl_probe_empty_launch(hs[0], hs[1], hs[2]), k=max(K, 20))))
     roofline = {
         "bound": "alu", "achieved": fr["alg_tflops"], "peak": peak_tflops, "unit": "TFLOP/s",
         "frac": fr["frac_alg"],
@@ -382,12 +381,12 @@ def main():
         "traffic_source": f"dram__bytes_read.sum + dram__bytes_write.sum of one hot_kernel launch, ncu --set full "
                           f"at commit {ncu.get('commit')} (profiles/r02_kernels.md); the path is ALU/latency-bound, "
                           "algorithmic HBM bytes are B*96 in, B*T*4 + B*4 out",
-        "kernel": "glh::hot_kernel<true> (+ transit_kernel in marker mode behind it: exits at once when no "
-                  "walker was deferred)",
+        "kernel": "glh::hot_kernel<true> (one launch per step, replayed as a CUDA graph)",
         "kernel_ms": k_ms, "kernel_ms_warm_l2": warm_ms,
-        "launch_floor_ms": floor_pair, "launch_floor_single_kernel_ms": floor_one,
-        "launch_floor_note": "EMPTY kernels of the same grid/block shapes (hot + dependent fallback pair; one "
-                             "kernel alone), timed exactly like a step, L2 flushed",
+        "launch_floor_ms": floor_graph, "launch_floor_stream_launch_ms": floor_stream,
+        "launch_floor_note": "an EMPTY kernel of hot_kernel's grid/block shape, replayed as a CUDA graph the way "
+                             "a step is (and launched on the stream, for comparison), timed exactly like a step, "
+                             "L2 flushed",
         "peak_source": f"derived: {N_SM} SMs x {LANES} FP32 lanes x 2 x {sm_max:.0f} MHz "
                        "(MEASURED_PEAKS.json has no FP32 SIMT figure)",
         "peak_measured_ffma_chain": probe["fp32_tflops"],
@@ -479,7 +478,7 @@ def extra_workloads(gl, dev, d, timed, fractions, peak_tflops, probe, ncu, w3, s
         slow = name in ("cfg3_fp64", "cfg5_fp64_200k", "simpson_fp32_20k_x4096")
         ms = float(np.mean(timed(fn, k=5 if slow else 20, warm=2 if slow else 3)))
         ex[name] = {"ms": ms, f"{unit}_per_s": units / (ms * 1e-3)}
-    ex["cfg3_gl_loglike_stateless"]["launches_per_step"] = 3
+    ex["cfg3_gl_loglike_stateless"]["launches_per_step"] = 2
     ex["cfg3_fp64"].update({"dtype": "f64", "dfma_chain_tflops": probe["fp64_tflops"]})
     exf = ncu.get("executed_fp64_flop", {}).get("cfg3_fp64")
     if exf:

@@ -74,8 +74,8 @@ typedef enum {
  *   flux_out [B, T] row-major, float (GL_F32) or double (GL_F64) (device), fully overwritten.
  * Steps: Kepler + sky position (eqs. 9-10, R7), outline (PAPER.md:89-96
  * eqs. 11-13), outline/limb crossings (R3), boundary integrals (eqs. 21-23),
- * exposure mean -- fused, nothing per-sub-sample is stored (GL_F32: hot_kernel + the full kernel for the
- * walkers it defers, see gl_loglike; GL_F64: the full kernel). */
+ * exposure mean -- one fused launch, nothing per-sub-sample is stored (GL_F32: hot_kernel, see gl_loglike;
+ * GL_F64: the full kernel). */
 int gl_lightcurve(const double* params, int B, const double* times, int T, double t_exp, int n_ss,
                   void* flux_out, gl_dtype dtype, void* stream);
 
@@ -85,13 +85,13 @@ int gl_lightcurve(const double* params, int B, const double* times, int T, doubl
  *   flux_out_or_null: optional [B, T] output as in gl_lightcurve; NULL => the model flux never
  *   leaves registers.  The residual sum is accumulated in fp64 in both dtypes.
  *   GL_F64: one launch of the full transit kernel, everything per walker in fp64.
- *   GL_F32 (12-column rows): THREE launches on `stream`, chained by programmatic dependent launch:
+ *   GL_F32 (12-column rows): TWO launches on `stream`, chained by programmatic dependent launch:
  *   (1) a one-CTA kernel forms the walker-independent part S = sum_i ((obs_i - 1)/sigma_i)^2 once;
- *   (2) hot_kernel finishes every walker on the common path (circular orbit, short transit window,
- *   sorted series, outline that can cross the limb at most twice): in-window exposures found as index
- *   ranges, chi^2 = S + sum over them of d (2 o r + d), o = obs - 1, r = 1/sigma, d = (1 - F) r, in
- *   fp32 terms summed in fp64; every other walker is left marked in its output slot;
- *   (3) the full transit kernel redoes exactly the marked walkers (it exits at once if there are none).
+ *   (2) hot_kernel: walkers on the common path (circular orbit, short transit window, sorted series,
+ *   outline that can cross the limb at most twice) get their in-window exposures as index ranges and
+ *   chi^2 = S + sum over them of d (2 o r + d), o = obs - 1, r = 1/sigma, d = (1 - F) r, in fp32 terms
+ *   summed in fp64; every other walker runs, inside the same launch, the full-featured arithmetic of
+ *   the fp64 kernel in fp32 (fp64 phases, Kepler's equation, four-crossing search).
  *   A caller that evaluates many batches against one series should use gl_series_* below, which does
  *   (1) once per series. */
 int gl_loglike(const double* params, int B, const double* times, int T, double t_exp, int n_ss,
@@ -193,13 +193,10 @@ int gl_flux_geometry_host(const double* geom, long long N, void* flux_out, gl_dt
  *   values as gl_loglike(GL_F32) up to the rounding of S (kept in fp64 here, narrowed there).
  * gl_series_loglike_dev: params, chi2_out, flux_out_or_null are DEVICE pointers; work is enqueued on
  *   `stream` without synchronising (the series buffers are only read, so several streams may use
- *   one handle through this call as long as the handle outlives the work).  The launch pair is
+ *   one handle through this call as long as the handle outlives the work).  The launch is
  *   captured once per distinct (params, B, chi2_out, flux_out_or_null) -- the last four are kept --
  *   and replayed as a CUDA graph: a sampler that reuses its buffers pays one graph launch per step.
- * Launches per call: hot_kernel (walkers on the common path: circular orbit, n_ss <= 32, sorted
- * series, at most two limb crossings) followed, by programmatic dependent launch, by the full
- * transit kernel for the walkers the first one deferred.  The host call launches the second kernel
- * only when the previous call needed it (or, failing that, after the first has reported so). */
+ * Launches per call: ONE (hot_kernel, see gl_loglike; the per-series kernel ran at creation). */
 typedef struct gl_series gl_series;
 int gl_series_create(const double* times, const double* obs, const double* sigma, int T, double t_exp,
                      int n_ss, int B_max, gl_series** out);
@@ -219,11 +216,14 @@ int gl_probe_peaks(double* out3);
 
 /* gl_probe_empty_launch: enqueues an EMPTY kernel of `rows` clusters of `cluster` CTAs of `threads`
  * threads on `stream` and, when fallback_rows > 0, a second empty grid (fallback_rows clusters of
- * fallback_cluster CTAs of 128 threads) chained to it by programmatic dependent launch -- the launch
- * shapes of a gl_loglike / gl_series_loglike_dev step without their work.  bench.py times it the way
+ * fallback_cluster CTAs of 128 threads) chained to it by programmatic dependent launch -- launch
+ * shapes of the library's calls without their work.  bench.py times it the way
  * it times a step and reports it as roofline.launch_floor_ms.  Not part of the hot path. */
 int gl_probe_empty_launch(int cluster, int rows, int threads, int fallback_cluster, int fallback_rows,
                           void* stream);
+/* gl_probe_empty_graph: the same single empty kernel, captured once per shape (and calling thread) and
+ * replayed as a CUDA graph on `stream` -- the way gl_series_loglike_dev launches a step. */
+int gl_probe_empty_graph(int cluster, int rows, int threads, void* stream);
 
 /* Number of kernel launches the calling thread's entry points have enqueued so far (HOST). */
 long long gl_launch_count(void);

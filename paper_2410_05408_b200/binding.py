@@ -19,7 +19,7 @@ _lib = None
 EXPORTS = ("gl_lightcurve", "gl_loglike", "gl_lightcurve_ex", "gl_loglike_ex", "gl_params_from_munu", "gl_munu_from_uniform", "gl_gp_loglike", "gl_flux_geometry", "gl_flux_geometry_simpson", "gl_lightcurve_host",
            "gl_loglike_host", "gl_flux_geometry_host", "gl_series_create", "gl_series_loglike",
            "gl_series_loglike_dev", "gl_series_info", "gl_series_destroy", "gl_probe_peaks",
-           "gl_probe_empty_launch", "gl_launch_count", "gl_strerror",
+           "gl_probe_empty_launch", "gl_probe_empty_graph", "gl_launch_count", "gl_strerror",
            "gl_last_cuda_error", "gl_version")
 
 
@@ -68,6 +68,8 @@ def load_library():
         getattr(lib, name).restype = i
     lib.gl_probe_empty_launch.argtypes = [i, i, i, i, i, vp]
     lib.gl_probe_empty_launch.restype = i
+    lib.gl_probe_empty_graph.argtypes = [i, i, i, vp]
+    lib.gl_probe_empty_graph.restype = i
     lib.gl_probe_peaks.argtypes = [vp]
     lib.gl_probe_peaks.restype = i
     lib.gl_launch_count.restype = ll
@@ -380,6 +382,14 @@ def gl_probe_empty_launch(cluster, rows, threads, fallback_cluster=1, fallback_r
     st = ctypes.c_void_p(torch.cuda.current_stream(dev).cuda_stream)
     _check(load_library().gl_probe_empty_launch(int(cluster), int(rows), int(threads), int(fallback_cluster),
                                                 int(fallback_rows), st))
+
+
+def gl_probe_empty_graph(cluster, rows, threads, device=None):
+    """The empty kernel of gl_probe_empty_launch replayed as a CUDA graph on torch's current stream."""
+    torch = _torch()
+    dev = torch.device("cuda", torch.cuda.current_device()) if device is None else device
+    st = ctypes.c_void_p(torch.cuda.current_stream(dev).cuda_stream)
+    _check(load_library().gl_probe_empty_graph(int(cluster), int(rows), int(threads), st))
 
 
 def gl_launch_count():

@@ -1,14 +1,13 @@
-// gl_hot.cuh -- hot_kernel: the COMMON path of the fused fp32 transit kernel and nothing else
-// (DESIGN.md 5.4).  A walker is "simple" when its orbit is circular (eqs. 9-10 as
-// printed), its transit window is short (|phi| <= 0.8 rad), at most MAXEP transits fall inside the
-// series, the star centre can never lie inside the outline's evolute while the outline is near the
-// limb (so the outline crosses the limb at most twice), and the series is sorted.  Simple walkers are
-// finished here; every other walker is DEFERRED: the kernel leaves a marker (a NaN with a payload) in
-// the walker's output slot and the full-featured transit_kernel, launched right behind with
-// programmatic dependent launch, redoes exactly the marked walkers.  Invalid walkers (NaN row,
-// chi^2 = +inf) are finished here too.
+// gl_hot.cuh -- hot_kernel: the fp32 transit kernel, built around the COMMON path.
+// A walker is "simple" when its orbit is circular (eqs. 9-10 as printed), its transit
+// window is short (|phi| <= 0.8 rad), at most MAXEP transits fall inside the series, the star centre can
+// never lie inside the outline's evolute while the outline is near the limb (so the outline crosses the
+// limb at most twice), and the series is sorted.  Simple walkers take the path described below; every
+// other walker is handed, inside the same launch, to generic_unit() -- the full-featured arithmetic of
+// greenlantern_b200.cu (fp64 phases, Kepler, four-crossing search) as a NON-inlined device function:
+// its code is only fetched when a walker needs it.  Invalid walkers: NaN row, chi^2 = +inf.
 //
-// Why a separate kernel: the full-featured kernel is ~340 KB of SASS (fp64 Kepler, the
+// Why a kernel of its own: round 1's single fused kernel inlined everything -- ~340 KB of SASS (fp64 Kepler, the
 // four-crossing search, libm slow paths); on a K2-shaped batch (config 3) it spent its time in
 // instruction fetch and barriers, not arithmetic (profiles/r01_v5.md).  This one has no fp64
 // arithmetic beyond the epoch bookkeeping of the prelude, the time difference t_i - t_c and the
@@ -72,7 +71,6 @@ constexpr int HOT_NW = HOT_NT / 32;
 constexpr int MAXEP = 8;              // transit epochs of one walker inside one series segment
 constexpr int MAXC = 8;               // CTAs per cluster (portable limit)
 constexpr int CAP = 2 * HOT_NT;       // (exposure, sub-exposure) pairs of the sparse mode
-constexpr uint32_t MARK_BITS = 0x7fc0deadu;   // "deferred": a quiet NaN no arithmetic here produces
 
 // cos, sin of pi k / 16, k = 0..15 (glf::whole_outline_lin's table), statically initialised.
 __constant__ float2 c_trap16[16] = {
@@ -425,7 +423,6 @@ struct HotArgs {
     const float2* ow;       // [T]  (obs - 1, 1/sigma) in fp32 (PRE = true: gl_series)
     float* flux;            // [B, T] or nullptr
     float* chi2;            // [B] or nullptr
-    int* status;            // nullptr, or a word that is set to 1 when any unit is deferred
     double S;               // PRE: baseline sum_i ((obs_i - 1)/sigma_i)^2
     double t_exp;
     float inv_ss, doff, off0;   // 1/n_ss, t_exp/n_ss, (0.5/n_ss - 0.5) t_exp: sub-exposure j sits at off0 + j doff (R18)
@@ -544,6 +541,15 @@ __device__ __forceinline__ int lower_bound_warp(const double* __restrict__ seg, 
     return min(base + 1 + cnt, n);
 }
 
+// A walker off the common path (eccentric orbit, long window, many transit epochs, evolute regime,
+// unsorted series): the CTA (or cluster) does the unit with the full-featured arithmetic of
+// greenlantern_b200.cu -- fp64 phase of every exposure, Kepler, generic crossing search -- one exposure
+// per lane and pass.  Defined in greenlantern_b200.cu (it needs that file's Walker machinery); NOT
+// inlined: this code is never fetched unless a walker needs it.  Returns CLS_INVALID for an invalid
+// walker (its flux row is NaN-filled), else CLS_SIMPLE with the thread's chi^2 terms added to *acc.
+__device__ int generic_unit(const HotArgs& A, bool pre, int wk, int t_lo, int nT, int gtid, int ntot,
+                            const glf::TrapNode* trap, double* acc);
+
 template <bool PRE>
 __global__ void __launch_bounds__(HOT_NT, 2) hot_kernel(const HotArgs A) {
     asm volatile("griddepcontrol.launch_dependents;");   // the fallback launch may become resident
@@ -556,7 +562,6 @@ __global__ void __launch_bounds__(HOT_NT, 2) hot_kernel(const HotArgs A) {
     __shared__ double s_coarse[HOT_NT];    // every stride-th time of the segment (+inf beyond its end)
     __shared__ double s_red[HOT_NW];
     __shared__ double s_gather[2][MAXC];   // rank 0's copy collects the cluster's chi^2 partials
-    __shared__ int s_gflag[2][MAXC];       // ... and their "my share of the series is out of order" flags
     __shared__ int s_cnt[2][HOT_NW];       // near-limb pairs per (pair slot, warp)
     __shared__ float s_px[CAP], s_py[CAP]; // sparse mode: folded kernel-frame centre of a near-limb pair
     __shared__ float s_d[CAP];             // ... blocked fraction of every pair
@@ -599,9 +604,9 @@ __global__ void __launch_bounds__(HOT_NT, 2) hot_kernel(const HotArgs A) {
             s_coarse[tid] = ci < nT ? seg[ci] : __longlong_as_double(0x7ff0000000000000LL);
         }
         int unsorted = 0;
-        if (!A.sorted_known) {
+        if (!A.sorted_known) {   // (every CTA of a cluster looks at ALL pairs: the verdict must be the cluster's)
             const int npairs = min(nT, A.T - t_lo - 1);
-            for (int i = gtid; i < npairs; i += ntot) unsorted |= !(seg[i] <= seg[i + 1]);
+            for (int i = tid; i < npairs; i += HOT_NT) unsorted |= !(seg[i] <= seg[i + 1]);
         }
         if (warp < 4) {
             const double v = lane < 12 ? p[lane] : 0.0;
@@ -627,7 +632,7 @@ __global__ void __launch_bounds__(HOT_NT, 2) hot_kernel(const HotArgs A) {
         if (cls == CLS_SIMPLE && !su.never &&
             (su.bad_period || su.defer_shape || !few || !(su.phimax + su.w * (float)A.t_exp <= 0.8f)))
             cls = CLS_DEFER;   // (0.8 rad: small_sincos's range)
-        if (cls == CLS_SIMPLE && unsorted && csize == 1) cls = CLS_DEFER;   // (clusters: decided at the end)
+        if (cls == CLS_SIMPLE && unsorted) cls = CLS_DEFER;
         const int nep = (cls == CLS_SIMPLE && !su.never && cnt > 0.0) ? (int)cnt : 0;
 
         // ---- 2. for a sorted series the in-window exposures of an epoch are ONE index range: warp
@@ -649,10 +654,15 @@ __global__ void __launch_bounds__(HOT_NT, 2) hot_kernel(const HotArgs A) {
         GLH_TL(2);
 
         double acc = 0.0;   // this thread's chi^2 terms
-        if (cls == CLS_INVALID) {
+        if (cls == CLS_DEFER) {   // (CTA-uniform, and the same in every CTA of a cluster)
+            double gacc = 0.0;    // (its address is taken: kept apart from acc, which stays in registers)
+            cls = generic_unit(A, PRE, wk, t_lo, nT, gtid, ntot, s_trap, &gacc);
+            acc = gacc;
+        }
+        else if (cls == CLS_INVALID) {
             if (frow)
                 for (int i = gtid; i < nT; i += ntot) frow[i] = __int_as_float(0x7fc00000);
-        } else if (cls == CLS_SIMPLE) {
+        } else {
             const float w = su.w, aR = su.aR, bimp = su.bimp, a = su.a, b = su.b;
             const float cpsi = su.cpsi, spsi = su.spsi, k0 = su.k0, k1 = su.k1, k2 = su.k2;
             const float ab = a * b, e2 = (a - b) * (a + b);
@@ -850,49 +860,30 @@ __global__ void __launch_bounds__(HOT_NT, 2) hot_kernel(const HotArgs A) {
                 double tot = 0.0;
                 for (int k = 0; k < HOT_NW; ++k) tot += s_red[k];
                 GLH_DELAY(2);
-                if (csize > 1) {
-                    *cluster.map_shared_rank(&s_gather[wpar][crank], 0) = tot;
-                    *cluster.map_shared_rank(&s_gflag[wpar][crank], 0) = unsorted;
-                } else {
-                    s_gather[wpar][0] = tot;
-                    s_gflag[wpar][0] = 0;   // (a single CTA has already deferred an unsorted unit)
-                }
+                if (csize > 1) *cluster.map_shared_rank(&s_gather[wpar][crank], 0) = tot;
+                else s_gather[wpar][0] = tot;
             }
             GLH_DELAY(3);
             if (csize > 1) cluster.sync();
             GLH_DELAY(4);
             if (crank == 0 && tid == 0) {
                 double d2 = 0.0;
-                int uns = 0;
-                for (int r = 0; r < csize; ++r) {
-                    d2 += s_gather[wpar][r];
-                    uns |= s_gflag[wpar][r];
-                }
-                if (uns && cls == CLS_SIMPLE) cls = CLS_DEFER;   // some CTA's share of the series is out of order
+                for (int r = 0; r < csize; ++r) d2 += s_gather[wpar][r];
                 // raw series: baseline_kernel, launched before this grid (which may have started early:
                 // programmatic dependent launch), writes S into chi2[0..B): wait before touching chi2
                 if (!PRE) asm volatile("griddepcontrol.wait;" ::: "memory");
                 float out;
                 if (cls == CLS_INVALID) {
                     out = __int_as_float(0x7f800000);
-                } else if (cls == CLS_DEFER) {
-                    out = __uint_as_float(MARK_BITS);
                 } else {
                     double Sb = A.S;
                     if (!PRE) Sb = (double)*(volatile float*)&A.chi2[wk];
                     out = (Sb > 1.79769313486231570e308) ? (float)Sb : (float)(Sb + d2);
                 }
                 A.chi2[wk] = out;
-                if (cls == CLS_DEFER && A.status) *A.status = 1;
             }
             GLH_TL(5);
             wpar ^= 1;
-        } else if (frow && cls == CLS_DEFER) {
-            // flux-only units are single CTAs; the marker goes where this segment's row starts
-            if (tid == 0) {
-                frow[0] = __uint_as_float(MARK_BITS);
-                if (A.status) *A.status = 1;
-            }
         }
     }
     if (!started) cluster.barrier_wait();

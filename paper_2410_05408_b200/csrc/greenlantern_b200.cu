@@ -460,6 +460,66 @@ __device__ __forceinline__ T blocked_fraction(const glf::TrapNode* trap, const W
 }
 
 
+}  // namespace
+
+// hot_kernel's path for a walker off the common path (declared in gl_hot.cuh): the CTA -- or every CTA of
+// the cluster, each on its share gtid, gtid + ntot, ... of the exposures -- runs the full-featured
+// arithmetic: general prelude (validity incl. the eccentric rules, Kepler constants, conservative
+// window), fp64 phase of every exposure (any order of the series, any number of transits), Kepler's
+// equation per sub-exposure for e > 0, the generic crossing search where the evolute test asks for it.
+// One exposure per lane and pass, sub-exposures in turn; chi^2 terms in hot_kernel's cancellation-free
+// form.  NOT inlined into hot_kernel: never fetched unless a walker needs it.
+__device__ __noinline__ int glh::generic_unit(const glh::HotArgs& A, bool pre, int wk, int t_lo, int nT,
+                                              int gtid, int ntot, const glf::TrapNode* trap, double* acc) {
+    __shared__ Walker gw;
+    const int tid = threadIdx.x;
+    const double* p = A.params + (size_t)wk * GL_NPARAMS;
+    if (tid == 0) walker_prelude_orbit<float>(p, GL_NPARAMS, A.t_exp, &gw);
+    if (tid == 32) walker_prelude_shape<float>(p, GL_NPARAMS, &gw);
+    __syncthreads();
+    const double* __restrict__ seg = A.times + t_lo;
+    float* frow = A.flux ? A.flux + (size_t)wk * A.T + t_lo : nullptr;
+    if (!gw.valid) {
+        if (frow)
+            for (int i = gtid; i < nT; i += ntot) frow[i] = __int_as_float(0x7fc00000);
+        return glh::CLS_INVALID;
+    }
+    const WalkerT<float> v = narrow<float>(gw);
+    const double hwin = gw.half_win_phase, inv_ss = 1.0 / (double)A.n_ss;
+    for (int i = gtid; i < nT; i += ntot) {
+        const double tc = seg[i];
+        if (!(fabs(reduced_phase(gw, tc)) < hwin)) {
+            if (frow) frow[i] = 1.f;
+            continue;
+        }
+        float sum = 0.f;
+        for (int j = 0; j < A.n_ss; ++j) {
+            const double t = tc + (((double)j + 0.5) * inv_ss - 0.5) * A.t_exp;
+            sum += blocked_fraction<float, false>(trap, gw, v, reduced_phase(gw, t));
+        }
+        const float dbar = sum * A.inv_ss;
+        if (frow) frow[i] = 1.f - dbar;
+        if (A.chi2) {
+            float ob, rs;
+            if (pre) {
+                const float2 o2 = A.ow[t_lo + i];
+                ob = o2.x;
+                rs = o2.y;
+            } else {
+                ob = (float)(A.obs[t_lo + i] - 1.0);
+                const float sf = (float)A.sigma[t_lo + i];
+                rs = glf::mufu_rcp(sf);
+                rs = rs * fmaf(-sf, rs, 2.f);
+            }
+            const float d = dbar * rs;
+            *acc += (double)(d * fmaf(2.f * ob, rs, d));
+        }
+    }
+    return glh::CLS_SIMPLE;
+}
+
+namespace {
+
 // ------------------------------------------------------------------------------------------
 // Deterministic sum of one double per thread over the CTA (fixed shuffle tree, fixed warp order).
 // ------------------------------------------------------------------------------------------
@@ -556,8 +616,8 @@ __global__ void __launch_bounds__(NT, sizeof(T) == 4 ? 8 : 2)
 transit_kernel(const double* __restrict__ params, int B,
                const double* __restrict__ times_all, int nT_all,
                int tile, double t_exp, int n_ss, const double* __restrict__ obs,
-               const double* __restrict__ sigma, T* flux, T* chi2, int shared_base,
-               int nseg_arg, int seglen_arg, int marker_mode) {
+               const double* __restrict__ sigma, T* __restrict__ flux, T* chi2, int shared_base,
+               int nseg_arg, int seglen_arg) {
     const int nseg = SEG ? nseg_arg : 1, seglen = SEG ? seglen_arg : nT_all;
     cg::cluster_group cluster = cg::this_cluster();
     const int crank = (int)cluster.block_rank(), csize = (int)cluster.num_blocks();
@@ -584,7 +644,7 @@ transit_kernel(const double* __restrict__ params, int B,
     bool lists_live = false;   // uniform over the cluster
 
     // warm the L2 with this CTA's first tile while the prelude runs (one line = 16 doubles)
-    for (int i = crank * tile + tid * 16; !marker_mode && i < min(nT_all, (crank + 1) * tile); i += NT * 16) {
+    for (int i = crank * tile + tid * 16; i < min(nT_all, (crank + 1) * tile); i += NT * 16) {
         asm volatile("prefetch.global.L2 [%0];" ::"l"(times_all + i));
         if (want_chi2) {
             asm volatile("prefetch.global.L2 [%0];" ::"l"(obs + i));
@@ -594,33 +654,8 @@ transit_kernel(const double* __restrict__ params, int B,
     // A cluster works on one (walker, segment of the series); nseg > 1 only for flux-only calls with
     // few walkers and a long series (one light curve of 1e5 exposures would otherwise use 8 CTAs of
     // the whole GPU); chi^2 calls keep nseg = 1 (the sum over a walker's series stays in one cluster).
-    // marker_mode: this launch FINISHES what hot_kernel (gl_hot.cuh), launched just before it, deferred:
-    // only (walker, segment) units whose output slot carries the marker are done; the others are
-    // left as they are.  The grid may have started early (programmatic dependent launch).
-    if (marker_mode) {
-        asm volatile("griddepcontrol.wait;" ::: "memory");
-        // common case: nothing was deferred.  Thread t looks at the slot of the t-th unit this cluster
-        // would take, all at once (one load latency), and the CTA leaves if none carries the marker.
-        // Every CTA of a cluster looks at the same slots, so the verdict is cluster-uniform.
-        bool any = false;
-        for (long long vw = blockIdx.y + (long long)tid * gridDim.y; vw < (long long)B * nseg;
-             vw += (long long)NT * gridDim.y) {
-            const int wk = (int)(vw / nseg), t_lo = (int)(vw - (long long)wk * nseg) * seglen;
-            const T* slot = want_chi2 ? chi2 + wk : flux + (size_t)wk * nT_all + t_lo;
-            any = any || (sizeof(T) == 4 && *reinterpret_cast<const volatile uint32_t*>(slot) == glh::MARK_BITS);
-        }
-        GLH_DELAY(11);
-        if (!__syncthreads_or(any ? 1 : 0)) return;
-    }
     for (long long vw = blockIdx.y; vw < (long long)B * nseg; vw += gridDim.y) {
         const int wk = (int)(vw / nseg), t_lo = (int)(vw - (long long)wk * nseg) * seglen;
-        if (sizeof(T) == 4 && marker_mode) {   // (markers are an fp32 affair: hot_kernel has no fp64 flavour)
-            const T* slot = want_chi2 ? chi2 + wk : flux + (size_t)wk * nT_all + t_lo;
-            const uint32_t bits = *reinterpret_cast<const volatile uint32_t*>(slot);
-            if (bits != glh::MARK_BITS) continue;   // (only this cluster ever rewrites this slot)
-            GLH_DELAY(12);
-            if (csize > 1) cluster.sync();   // every CTA has read the slot before any CTA rewrites it
-        }
         const double* __restrict__ times = times_all + t_lo;
         const int nT = min(seglen, nT_all - t_lo);
         const int nrounds = (nT + round_span - 1) / round_span;
@@ -875,6 +910,7 @@ geometry_kernel(const double* __restrict__ geom, long long N, T* __restrict__ ou
 //   stage 4  those three lists, full warps each (glh::near_rest, glc::overlap_areas)
 // Outputs go to fixed slots, so the order inside a list (atomics) does not matter.
 constexpr int GEO_NT = 256, GEO_PER = 4, GEO_ROWS = GEO_NT * GEO_PER;
+constexpr uint32_t GEO_MARK = 0x7fc0deadu;   // "left to geometry_evolute_kernel": a quiet NaN no arithmetic here produces
 __global__ void __launch_bounds__(GEO_NT)
 geometry_sorted_kernel(const double* __restrict__ geom, long long N, float* __restrict__ out) {
     __shared__ glf::TrapNode s_trap[16];
@@ -967,7 +1003,7 @@ geometry_sorted_kernel(const double* __restrict__ geom, long long N, float* __re
         if (Aa < e2 && Bb < e2 && glf::evolute_inside(Aa, Bb, e2)) {
             // the generic bracketed search is ~10x longer than anything else here: left to
             // geometry_evolute_kernel, which gathers these rows from the whole grid into full warps
-            out[row_of(loc)] = __uint_as_float(glh::MARK_BITS);
+            out[row_of(loc)] = __uint_as_float(GEO_MARK);
             s_ord2[j] = 0xffffu;
             continue;
         } else {
@@ -1047,7 +1083,7 @@ geometry_evolute_kernel(const double* __restrict__ geom, long long N, float* out
         for (int r = tid; r < EVO_ROWS; r += EVO_NT) {
             const long long blk = b0 + (long long)(r >> 5) * gridDim.x;
             const long long k = blk * 32 + (r & 31);
-            if (blk < nblocks && k < N && *reinterpret_cast<const volatile uint32_t*>(out + k) == glh::MARK_BITS)
+            if (blk < nblocks && k < N && *reinterpret_cast<const volatile uint32_t*>(out + k) == GEO_MARK)
                 s_rows[atomicAdd(&s_n, 1)] = k;
         }
         __syncthreads();
@@ -1177,15 +1213,13 @@ void pick_shape(long long rows, int nT, int* C, int* tile) {
     *tile = t;
 }
 
-// One launch of transit_kernel<T, EX, SEG>.  marker_mode: finish the units hot_kernel deferred.
+// One launch of transit_kernel<T, EX, SEG>.
 template <typename T>
 int launch_full(const double* params, int nparams, int B, const double* times, int nT, double t_exp,
                 int n_ss, const double* obs, const double* sigma, void* flux, void* chi2,
-                int shared_base, int nseg, int seglen, int marker_mode, long long max_rows, bool pdl,
-                cudaStream_t st) {
+                int shared_base, int nseg, int seglen, bool pdl, cudaStream_t st) {
     const long long units = (long long)B * nseg;
-    long long rows = units < 65535 ? units : 65535;
-    if (max_rows > 0 && rows > max_rows) rows = max_rows;
+    const long long rows = units < 65535 ? units : 65535;
     int C, tile;
     pick_shape(rows, seglen, &C, &tile);
     cudaLaunchConfig_t cfg = {};
@@ -1207,17 +1241,15 @@ int launch_full(const double* params, int nparams, int B, const double* times, i
             return (nparams == GL_NPARAMS_EX)
                        ? cudaLaunchKernelEx(&cfg, transit_kernel<T, true, true>, params, B, times, nT, tile,
                                             t_exp, n_ss, obs, sigma, (T*)flux, (T*)chi2, shared_base, nseg,
-                                            seglen, marker_mode)
+                                            seglen)
                        : cudaLaunchKernelEx(&cfg, transit_kernel<T, false, true>, params, B, times, nT, tile,
                                             t_exp, n_ss, obs, sigma, (T*)flux, (T*)chi2, shared_base, nseg,
-                                            seglen, marker_mode);
+                                            seglen);
         return (nparams == GL_NPARAMS_EX)
                    ? cudaLaunchKernelEx(&cfg, transit_kernel<T, true, false>, params, B, times, nT, tile,
-                                        t_exp, n_ss, obs, sigma, (T*)flux, (T*)chi2, shared_base, 1, nT,
-                                        marker_mode)
+                                        t_exp, n_ss, obs, sigma, (T*)flux, (T*)chi2, shared_base, 1, nT)
                    : cudaLaunchKernelEx(&cfg, transit_kernel<T, false, false>, params, B, times, nT, tile,
-                                        t_exp, n_ss, obs, sigma, (T*)flux, (T*)chi2, shared_base, 1, nT,
-                                        marker_mode);
+                                        t_exp, n_ss, obs, sigma, (T*)flux, (T*)chi2, shared_base, 1, nT);
     };
     cudaError_t e = launch();
     if (e != cudaSuccess && pdl) {
@@ -1258,27 +1290,22 @@ HotShape pick_hot_shape(int B, int nT, bool want_chi2) {
     return h;
 }
 
-// Rows of the fallback grid (transit_kernel in marker mode) behind a hot launch: it finds work only
-// for deferred walkers, so in the common case it is pure overhead at the end of the step; one
-// cluster per SM keeps that small and still finishes a fully deferred batch in a few rounds.
-#ifndef GL_FALLBACK_ROWS
-#define GL_FALLBACK_ROWS 148
-#endif
-
 struct SeriesView {          // what gl_series keeps resident (all nullptr / 0 for a plain call)
     const float2* ow = nullptr;
     double S = 0.0;
     int sorted_known = 0;
-    int* status = nullptr;
-    bool with_fallback = true;
 };
 
-// fp32, 12-column rows, nT > 0: [baseline_kernel ->] hot_kernel -> transit_kernel (marker mode).
+// fp32, 12-column rows, nT > 0: [baseline_kernel ->] hot_kernel.
 int launch_hot(const double* params, int B, const double* times, int nT, double t_exp, int n_ss,
                const double* obs, const double* sigma, float* flux, float* chi2, const SeriesView& sv,
                cudaStream_t st) {
     const bool pre = sv.ow != nullptr, want_chi2 = chi2 != nullptr;
     const HotShape h = pick_hot_shape(B, nT, want_chi2);
+    {   // (a walker off the common path runs the generic code, which reads the constant-memory tables)
+        const int rc = ensure_tables();
+        if (rc != GL_OK) return rc;
+    }
     if (want_chi2 && !pre) {
         baseline_kernel<<<1, 1024, 0, st>>>(obs, sigma, nT, chi2, B);
         cudaError_t e0 = cudaGetLastError();
@@ -1293,7 +1320,6 @@ int launch_hot(const double* params, int B, const double* times, int nT, double 
     a.ow = sv.ow;
     a.flux = flux;
     a.chi2 = chi2;
-    a.status = sv.status;
     a.S = sv.S;
     a.t_exp = t_exp;
     a.inv_ss = 1.f / (float)n_ss;
@@ -1340,9 +1366,7 @@ int launch_hot(const double* params, int B, const double* times, int nT, double 
     }
     if (e != cudaSuccess) return cuda_fail(e, "hot_kernel launch");
     ++tl_launches;
-    if (!sv.with_fallback) return GL_OK;
-    return launch_full<float>(params, GL_NPARAMS, B, times, nT, t_exp, n_ss, obs, sigma, flux, chi2, 0,
-                              h.nseg, h.seglen, 1, GL_FALLBACK_ROWS, true, st);
+    return GL_OK;
 }
 
 template <typename T>
@@ -1378,7 +1402,7 @@ int launch_transit(const double* params, int nparams, int B, const double* times
         ++tl_launches;
     }
     return launch_full<T>(params, nparams, B, times, nT, t_exp, n_ss, obs, sigma, flux, chi2, shared_base,
-                          nseg, seglen, 0, 0, shared_base != 0, st);
+                          nseg, seglen, shared_base != 0, st);
 }
 
 int run_transit(const double* params, int nparams, int B, const double* times, int nT, double t_exp,
@@ -1617,6 +1641,39 @@ int gl_probe_empty_launch(int cluster, int rows, int threads, int fallback_clust
     return GL_OK;
 }
 
+// The same empty kernel replayed as a CUDA graph (captured once per shape and calling thread), the way
+// gl_series_loglike_dev launches a step.
+int gl_probe_empty_graph(int cluster, int rows, int threads, void* stream) {
+    if (cluster < 1 || cluster > 8 || rows < 1 || threads < 32 || threads > 1024) return GL_EINVAL;
+    thread_local cudaGraphExec_t exec = nullptr;
+    thread_local int shape[3] = {0, 0, 0};
+    if (!exec || shape[0] != cluster || shape[1] != rows || shape[2] != threads) {
+        if (exec) cudaGraphExecDestroy(exec);
+        exec = nullptr;
+        cudaStream_t cs = nullptr;
+        cudaGraph_t graph = nullptr;
+        cudaError_t e = cudaStreamCreateWithFlags(&cs, cudaStreamNonBlocking);
+        if (e == cudaSuccess) e = cudaStreamBeginCapture(cs, cudaStreamCaptureModeThreadLocal);
+        if (e == cudaSuccess) {
+            const int rc = gl_probe_empty_launch(cluster, rows, threads, 1, 0, cs);
+            e = cudaStreamEndCapture(cs, &graph);
+            if (rc != GL_OK && e == cudaSuccess) e = cudaErrorUnknown;
+        }
+        if (e == cudaSuccess) e = cudaGraphInstantiate(&exec, graph, 0);
+        if (graph) cudaGraphDestroy(graph);
+        if (cs) cudaStreamDestroy(cs);
+        if (e != cudaSuccess) {
+            exec = nullptr;
+            return cuda_fail(e, "gl_probe_empty_graph capture");
+        }
+        shape[0] = cluster;
+        shape[1] = rows;
+        shape[2] = threads;
+    }
+    const cudaError_t e = cudaGraphLaunch(exec, (cudaStream_t)stream);
+    return e == cudaSuccess ? GL_OK : cuda_fail(e, "gl_probe_empty_graph launch");
+}
+
 long long gl_launch_count(void) { return tl_launches; }
 const char* gl_last_cuda_error(void) { return tl_cuda_err; }
 int gl_version(void) { return 100; }
@@ -1819,7 +1876,6 @@ struct gl_series {
     int dev = 0, T = 0, n_ss = 1, B_max = 0;
     double t_exp = 0.0, S = 0.0;
     int sorted = 0;
-    bool fallback_hint = false;      // the last host call needed the fallback launch
     cudaStream_t st = nullptr;       // host calls run here
     double *d_times = nullptr, *d_obs = nullptr, *d_sigma = nullptr;
     float2* d_ow = nullptr;
@@ -1827,14 +1883,11 @@ struct gl_series {
     // pinned, device-mapped staging: the kernel reads params and writes chi^2 over PCIe
     double* h_params = nullptr;
     float* h_chi2 = nullptr;
-    int* h_status = nullptr;
     double* m_params = nullptr;      // device aliases
     float* m_chi2 = nullptr;
-    int* m_status = nullptr;
-    int* d_status = nullptr;         // device word for gl_series_loglike_dev (never read back)
-    // gl_series_loglike_dev: the launch pair captured once per (params, B, chi2, flux) and replayed as a
+    // gl_series_loglike_dev: the launch captured once per (params, B, chi2, flux) and replayed as a
     // CUDA graph (callers reuse their buffers from step to step; a graph launch costs the GPU ~1 us
-    // less than the two stream launches it replaces)
+    // less than the stream launch it replaces)
     struct DevGraph {
         const double* params = nullptr;
         float *chi2 = nullptr, *flux = nullptr;
@@ -1876,17 +1929,13 @@ int gl_series_create(const double* times, const double* obs, const double* sigma
     if (ok()) e = cudaMalloc(&s->d_ow, sizeof(float2) * (size_t)T);
     if (ok()) e = cudaMalloc(&d_S, sizeof(double));
     if (ok()) e = cudaMalloc(&d_sorted, sizeof(int));
-    if (ok()) e = cudaMalloc(&s->d_status, sizeof(int));
     if (ok()) e = cudaHostAlloc(&s->h_params, sizeof(double) * GL_NPARAMS * (size_t)B_max, cudaHostAllocMapped);
     if (ok()) e = cudaHostAlloc(&s->h_chi2, sizeof(float) * (size_t)B_max, cudaHostAllocMapped);
-    if (ok()) e = cudaHostAlloc(&s->h_status, sizeof(int), cudaHostAllocMapped);
     if (ok()) e = cudaHostGetDevicePointer(&s->m_params, s->h_params, 0);
     if (ok()) e = cudaHostGetDevicePointer(&s->m_chi2, s->h_chi2, 0);
-    if (ok()) e = cudaHostGetDevicePointer(&s->m_status, s->h_status, 0);
     if (ok()) e = cudaMemcpyAsync(s->d_times, times, tb, cudaMemcpyHostToDevice, s->st);
     if (ok()) e = cudaMemcpyAsync(s->d_obs, obs, tb, cudaMemcpyHostToDevice, s->st);
     if (ok()) e = cudaMemcpyAsync(s->d_sigma, sigma, tb, cudaMemcpyHostToDevice, s->st);
-    if (ok()) e = cudaMemsetAsync(s->d_status, 0, sizeof(int), s->st);
     if (ok()) {
         series_prepare_kernel<<<1, 1024, 0, s->st>>>(s->d_times, s->d_obs, s->d_sigma, T, s->d_ow, d_S, d_sorted);
         e = cudaGetLastError();
@@ -1916,10 +1965,8 @@ int gl_series_destroy(gl_series* s) {
     cudaFree(s->d_sigma);
     cudaFree(s->d_ow);
     cudaFree(s->d_flux);
-    cudaFree(s->d_status);
     if (s->h_params) cudaFreeHost(s->h_params);
     if (s->h_chi2) cudaFreeHost(s->h_chi2);
-    if (s->h_status) cudaFreeHost(s->h_status);
     if (s->st) cudaStreamDestroy(s->st);
     delete s;
     return GL_OK;
@@ -1935,11 +1982,12 @@ int gl_series_info(const gl_series* s, int* T, int* n_ss, int* B_max, int* sorte
     return GL_OK;
 }
 
-int gl_series_loglike_dev(gl_series* s, const double* params, int B, float* chi2_out,
-                          float* flux_out_or_null, void* stream) {
-    if (!s || B < 0) return GL_EINVAL;
-    if (B == 0) return GL_OK;
-    if (!params || !chi2_out) return GL_EINVAL;
+}  // extern "C"
+
+// One likelihood launch against the resident series on `stream`: replay of the captured graph if this
+// (params, B, chi2, flux) was seen before, else capture + launch; plain stream launch if capture fails.
+static int series_launch(gl_series* s, const double* params, int B, float* chi2_out, float* flux_out_or_null,
+                         void* stream) {
     {
         std::lock_guard<std::mutex> lock(s->graph_mu);
         gl_series::DevGraph* slot = &s->graphs[0];
@@ -1948,12 +1996,12 @@ int gl_series_loglike_dev(gl_series* s, const double* params, int B, float* chi2
                 g.used = ++s->graph_clock;
                 const cudaError_t e = cudaGraphLaunch(g.exec, (cudaStream_t)stream);
                 if (e != cudaSuccess) return cuda_fail(e, "gl_series_loglike_dev graph launch");
-                tl_launches += 2;
+                tl_launches += 1;
                 return GL_OK;
             }
             if (g.used < slot->used) slot = &g;   // least recently used (empty slots have used = 0)
         }
-        // not seen before: capture the launch pair on the handle's own stream, keep it, launch it
+        // not seen before: capture the launch on the handle's own stream, keep it, launch it
         SeriesView svc;
         svc.ow = s->d_ow;
         svc.S = s->S;
@@ -1981,7 +2029,7 @@ int gl_series_loglike_dev(gl_series* s, const double* params, int B, float* chi2
             slot->used = ++s->graph_clock;
             e = cudaGraphLaunch(exec, (cudaStream_t)stream);
             if (e != cudaSuccess) return cuda_fail(e, "gl_series_loglike_dev graph launch");
-            tl_launches += 2;
+            tl_launches += 1;
             return GL_OK;
         }
         (void)cudaGetLastError();   // no graph then: plain stream launches below
@@ -1990,10 +2038,18 @@ int gl_series_loglike_dev(gl_series* s, const double* params, int B, float* chi2
     sv.ow = s->d_ow;
     sv.S = s->S;
     sv.sorted_known = s->sorted;
-    sv.status = nullptr;
-    sv.with_fallback = true;
     return launch_hot(params, B, s->d_times, s->T, s->t_exp, s->n_ss, s->d_obs, s->d_sigma,
                       flux_out_or_null, chi2_out, sv, (cudaStream_t)stream);
+}
+
+extern "C" {
+
+int gl_series_loglike_dev(gl_series* s, const double* params, int B, float* chi2_out,
+                          float* flux_out_or_null, void* stream) {
+    if (!s || B < 0) return GL_EINVAL;
+    if (B == 0) return GL_OK;
+    if (!params || !chi2_out) return GL_EINVAL;
+    return series_launch(s, params, B, chi2_out, flux_out_or_null, stream);
 }
 
 int gl_series_loglike(gl_series* s, const double* params, int B, float* chi2_out, float* flux_out_or_null) {
@@ -2006,36 +2062,14 @@ int gl_series_loglike(gl_series* s, const double* params, int B, float* chi2_out
         if (e != cudaSuccess) return cuda_fail(e, "gl_series_loglike flux buffer");
     }
     memcpy(s->h_params, params, sizeof(double) * GL_NPARAMS * (size_t)B);
-    *(volatile int*)s->h_status = 0;
-    SeriesView sv;
-    sv.ow = s->d_ow;
-    sv.S = s->S;
-    sv.sorted_known = s->sorted;
-    sv.status = s->m_status;
-    sv.with_fallback = s->fallback_hint;
     float* flux = flux_out_or_null ? s->d_flux : nullptr;
-    int rc = launch_hot(s->m_params, B, s->d_times, s->T, s->t_exp, s->n_ss, s->d_obs, s->d_sigma, flux,
-                        s->m_chi2, sv, s->st);
+    const int rc = series_launch(s, s->m_params, B, s->m_chi2, flux, s->st);   // (graph replay after the first call)
     if (rc != GL_OK) return rc;
-    e = cudaStreamSynchronize(s->st);
-    if (e != cudaSuccess) return cuda_fail(e, "gl_series_loglike");
-    const int deferred = *(volatile int*)s->h_status;
-    if (deferred && !sv.with_fallback) {
-        // some walker needs the full-featured kernel and it was not launched: do it now, and launch it
-        // together with the hot kernel from the next call on
-        rc = launch_full<float>(s->m_params, GL_NPARAMS, B, s->d_times, s->T, s->t_exp, s->n_ss, s->d_obs,
-                                s->d_sigma, flux, s->m_chi2, 0, 1, s->T, 1, 0, false, s->st);
-        if (rc != GL_OK) return rc;
-        e = cudaStreamSynchronize(s->st);
-        if (e != cudaSuccess) return cuda_fail(e, "gl_series_loglike (fallback)");
-    }
-    s->fallback_hint = deferred != 0;
-    if (flux) {
+    if (flux)
         e = cudaMemcpyAsync(flux_out_or_null, flux, sizeof(float) * (size_t)B * (size_t)s->T,
                             cudaMemcpyDeviceToHost, s->st);
-        if (e == cudaSuccess) e = cudaStreamSynchronize(s->st);
-        if (e != cudaSuccess) return cuda_fail(e, "gl_series_loglike flux copy");
-    }
+    if (e == cudaSuccess) e = cudaStreamSynchronize(s->st);
+    if (e != cudaSuccess) return cuda_fail(e, "gl_series_loglike");
     memcpy(chi2_out, s->h_chi2, sizeof(float) * (size_t)B);
     return GL_OK;
 }

@@ -7,14 +7,14 @@
 same launches through another build of the library (the CHECKED build: index assertions + random
 per-CTA delays), `--dump <.npz>` writes every fp32 output for a bitwise comparison between builds.  Every output is also
 compared with the fp64 path of the library itself, so a run that "passes" the tool on garbage shows.
-Patterns: hot_kernel sparse mode (two compactions, two-lane near-limb pairs, fill by idle warps) and
-dense mode; hot_kernel as a cluster (barrier_arrive at entry / wait before the first DSMEM push, flags
-pushed with the partials); flux-only calls cut into segments; units looping over grid rows; the
-fallback transit_kernel in marker mode (parallel marker pre-check, cluster.sync before the first
-rewrite) on eccentric, extended/locked and many-walkers-per-cluster batches; multi-round series
-(T > C * tile) with the lists reused under a cluster barrier; the fp32 baseline + hot + fallback
-PDL chain; the GP scan behind them; the resident-series host and device calls (graph replay); the
-bare-geometry kernels.  Not collected by pytest (run under the tool).
+Patterns: hot_kernel sparse mode (compaction of the near-limb pairs, two lanes per pair, fill by idle
+warps) and dense mode; hot_kernel as a cluster (barrier_arrive at entry / wait before the first DSMEM
+push); flux-only calls cut into segments; units looping over grid rows; walkers off the common path
+(eccentric, flat, close-in, short-period: generic_unit inside hot_kernel) alone and mixed with common
+and invalid ones; the full transit_kernel (fp64, extended/locked rows) with several walkers per
+cluster and multi-round series (T > C * tile: lists reused under a cluster barrier); the fp32
+baseline + hot PDL chain; the GP scan behind it; the resident-series host and device calls (graph
+replay); the bare-geometry kernels.  Not collected by pytest (run under the tool).
 """
 import sys
 from pathlib import Path
@@ -89,7 +89,7 @@ def main():
     torch.cuda.synchronize()
     assert (lc[0] - f32[0]).abs().max().item() <= 1.2e-7
 
-    print("mixed batch: walkers the hot kernel defers (eccentric, flat, close-in, short period) + invalid ones")
+    print("mixed batch: walkers off the common path (eccentric, flat, close-in, short period) + invalid ones")
     q = wl.config3(B=16 if QUICK else 40).params.copy()
     q[1::8, 4], q[1::8, 5] = 0.3, 1.0
     q[2::8, 7], q[2::8, 9] = 0.97, 0.02
@@ -100,7 +100,7 @@ def main():
     check("flux", f32, f64, 5e-7)
     check("chi2", c32, c64, 1e-4)
 
-    print("fallback kernel, several deferred walkers per cluster and a multi-round series (lists reused)")
+    print("all walkers eccentric (generic_unit; fp64: several walkers per cluster), and a multi-round two-transit series")
     B = 200 if QUICK else 600
     e = wl.draw_walkers(B, 5)
     e[:, 4], e[:, 5] = 0.2, rng.uniform(0, 6, B)
