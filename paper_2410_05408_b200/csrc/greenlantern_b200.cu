@@ -21,6 +21,8 @@
 #include <stdlib.h>
 #include <string.h>
 
+#include <atomic>
+#include <chrono>
 #include <new>
 
 #include <mutex>
@@ -1294,6 +1296,8 @@ struct SeriesView {          // what gl_series keeps resident (all nullptr / 0 f
     const float2* ow = nullptr;
     double S = 0.0;
     int sorted_known = 0;
+    int* done_count = nullptr;   // see glh::HotArgs
+    int* done_flag = nullptr;
 };
 
 // fp32, 12-column rows, nT > 0: [baseline_kernel ->] hot_kernel.
@@ -1332,6 +1336,8 @@ int launch_hot(const double* params, int B, const double* times, int nT, double 
     a.nseg = h.nseg;
     a.seglen = h.seglen;
     a.sorted_known = sv.sorted_known;
+    a.done_count = sv.done_count;
+    a.done_flag = sv.done_flag;
     const long long units = (long long)B * h.nseg;
     cudaLaunchConfig_t cfg = {};
     cfg.gridDim = dim3((unsigned)h.C, (unsigned)(units < 65535 ? units : 65535), 1);
@@ -1885,6 +1891,9 @@ struct gl_series {
     float* h_chi2 = nullptr;
     double* m_params = nullptr;      // device aliases
     float* m_chi2 = nullptr;
+    int* h_done = nullptr;           // completion flag of the host call (pinned, mapped) ...
+    int* m_done = nullptr;
+    int* d_done_count = nullptr;     // ... and the device counter behind it
     // gl_series_loglike_dev: the launch captured once per (params, B, chi2, flux) and replayed as a
     // CUDA graph (callers reuse their buffers from step to step; a graph launch costs the GPU ~1 us
     // less than the stream launch it replaces)
@@ -1892,6 +1901,7 @@ struct gl_series {
         const double* params = nullptr;
         float *chi2 = nullptr, *flux = nullptr;
         int B = 0;
+        bool signal = false;
         cudaGraphExec_t exec = nullptr;
         unsigned long long used = 0;
     } graphs[4];
@@ -1931,6 +1941,10 @@ int gl_series_create(const double* times, const double* obs, const double* sigma
     if (ok()) e = cudaMalloc(&d_sorted, sizeof(int));
     if (ok()) e = cudaHostAlloc(&s->h_params, sizeof(double) * GL_NPARAMS * (size_t)B_max, cudaHostAllocMapped);
     if (ok()) e = cudaHostAlloc(&s->h_chi2, sizeof(float) * (size_t)B_max, cudaHostAllocMapped);
+    if (ok()) e = cudaHostAlloc(&s->h_done, sizeof(int), cudaHostAllocMapped);
+    if (ok()) e = cudaHostGetDevicePointer(&s->m_done, s->h_done, 0);
+    if (ok()) e = cudaMalloc(&s->d_done_count, sizeof(int));
+    if (ok()) e = cudaMemsetAsync(s->d_done_count, 0, sizeof(int), s->st);
     if (ok()) e = cudaHostGetDevicePointer(&s->m_params, s->h_params, 0);
     if (ok()) e = cudaHostGetDevicePointer(&s->m_chi2, s->h_chi2, 0);
     if (ok()) e = cudaMemcpyAsync(s->d_times, times, tb, cudaMemcpyHostToDevice, s->st);
@@ -1967,6 +1981,8 @@ int gl_series_destroy(gl_series* s) {
     cudaFree(s->d_flux);
     if (s->h_params) cudaFreeHost(s->h_params);
     if (s->h_chi2) cudaFreeHost(s->h_chi2);
+    if (s->h_done) cudaFreeHost(s->h_done);
+    cudaFree(s->d_done_count);
     if (s->st) cudaStreamDestroy(s->st);
     delete s;
     return GL_OK;
@@ -1987,12 +2003,13 @@ int gl_series_info(const gl_series* s, int* T, int* n_ss, int* B_max, int* sorte
 // One likelihood launch against the resident series on `stream`: replay of the captured graph if this
 // (params, B, chi2, flux) was seen before, else capture + launch; plain stream launch if capture fails.
 static int series_launch(gl_series* s, const double* params, int B, float* chi2_out, float* flux_out_or_null,
-                         void* stream) {
+                         void* stream, bool signal = false) {
     {
         std::lock_guard<std::mutex> lock(s->graph_mu);
         gl_series::DevGraph* slot = &s->graphs[0];
         for (auto& g : s->graphs) {
-            if (g.exec && g.params == params && g.B == B && g.chi2 == chi2_out && g.flux == flux_out_or_null) {
+            if (g.exec && g.params == params && g.B == B && g.chi2 == chi2_out && g.flux == flux_out_or_null &&
+                g.signal == signal) {
                 g.used = ++s->graph_clock;
                 const cudaError_t e = cudaGraphLaunch(g.exec, (cudaStream_t)stream);
                 if (e != cudaSuccess) return cuda_fail(e, "gl_series_loglike_dev graph launch");
@@ -2006,6 +2023,10 @@ static int series_launch(gl_series* s, const double* params, int B, float* chi2_
         svc.ow = s->d_ow;
         svc.S = s->S;
         svc.sorted_known = s->sorted;
+        if (signal) {
+            svc.done_count = s->d_done_count;
+            svc.done_flag = s->m_done;
+        }
         cudaGraph_t graph = nullptr;
         cudaGraphExec_t exec = nullptr;
         const long long before = tl_launches;
@@ -2025,6 +2046,7 @@ static int series_launch(gl_series* s, const double* params, int B, float* chi2_
             slot->B = B;
             slot->chi2 = chi2_out;
             slot->flux = flux_out_or_null;
+            slot->signal = signal;
             slot->exec = exec;
             slot->used = ++s->graph_clock;
             e = cudaGraphLaunch(exec, (cudaStream_t)stream);
@@ -2038,6 +2060,10 @@ static int series_launch(gl_series* s, const double* params, int B, float* chi2_
     sv.ow = s->d_ow;
     sv.S = s->S;
     sv.sorted_known = s->sorted;
+    if (signal) {
+        sv.done_count = s->d_done_count;
+        sv.done_flag = s->m_done;
+    }
     return launch_hot(params, B, s->d_times, s->T, s->t_exp, s->n_ss, s->d_obs, s->d_sigma,
                       flux_out_or_null, chi2_out, sv, (cudaStream_t)stream);
 }
@@ -2063,12 +2089,31 @@ int gl_series_loglike(gl_series* s, const double* params, int B, float* chi2_out
     }
     memcpy(s->h_params, params, sizeof(double) * GL_NPARAMS * (size_t)B);
     float* flux = flux_out_or_null ? s->d_flux : nullptr;
-    const int rc = series_launch(s, s->m_params, B, s->m_chi2, flux, s->st);   // (graph replay after the first call)
+    *(volatile int*)s->h_done = 0;
+    const int rc = series_launch(s, s->m_params, B, s->m_chi2, flux, s->st, /*signal=*/!flux);   // (graph replay)
     if (rc != GL_OK) return rc;
-    if (flux)
+    if (flux) {
         e = cudaMemcpyAsync(flux_out_or_null, flux, sizeof(float) * (size_t)B * (size_t)s->T,
                             cudaMemcpyDeviceToHost, s->st);
-    if (e == cudaSuccess) e = cudaStreamSynchronize(s->st);
+        if (e == cudaSuccess) e = cudaStreamSynchronize(s->st);
+    } else {
+        // chi^2 only: the kernel's last CTA raises a flag in pinned host memory once every chi^2 is written;
+        // spinning on it returns sooner than a stream synchronise.  No flag within 2 s: let the stream say why.
+        const auto t_start = std::chrono::steady_clock::now();
+        unsigned spins = 0;
+        while (*(volatile int*)s->h_done == 0) {
+            if ((++spins & 0x3ffu) == 0 &&
+                std::chrono::steady_clock::now() - t_start > std::chrono::seconds(2)) {
+                e = cudaStreamSynchronize(s->st);
+                if (e == cudaSuccess && *(volatile int*)s->h_done == 0) {
+                    cudaMemsetAsync(s->d_done_count, 0, sizeof(int), s->st);   // re-arm for the next call
+                    e = cudaErrorUnknown;
+                }
+                break;
+            }
+        }
+        std::atomic_thread_fence(std::memory_order_acquire);
+    }
     if (e != cudaSuccess) return cuda_fail(e, "gl_series_loglike");
     memcpy(chi2_out, s->h_chi2, sizeof(float) * (size_t)B);
     return GL_OK;
