@@ -65,7 +65,8 @@ typedef enum {
     GL_OK = 0,
     GL_EINVAL = -1,       /* null pointer, negative size, n_ss < 1, unknown dtype, t_exp not finite */
     GL_ECUDA = -2,        /* a CUDA runtime call or a launch failed; see gl_last_cuda_error() */
-    GL_EUNSUPPORTED = -3  /* size outside what one launch can index (B*T or N >= 2^40)         */
+    GL_EUNSUPPORTED = -3, /* size outside what one launch can index (B*T or N >= 2^40)         */
+    GL_ECAPACITY = -4     /* size beyond the fixed capacity of a static-scratch entry point    */
 } gl_status;
 
 /* gl_lightcurve: flux_out[b*T + i] = F_b(times[i]).
@@ -144,6 +145,27 @@ int gl_munu_from_uniform(const double* uw, int B, double* munu_out, void* stream
 int gl_gp_loglike(const double* params, int B, const double* times, int T, double t_exp, int n_ss,
                   const double* obs, const double* sigma, const double* gp, double* loglike_out,
                   void* flux_work, gl_dtype dtype, void* stream);
+
+/* gl_gp_loglike_static: gl_gp_loglike in fp32 for callers that cannot allocate device memory (code
+ * under CUDA stream capture, tight serving loops, harnesses that forbid cudaMalloc).  The [B, T] fp32
+ * flux scratch that gl_gp_loglike takes as `flux_work` lives in a file-scope `static __device__` array
+ * of the library instead: GL_GP_STATIC_MAX_ELEMS floats = 4 MiB of EVERY GPU that loads the library,
+ * held until the process exits.  Inputs and the output are still the caller's (device pointers, as
+ * gl_gp_loglike); result and launches are those of gl_gp_loglike(..., GL_F32, ...) bit for bit.
+ *   - B * T > GL_GP_STATIC_MAX_ELEMS (also returned by gl_gp_static_capacity()): GL_ECAPACITY,
+ *     nothing enqueued.  Config 3 (256 x 3900) fits.
+ *   - Calls no cudaMalloc / cudaFree / allocating routine.  The first call on each device resolves the
+ *     array's address (cudaGetSymbolAddress, with that device current) and uploads the library's constant
+ *     tables if no other call has; later calls only launch.
+ *   - ALL calls on a device share the one array and it keeps the last call's contents.  Nothing in it
+ *     needs clearing: every element a call reads it has written first.  Calls that overlap on the GPU
+ *     (different streams, no ordering between them) RACE on it: order them, or use gl_gp_loglike with
+ *     buffers of your own. */
+#define GL_GP_STATIC_MAX_ELEMS (1 << 20)
+int gl_gp_loglike_static(const double* params, int B, const double* times, int T, double t_exp, int n_ss,
+                         const double* obs, const double* sigma, const double* gp, double* loglike_out,
+                         void* stream);
+long long gl_gp_static_capacity(void);
 
 /* gl_flux_geometry: steps "crossings + boundary integrals" alone, for N bare geometries.
  *   geom [N, GL_NGEOM] row-major fp64 (device): (d, Rp, f_proj, PA, u1, u2) -- planet centre at

@@ -16,7 +16,7 @@ GL_NPARAMS, GL_NGEOM, GL_NPARAMS_EX = 12, 6, 16
 _LIBPATH = Path(__file__).resolve().parent / "csrc" / "libgreenlantern_b200.so"
 _lib = None
 
-EXPORTS = ("gl_lightcurve", "gl_loglike", "gl_lightcurve_ex", "gl_loglike_ex", "gl_params_from_munu", "gl_munu_from_uniform", "gl_gp_loglike", "gl_flux_geometry", "gl_flux_geometry_simpson", "gl_lightcurve_host",
+EXPORTS = ("gl_lightcurve", "gl_loglike", "gl_lightcurve_ex", "gl_loglike_ex", "gl_params_from_munu", "gl_munu_from_uniform", "gl_gp_loglike", "gl_gp_loglike_static", "gl_gp_static_capacity", "gl_flux_geometry", "gl_flux_geometry_simpson", "gl_lightcurve_host",
            "gl_loglike_host", "gl_flux_geometry_host", "gl_series_create", "gl_series_loglike",
            "gl_series_loglike_dev", "gl_series_info", "gl_series_destroy", "gl_probe_peaks",
            "gl_probe_empty_launch", "gl_probe_empty_graph", "gl_launch_count", "gl_strerror",
@@ -48,6 +48,10 @@ def load_library():
     lib.gl_params_from_munu.restype = lib.gl_munu_from_uniform.restype = i
     lib.gl_gp_loglike.argtypes = [vp, i, vp, i, d, i, vp, vp, vp, vp, vp, i, vp]
     lib.gl_gp_loglike.restype = i
+    lib.gl_gp_loglike_static.argtypes = [vp, i, vp, i, d, i, vp, vp, vp, vp, vp]
+    lib.gl_gp_loglike_static.restype = i
+    lib.gl_gp_static_capacity.argtypes = []
+    lib.gl_gp_static_capacity.restype = ll
     lib.gl_flux_geometry.argtypes = [vp, ll, vp, i, vp]
     lib.gl_flux_geometry_simpson.argtypes = [vp, ll, i, vp, i, vp]
     lib.gl_flux_geometry_simpson.restype = i
@@ -215,6 +219,34 @@ def gl_gp_loglike(params, times, t_exp, n_ss, obs, sigma, gp, dtype="f32", want_
                                  obs.data_ptr(), sigma.data_ptr(), gp.data_ptr(), out.data_ptr(),
                                  flux.data_ptr(), code, _stream(params)))
     return (out, flux) if want_flux else out
+
+
+def gl_gp_static_capacity():
+    """Largest B * T gl_gp_loglike_static accepts (elements of its file-scope fp32 scratch array)."""
+    return int(load_library().gl_gp_static_capacity())
+
+
+def gl_gp_loglike_static(params, times, t_exp, n_ss, obs, sigma, gp, out=None):
+    """gl_gp_loglike in fp32 with the flux scratch inside the library (no device allocation by the
+    library; B * T <= gl_gp_static_capacity(), else GreenlanternError).  `out`: optional preallocated
+    CUDA float64 [B] tensor, so that the call allocates nothing at all.  Calls that overlap on the GPU
+    share the scratch and race: keep them on one stream."""
+    torch = _torch()
+    lib = load_library()
+    params, times = _dev_f64(params, GL_NPARAMS), _dev_f64(times)
+    obs, sigma, gp = _dev_f64(obs), _dev_f64(sigma), _dev_f64(gp, 3)
+    B, T = params.shape[0], times.shape[0]
+    if obs.shape[0] != T or sigma.shape[0] != T or gp.shape[0] != B:
+        raise GreenlanternError("obs, sigma must have the length of times and gp one row per walker")
+    if out is None:
+        out = torch.empty((B,), dtype=torch.float64, device=params.device)
+    elif not (out.is_cuda and out.dtype == torch.float64 and out.is_contiguous() and tuple(out.shape) == (B,)):
+        raise GreenlanternError(f"out must be a contiguous CUDA float64 tensor of shape ({B},)")
+    with torch.cuda.device(params.device):
+        _check(lib.gl_gp_loglike_static(params.data_ptr(), B, times.data_ptr(), T, float(t_exp), int(n_ss),
+                                        obs.data_ptr(), sigma.data_ptr(), gp.data_ptr(), out.data_ptr(),
+                                        _stream(params)))
+    return out
 
 
 def gl_flux_geometry(geom, dtype="f32"):

@@ -1684,12 +1684,67 @@ long long gl_launch_count(void) { return tl_launches; }
 const char* gl_last_cuda_error(void) { return tl_cuda_err; }
 int gl_version(void) { return 100; }
 
+}  // extern "C"
+
+// ------------------------------------------------------------------------------------------
+// gl_gp_loglike_static: the GP likelihood with its flux scratch in a file-scope device array, for
+// callers that may not allocate (stream capture, serving loops).  Nothing here calls an allocator.
+// ------------------------------------------------------------------------------------------
+namespace {
+
+// [B, T] fp32 model flux between the transit kernel and gp_scan_kernel.  4 MiB of every GPU that loads the
+// library, until the process exits.  In host code this NAME is a host-side stand-in, not a device address:
+// the address the kernels get comes from cudaGetSymbolAddress below.
+static __device__ __align__(256) float g_gp_static_flux[GL_GP_STATIC_MAX_ELEMS];
+
+// Device address of g_gp_static_flux on the CURRENT device, resolved once per device.
+int gp_static_scratch(float** out) {
+    static std::mutex mu;
+    static float* ptrs[64] = {};
+    int dev = 0;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) return cuda_fail(e, "cudaGetDevice");
+    std::lock_guard<std::mutex> lock(mu);
+    if (dev >= 0 && dev < 64 && ptrs[dev]) {
+        *out = ptrs[dev];
+        return GL_OK;
+    }
+    float* p = nullptr;
+    e = cudaGetSymbolAddress((void**)&p, g_gp_static_flux);
+    if (e != cudaSuccess) return cuda_fail(e, "cudaGetSymbolAddress(g_gp_static_flux)");
+    if (!p) return cuda_fail(cudaErrorInvalidSymbol, "cudaGetSymbolAddress(g_gp_static_flux)");
+    if (dev >= 0 && dev < 64) ptrs[dev] = p;
+    *out = p;
+    return GL_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+long long gl_gp_static_capacity(void) { return (long long)GL_GP_STATIC_MAX_ELEMS; }
+
+int gl_gp_loglike_static(const double* params, int B, const double* times, int T, double t_exp, int n_ss,
+                         const double* obs, const double* sigma, const double* gp, double* loglike_out,
+                         void* stream) {
+    if (B < 0 || T < 0) return GL_EINVAL;
+    if (B == 0) return GL_OK;
+    if ((long long)B * (long long)T > (long long)GL_GP_STATIC_MAX_ELEMS) return GL_ECAPACITY;
+    float* scratch = nullptr;
+    const int rc = gp_static_scratch(&scratch);
+    if (rc != GL_OK) return rc;
+    // every one of the B*T elements is rewritten by the transit kernel before gp_scan_kernel reads it
+    // (in-transit flux, 1 out of transit, NaN rows for invalid walkers): nothing has to start at zero
+    return gl_gp_loglike(params, B, times, T, t_exp, n_ss, obs, sigma, gp, loglike_out, scratch, GL_F32, stream);
+}
+
 const char* gl_strerror(int code) {
     switch (code) {
         case GL_OK: return "ok";
         case GL_EINVAL: return "invalid argument";
         case GL_ECUDA: return "CUDA error (see gl_last_cuda_error)";
         case GL_EUNSUPPORTED: return "size not supported";
+        case GL_ECAPACITY: return "size beyond the fixed capacity of a static-scratch entry point";
         default: return "unknown status";
     }
 }
