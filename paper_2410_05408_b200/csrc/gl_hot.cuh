@@ -3,9 +3,10 @@
 // window is short (|phi| <= 0.8 rad), at most MAXEP transits fall inside the series, the star centre can
 // never lie inside the outline's evolute while the outline is near the limb (so the outline crosses the
 // limb at most twice), and the series is sorted.  Simple walkers take the path described below; every
-// other walker is handed, inside the same launch, to generic_unit() -- the full-featured arithmetic of
-// greenlantern_b200.cu (fp64 phases, Kepler, four-crossing search) as a NON-inlined device function:
-// its code is only fetched when a walker needs it.  Invalid walkers: NaN row, chi^2 = +inf.
+// other walker is only NOTED by the main loop and done, inside the same launch, by a second loop behind it
+// that runs generic_unit() -- the full-featured arithmetic of greenlantern_b200.cu (fp64 phases, Kepler,
+// four-crossing search), inlined THERE: behind the common path's code, never fetched unless a walker needs
+// it, and with no call inside the main loop.  Invalid walkers: NaN row, chi^2 = +inf.
 //
 // Why a kernel of its own: round 1's single fused kernel inlined everything -- ~340 KB of SASS (fp64 Kepler, the
 // four-crossing search, libm slow paths); on a K2-shaped batch (config 3) it spent its time in
@@ -435,6 +436,7 @@ struct HotArgs {
 };
 
 enum { CLS_SIMPLE = 0, CLS_INVALID = 1, CLS_DEFER = 2 };
+constexpr int MAXDEFER_WORDS = 1025;   // one bit per unit of a CTA: B * nseg < 2^31 over >= 65535 grid rows
 
 struct Unit {
     // written by the four prelude threads
@@ -547,10 +549,12 @@ __device__ __forceinline__ int lower_bound_warp(const double* __restrict__ seg, 
 // A walker off the common path (eccentric orbit, long window, many transit epochs, evolute regime,
 // unsorted series): the CTA (or cluster) does the unit with the full-featured arithmetic of
 // greenlantern_b200.cu -- fp64 phase of every exposure, Kepler, generic crossing search -- one exposure
-// per lane and pass.  Defined in greenlantern_b200.cu (it needs that file's Walker machinery); NOT
-// inlined: this code is never fetched unless a walker needs it.  Returns CLS_INVALID for an invalid
-// walker (its flux row is NaN-filled), else CLS_SIMPLE with the thread's chi^2 terms added to *acc.
-__device__ int generic_unit(const HotArgs& A, bool pre, int wk, int t_lo, int nT, int gtid, int ntot,
+// per lane and pass.  Defined in greenlantern_b200.cu (it needs that file's Walker machinery) and inlined
+// into hot_kernel's SECOND loop.  (As a real call -- __noinline__, in either loop -- it cost the common path
+// 2 us of 16 on config 3 and 4 of 86 on config 4: the call ABI changes the register allocation of the whole
+// kernel.)  Returns CLS_INVALID for an invalid walker (its flux row is NaN-filled), else CLS_SIMPLE with the
+// thread's chi^2 terms added to *acc.
+__device__ __forceinline__ int generic_unit(const HotArgs& A, bool pre, int wk, int t_lo, int nT, int gtid, int ntot,
                             const glf::TrapNode* trap, double* acc);
 
 template <bool PRE>
@@ -585,8 +589,60 @@ __global__ void __launch_bounds__(HOT_NT, 2) hot_kernel(const HotArgs A) {
     bool started = (csize == 1);
     if (csize > 1) cluster.barrier_arrive();
 
+    // chi^2 of one unit: CTA sum in fixed order, partials pushed into rank 0's shared memory, one cluster
+    // barrier, rank 0 adds them in rank order (used by the common path and by the generic pass below)
+    auto chi2_unit = [&](double acc, int cls, int wk) {
+#pragma unroll
+        for (int off = 16; off > 0; off >>= 1) acc += __shfl_down_sync(0xffffffffu, acc, off);
+        if (lane == 0) s_red[warp] = acc;
+        GLH_DELAY(1);
+        if (!started) {
+            cluster.barrier_wait();
+            started = true;
+        }
+        __syncthreads();
+        if (tid == 0) {
+            double tot = 0.0;
+            for (int k = 0; k < HOT_NW; ++k) tot += s_red[k];
+            GLH_DELAY(2);
+            if (csize > 1) *cluster.map_shared_rank(&s_gather[wpar][crank], 0) = tot;
+            else s_gather[wpar][0] = tot;
+        }
+        GLH_DELAY(3);
+        if (csize > 1) cluster.sync();
+        GLH_DELAY(4);
+        if (crank == 0 && tid == 0) {
+            double d2 = 0.0;
+            for (int r = 0; r < csize; ++r) d2 += s_gather[wpar][r];
+            // raw series: baseline_kernel, launched before this grid (which may have started early:
+            // programmatic dependent launch), writes S into chi2[0..B): wait before touching chi2
+            if (!PRE) asm volatile("griddepcontrol.wait;" ::: "memory");
+            float out;
+            if (cls == CLS_INVALID) {
+                out = __int_as_float(0x7f800000);
+            } else {
+                double Sb = A.S;
+                if (!PRE) Sb = (double)*(volatile float*)&A.chi2[wk];
+                out = (Sb > 1.79769313486231570e308) ? (float)Sb : (float)(Sb + d2);
+            }
+            A.chi2[wk] = out;
+        }
+        GLH_TL(5);
+        wpar ^= 1;
+    };
+
+    // Units off the common path are only NOTED in the main loop (one bit per unit of this CTA) and done in
+    // a second loop behind it, so that the main loop holds the common path's code and nothing else.
+    __shared__ unsigned s_defer[MAXDEFER_WORDS];
     const unsigned nunits = (unsigned)A.B * (unsigned)A.nseg;
-    for (unsigned un = blockIdx.y; un < nunits; un += gridDim.y) {
+    {
+        const unsigned mine = blockIdx.y < nunits ? (nunits - blockIdx.y + gridDim.y - 1) / gridDim.y : 0u;
+        GLH_ASSERT((mine + 31) / 32 <= MAXDEFER_WORDS);
+        for (unsigned i = tid; i < (mine + 31) / 32; i += HOT_NT) s_defer[i] = 0u;   // (barrier: top of the loop)
+    }
+    bool any_defer = false;
+    unsigned kun = 0;
+    for (unsigned un = blockIdx.y; un < nunits; un += gridDim.y, ++kun) {
         const int wk = A.nseg == 1 ? (int)un : (int)(un / (unsigned)A.nseg);
         const int t_lo = (int)(un - (unsigned)wk * (unsigned)A.nseg) * A.seglen;
         const double* __restrict__ seg = A.times + t_lo;
@@ -658,11 +714,11 @@ __global__ void __launch_bounds__(HOT_NT, 2) hot_kernel(const HotArgs A) {
 
         double acc = 0.0;   // this thread's chi^2 terms
         if (cls == CLS_DEFER) {   // (CTA-uniform, and the same in every CTA of a cluster)
-            double gacc = 0.0;    // (its address is taken: kept apart from acc, which stays in registers)
-            cls = generic_unit(A, PRE, wk, t_lo, nT, gtid, ntot, s_trap, &gacc);
-            acc = gacc;
+            if (tid == 0) s_defer[kun >> 5] |= 1u << (kun & 31u);
+            any_defer = true;
+            continue;
         }
-        else if (cls == CLS_INVALID) {
+        if (cls == CLS_INVALID) {
             if (frow)
                 for (int i = gtid; i < nT; i += ntot) frow[i] = __int_as_float(0x7fc00000);
         } else {
@@ -847,46 +903,19 @@ __global__ void __launch_bounds__(HOT_NT, 2) hot_kernel(const HotArgs A) {
             }
         }
         GLH_TL(4);
-        // ---- 4. chi^2: CTA sum in fixed order, partials pushed into rank 0's shared memory, one
-        // cluster barrier, rank 0 adds them in rank order
-        if (want_chi2) {
-#pragma unroll
-            for (int off = 16; off > 0; off >>= 1) acc += __shfl_down_sync(0xffffffffu, acc, off);
-            if (lane == 0) s_red[warp] = acc;
-            GLH_DELAY(1);
-            if (!started) {
-                cluster.barrier_wait();
-                started = true;
-            }
-            __syncthreads();
-            if (tid == 0) {
-                double tot = 0.0;
-                for (int k = 0; k < HOT_NW; ++k) tot += s_red[k];
-                GLH_DELAY(2);
-                if (csize > 1) *cluster.map_shared_rank(&s_gather[wpar][crank], 0) = tot;
-                else s_gather[wpar][0] = tot;
-            }
-            GLH_DELAY(3);
-            if (csize > 1) cluster.sync();
-            GLH_DELAY(4);
-            if (crank == 0 && tid == 0) {
-                double d2 = 0.0;
-                for (int r = 0; r < csize; ++r) d2 += s_gather[wpar][r];
-                // raw series: baseline_kernel, launched before this grid (which may have started early:
-                // programmatic dependent launch), writes S into chi2[0..B): wait before touching chi2
-                if (!PRE) asm volatile("griddepcontrol.wait;" ::: "memory");
-                float out;
-                if (cls == CLS_INVALID) {
-                    out = __int_as_float(0x7f800000);
-                } else {
-                    double Sb = A.S;
-                    if (!PRE) Sb = (double)*(volatile float*)&A.chi2[wk];
-                    out = (Sb > 1.79769313486231570e308) ? (float)Sb : (float)(Sb + d2);
-                }
-                A.chi2[wk] = out;
-            }
-            GLH_TL(5);
-            wpar ^= 1;
+        // ---- 4. chi^2
+        if (want_chi2) chi2_unit(acc, cls, wk);
+    }
+    if (any_defer) {
+        kun = 0;
+        for (unsigned un = blockIdx.y; un < nunits; un += gridDim.y, ++kun) {
+            __syncthreads();   // generic_unit's shared walker of the previous unit is dead; s_defer is visible
+            if (!((s_defer[kun >> 5] >> (kun & 31u)) & 1u)) continue;
+            const int wk = A.nseg == 1 ? (int)un : (int)(un / (unsigned)A.nseg);
+            const int t_lo = (int)(un - (unsigned)wk * (unsigned)A.nseg) * A.seglen;
+            double gacc = 0.0;
+            const int cls = generic_unit(A, PRE, wk, t_lo, min(A.seglen, A.T - t_lo), gtid, ntot, s_trap, &gacc);
+            if (want_chi2) chi2_unit(gacc, cls, wk);
         }
     }
     if (!started) cluster.barrier_wait();

@@ -470,8 +470,8 @@ __device__ __forceinline__ T blocked_fraction(const glf::TrapNode* trap, const W
 // window), fp64 phase of every exposure (any order of the series, any number of transits), Kepler's
 // equation per sub-exposure for e > 0, the generic crossing search where the evolute test asks for it.
 // One exposure per lane and pass, sub-exposures in turn; chi^2 terms in hot_kernel's cancellation-free
-// form.  NOT inlined into hot_kernel: never fetched unless a walker needs it.
-__device__ __noinline__ int glh::generic_unit(const glh::HotArgs& A, bool pre, int wk, int t_lo, int nT,
+// form.  Inlined into hot_kernel's second loop (behind the common path: fetched only when a walker needs it).
+__device__ __forceinline__ int glh::generic_unit(const glh::HotArgs& A, bool pre, int wk, int t_lo, int nT,
                                               int gtid, int ntot, const glf::TrapNode* trap, double* acc) {
     __shared__ Walker gw;
     const int tid = threadIdx.x;
