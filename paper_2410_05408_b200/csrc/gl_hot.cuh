@@ -555,7 +555,8 @@ __device__ __forceinline__ int lower_bound_warp(const double* __restrict__ seg, 
 // kernel.)  Returns CLS_INVALID for an invalid walker (its flux row is NaN-filled), else CLS_SIMPLE with the
 // thread's chi^2 terms added to *acc.
 __device__ __forceinline__ int generic_unit(const HotArgs& A, bool pre, int wk, int t_lo, int nT, int gtid, int ntot,
-                            const glf::TrapNode* trap, double* acc);
+                                            const glf::TrapNode* trap, double* acc, float* s_d, int* s_li,
+                                            int* s_cnt);   // (s_d[CAP], s_li[CAP], s_cnt[HOT_NW]: the kernel's)
 
 template <bool PRE>
 __global__ void __launch_bounds__(HOT_NT, 2) hot_kernel(const HotArgs A) {
@@ -914,7 +915,8 @@ __global__ void __launch_bounds__(HOT_NT, 2) hot_kernel(const HotArgs A) {
             const int wk = A.nseg == 1 ? (int)un : (int)(un / (unsigned)A.nseg);
             const int t_lo = (int)(un - (unsigned)wk * (unsigned)A.nseg) * A.seglen;
             double gacc = 0.0;
-            const int cls = generic_unit(A, PRE, wk, t_lo, min(A.seglen, A.T - t_lo), gtid, ntot, s_trap, &gacc);
+            const int cls = generic_unit(A, PRE, wk, t_lo, min(A.seglen, A.T - t_lo), gtid, ntot, s_trap, &gacc,
+                                         s_d, s_li, &s_cnt[0][0]);
             if (want_chi2) chi2_unit(gacc, cls, wk);
         }
     }

@@ -472,9 +472,10 @@ __device__ __forceinline__ T blocked_fraction(const glf::TrapNode* trap, const W
 // One exposure per lane and pass, sub-exposures in turn; chi^2 terms in hot_kernel's cancellation-free
 // form.  Inlined into hot_kernel's second loop (behind the common path: fetched only when a walker needs it).
 __device__ __forceinline__ int glh::generic_unit(const glh::HotArgs& A, bool pre, int wk, int t_lo, int nT,
-                                              int gtid, int ntot, const glf::TrapNode* trap, double* acc) {
+                                                 int gtid, int ntot, const glf::TrapNode* trap, double* acc,
+                                                 float* s_d, int* s_li, int* s_cnt) {
     __shared__ Walker gw;
-    const int tid = threadIdx.x;
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const double* p = A.params + (size_t)wk * GL_NPARAMS;
     if (tid == 0) walker_prelude_orbit<float>(p, GL_NPARAMS, A.t_exp, &gw);
     if (tid == 32) walker_prelude_shape<float>(p, GL_NPARAMS, &gw);
@@ -487,19 +488,10 @@ __device__ __forceinline__ int glh::generic_unit(const glh::HotArgs& A, bool pre
         return glh::CLS_INVALID;
     }
     const WalkerT<float> v = narrow<float>(gw);
-    const double hwin = gw.half_win_phase, inv_ss = 1.0 / (double)A.n_ss;
-    for (int i = gtid; i < nT; i += ntot) {
-        const double tc = seg[i];
-        if (!(fabs(reduced_phase(gw, tc)) < hwin)) {
-            if (frow) frow[i] = 1.f;
-            continue;
-        }
-        float sum = 0.f;
-        for (int j = 0; j < A.n_ss; ++j) {
-            const double t = tc + (((double)j + 0.5) * inv_ss - 0.5) * A.t_exp;
-            sum += blocked_fraction<float, false>(trap, gw, v, reduced_phase(gw, t));
-        }
-        const float dbar = sum * A.inv_ss;
+    const int S = A.n_ss;
+    const double hwin = gw.half_win_phase, inv_ss = 1.0 / (double)S;
+    // mean over the exposure -> flux and this exposure's chi^2 term (hot_kernel's cancellation-free form)
+    auto finish = [&](int i, float dbar) {
         if (frow) frow[i] = 1.f - dbar;
         if (A.chi2) {
             float ob, rs;
@@ -515,6 +507,63 @@ __device__ __forceinline__ int glh::generic_unit(const glh::HotArgs& A, bool pre
             }
             const float d = dbar * rs;
             *acc += (double)(d * fmaf(2.f * ob, rs, d));
+        }
+    };
+    auto sample = [&](double tc, int j) {
+        const double t = tc + (((double)j + 0.5) * inv_ss - 0.5) * A.t_exp;
+        return blocked_fraction<float, false>(trap, gw, v, reduced_phase(gw, t));
+    };
+    if (S > glh::CAP) {   // (more sub-exposures than the pair buffer holds: one exposure per lane, in turn)
+        for (int i = gtid; i < nT; i += ntot) {
+            const double tc = seg[i];
+            if (!(fabs(reduced_phase(gw, tc)) < hwin)) {
+                if (frow) frow[i] = 1.f;
+                continue;
+            }
+            float sum = 0.f;
+            for (int j = 0; j < S; ++j) sum += sample(tc, j);
+            finish(i, sum * A.inv_ss);
+        }
+        return glh::CLS_SIMPLE;
+    }
+    // Passes of one exposure per thread: window test on the fp64 phase (any order of the series, any number
+    // of transits), in-window indices compacted in thread order (ballot + counts of the 16 warps: the same
+    // list in every run), then lane = (exposure, sub-exposure) pair in groups that fit the pair buffer,
+    // exposure means in sub-exposure order (R18).  In-transit exposures are few and the generic geometry is
+    // long: one exposure per lane with its sub-exposures in turn left most of the CTA idle.
+    const int G = glh::CAP / S;   // exposures per group (>= 1)
+    for (int base = 0; base < nT; base += ntot) {
+        const int i = base + gtid;
+        bool in = false;
+        if (i < nT) {
+            in = fabs(reduced_phase(gw, seg[i])) < hwin;
+            if (!in && frow) frow[i] = 1.f;
+        }
+        const unsigned bal = __ballot_sync(0xffffffffu, in);
+        __syncthreads();   // the previous pass is done with s_li / s_d / s_cnt
+        if (lane == 0) s_cnt[warp] = __popc(bal);
+        __syncthreads();
+        int before = 0, n_in = 0;
+        for (int k = 0; k < glh::HOT_NW; ++k) {
+            const int c = s_cnt[k];
+            before += k < warp ? c : 0;
+            n_in += c;
+        }
+        if (in) s_li[before + __popc(bal & ((1u << lane) - 1u))] = i;
+        __syncthreads();
+        for (int g0 = 0; g0 < n_in; g0 += G) {   // (n_in is the CTA's: the barriers below are uniform)
+            const int ng = min(G, n_in - g0);
+            for (int q = tid; q < ng * S; q += glh::HOT_NT) {
+                const int e = q / S, j = q - e * S;
+                s_d[q] = sample(seg[s_li[g0 + e]], j);
+            }
+            __syncthreads();
+            for (int e = tid; e < ng; e += glh::HOT_NT) {
+                float sum = 0.f;
+                for (int j = 0; j < S; ++j) sum += s_d[e * S + j];
+                finish(s_li[g0 + e], sum * A.inv_ss);
+            }
+            __syncthreads();
         }
     }
     return glh::CLS_SIMPLE;
