@@ -78,6 +78,11 @@ GLF_DEV float mufu_cos(float x) { return cosf(x); }
 #endif
 GLF_DEV float fast_div(float x, float y) { return x / y; }
 #endif
+// pi / nh for nh = 4, 8 or 16 half-nodes of a fixed-angle rule.  A division by a power of two is exact, so
+// the selected constants ARE what the IEEE division gives -- without its slow-path call in the inner code.
+GLF_DEV float pi_over_nodes(int nh) {
+    return nh == 4 ? 0.25f * kPiF : (nh == 8 ? 0.125f * kPiF : (nh == 16 ? 0.0625f * kPiF : kPiF * 0.5f));
+}
 // sin, cos of an angle in [-pi, 3 pi]: folded into [-pi, pi], where the MUFU error is 2^-21.
 GLF_DEV void mufu_sincos(float t, float* s, float* c) {
     const float tr = (t > kPiF) ? t - kTwoPiF : t;
@@ -125,7 +130,7 @@ GLF_DEV float whole_outline_lin(const TrapNode* trap, int nh, float xc, float yc
             acc += pair_term<true>(m2p, ab + w, m2q, ab - w);
         }
     }
-    return acc * (kPiF / float(nh));
+    return acc * pi_over_nodes(nh);
 }
 
 // The same integral with SIX nodes (0, 60, ..., 300 degrees), for outlines deep inside the disc: the

@@ -222,7 +222,7 @@ __device__ __forceinline__ float cheap_delta(const glf::TrapNode* trap, int path
         lin = glf::whole_outline_lin6(xc, yc, a, b, ab, u, v);
     } else {
         const int nh = path == 2 ? 4 : 8;
-        lin = outline_lin_part(trap, nh, 0, 1, xc, yc, a, b, ab, u, v) * (glf::kPiF / float(nh));
+        lin = outline_lin_part(trap, nh, 0, 1, xc, yc, a, b, ab, u, v) * glf::pi_over_nodes(nh);
     }
     return inside_delta(lin, a, b, ab, r0sq, k0, k1, k2);
 }
@@ -312,7 +312,7 @@ __device__ __forceinline__ float near_rest(const glf::TrapNode* trap, float xc, 
             p0 = outline_lin_part(trap, nh, 0, 2, xc, yc, a, b, ab, u, v);
             p1 = outline_lin_part(trap, nh, 1, 2, xc, yc, a, b, ab, u, v);
         }
-        return inside_delta((p0 + p1) * (kPiF / float(nh)), a, b, ab, r0sq, k0, k1, k2);
+        return inside_delta((p0 + p1) * glf::pi_over_nodes(nh), a, b, ab, r0sq, k0, k1, k2);
     }
     // ---- the outline crosses the limb twice (or misses the disc).  tau = t - t_far in [0, 2 pi).
     Arc o = {xc, yc, a, b, cf, sf};
@@ -590,31 +590,50 @@ __global__ void __launch_bounds__(HOT_NT, 2) hot_kernel(const HotArgs A) {
     bool started = (csize == 1);
     if (csize > 1) cluster.barrier_arrive();
 
-    // chi^2 of one unit: CTA sum in fixed order, partials pushed into rank 0's shared memory, one cluster
-    // barrier, rank 0 adds them in rank order (used by the common path and by the generic pass below)
-    auto chi2_unit = [&](double acc, int cls, int wk) {
+    // chi^2 of one unit.  Every step below is a fixed tree or a fixed loop: the same bits in every run of a
+    // launch shape.  The thread's terms (fp64 accumulator of fp32 terms) are narrowed and summed over the warp
+    // in fp32 (5 shuffles; each term carries fp32 rounding already), the <= 16 warp sums go through shared
+    // memory to warp 0, which adds them in fp64 by a shuffle tree; lane 0 adds the series' baseline S and
+    // writes chi^2 -- or, in a cluster, pushes the CTA's sum into rank 0's shared memory, and rank 0 adds
+    // the sums in rank order behind ONE cluster barrier.  A single thread walking the partials (round 1, and
+    // this kernel before) took 1.3 us of config 3's 8 us: dependent shared-memory / fp64 round trips cost
+    // 60-100 cycles each when nothing else runs.
+    // nwsum: only the first nwsum warps can hold non-zero terms (sparse mode: the threads that formed the
+    // exposure means); the others are neither reduced nor read.
+    auto chi2_unit = [&](double acc, int cls, int wk, int nwsum) {
+        if (warp < nwsum) {
+            float part = (float)acc;
 #pragma unroll
-        for (int off = 16; off > 0; off >>= 1) acc += __shfl_down_sync(0xffffffffu, acc, off);
-        if (lane == 0) s_red[warp] = acc;
+            for (int off = 16; off > 0; off >>= 1) part += __shfl_down_sync(0xffffffffu, part, off);
+            if (lane == 0) s_red[warp] = (double)part;
+        }
+        GLH_TL(8);
         GLH_DELAY(1);
         if (!started) {
             cluster.barrier_wait();
             started = true;
         }
         __syncthreads();
-        if (tid == 0) {
-            double tot = 0.0;
-            for (int k = 0; k < HOT_NW; ++k) tot += s_red[k];
+        GLH_TL(9);
+        double tot = 0.0;
+        if (warp == 0) {
+            tot = lane < nwsum ? s_red[lane] : 0.0;
+#pragma unroll
+            for (int off = HOT_NW / 2; off > 0; off >>= 1)
+                if (nwsum > off) tot += __shfl_down_sync(0xffffffffu, tot, off);   // (nwsum is CTA-uniform)
             GLH_DELAY(2);
-            if (csize > 1) *cluster.map_shared_rank(&s_gather[wpar][crank], 0) = tot;
-            else s_gather[wpar][0] = tot;
+            if (csize > 1 && lane == 0) *cluster.map_shared_rank(&s_gather[wpar][crank], 0) = tot;
         }
+        GLH_TL(10);
         GLH_DELAY(3);
         if (csize > 1) cluster.sync();
         GLH_DELAY(4);
         if (crank == 0 && tid == 0) {
-            double d2 = 0.0;
-            for (int r = 0; r < csize; ++r) d2 += s_gather[wpar][r];
+            double d2 = tot;
+            if (csize > 1) {
+                d2 = 0.0;
+                for (int r = 0; r < csize; ++r) d2 += s_gather[wpar][r];
+            }
             // raw series: baseline_kernel, launched before this grid (which may have started early:
             // programmatic dependent launch), writes S into chi2[0..B): wait before touching chi2
             if (!PRE) asm volatile("griddepcontrol.wait;" ::: "memory");
@@ -714,6 +733,7 @@ __global__ void __launch_bounds__(HOT_NT, 2) hot_kernel(const HotArgs A) {
         GLH_TL(2);
 
         double acc = 0.0;   // this thread's chi^2 terms
+        int nwsum = HOT_NW;   // ... and the warps that can hold any
         if (cls == CLS_DEFER) {   // (CTA-uniform, and the same in every CTA of a cluster)
             if (tid == 0) s_defer[kun >> 5] |= 1u << (kun & 31u);
             any_defer = true;
@@ -874,6 +894,7 @@ __global__ void __launch_bounds__(HOT_NT, 2) hot_kernel(const HotArgs A) {
                 __syncthreads();
                 GLH_TL(6);
                 // exposure means, in sub-exposure order (R18)
+                nwsum = min((M + 31) >> 5, HOT_NW);
                 for (int e = tid; e < M; e += HOT_NT) {
                     GLH_ASSERT(e * S + S <= CAP);
                     float sum = 0.f;
@@ -905,7 +926,7 @@ __global__ void __launch_bounds__(HOT_NT, 2) hot_kernel(const HotArgs A) {
         }
         GLH_TL(4);
         // ---- 4. chi^2
-        if (want_chi2) chi2_unit(acc, cls, wk);
+        if (want_chi2) chi2_unit(acc, cls, wk, nwsum);
     }
     if (any_defer) {
         kun = 0;
@@ -917,7 +938,7 @@ __global__ void __launch_bounds__(HOT_NT, 2) hot_kernel(const HotArgs A) {
             double gacc = 0.0;
             const int cls = generic_unit(A, PRE, wk, t_lo, min(A.seglen, A.T - t_lo), gtid, ntot, s_trap, &gacc,
                                          s_d, s_li, &s_cnt[0][0]);
-            if (want_chi2) chi2_unit(gacc, cls, wk);
+            if (want_chi2) chi2_unit(gacc, cls, wk, HOT_NW);
         }
     }
     if (!started) cluster.barrier_wait();
