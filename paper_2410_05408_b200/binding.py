@@ -351,6 +351,7 @@ class GlSeries:
             raise GreenlanternError("times, obs and sigma must be 1-d arrays of one length")
         self._h = ctypes.c_void_p()
         self._loglike = lib.gl_series_loglike
+        self._p_obj = self._p_shape = self._p_addr = self._c_obj = self._c_addr = None
         self.T, self.B_max = int(times.shape[0]), int(B_max)
         self._device = device
         if device is not None:
@@ -371,15 +372,30 @@ class GlSeries:
                 "baseline": base.value}
 
     def loglike(self, params, want_flux=False, chi2_out=None, flux_out=None):
-        if not (type(params) is np.ndarray and params.ndim == 2 and params.dtype == np.float64
-                and params.flags.c_contiguous):
-            params = _host_f64(np.atleast_2d(params))
-        if params.shape[1] != GL_NPARAMS:
-            raise GreenlanternError(f"expected shape [*, {GL_NPARAMS}]")
-        B = params.shape[0]
-        chi2 = _host_out(chi2_out, (B,), np.float32)
+        # An MCMC loop calls this every ~20 us with the SAME arrays: the checks and the address look-ups of
+        # the last params / chi2_out objects are remembered (a reference is held, so identity means the same
+        # live buffer; the shape is compared again because it can be reassigned in place).
+        if params is self._p_obj and params.shape == self._p_shape:
+            paddr, B = self._p_addr, self._p_shape[0]
+        else:
+            obj = params
+            if not (type(params) is np.ndarray and params.ndim == 2 and params.dtype == np.float64
+                    and params.flags.c_contiguous):
+                params = _host_f64(np.atleast_2d(params))
+            if params.shape[1] != GL_NPARAMS:
+                raise GreenlanternError(f"expected shape [*, {GL_NPARAMS}]")
+            paddr, B = _addr(params), params.shape[0]
+            if obj is params:      # (a converted copy is not worth remembering)
+                self._p_obj, self._p_shape, self._p_addr = params, params.shape, paddr
+        if chi2_out is not None and chi2_out is self._c_obj and chi2_out.shape == (B,):
+            chi2, caddr = chi2_out, self._c_addr
+        else:
+            chi2 = _host_out(chi2_out, (B,), np.float32)
+            caddr = _addr(chi2)
+            if chi2_out is not None:
+                self._c_obj, self._c_addr = chi2, caddr
         flux = _host_out(flux_out, (B, self.T), np.float32) if want_flux else None
-        _check(self._loglike(self._h, _addr(params), B, _addr(chi2), _addr(flux) if want_flux else None))
+        _check(self._loglike(self._h, paddr, B, caddr, _addr(flux) if want_flux else None))
         return (chi2, flux) if want_flux else chi2
 
     def loglike_dev(self, params, want_flux=False, chi2_out=None, flux_out=None):

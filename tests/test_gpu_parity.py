@@ -764,6 +764,15 @@ def test_resident_series_api(gl):
     cs_ref, _ = orc.loglike(simple, w.times, w.t_exp, w.n_ss, w.obs, w.sigma)
     for rep in range(2):
         assert np.abs(ser.loglike(simple).astype(np.float64) / cs_ref - 1.0).max() <= 1e-4
+    # the SAME host buffers reused from call to call (the binding remembers their addresses): new contents
+    # written in place must be seen, and another array object of another batch size must not be confused
+    buf, out = simple.copy(), np.empty(64, dtype=np.float32)
+    first = ser.loglike(buf, chi2_out=out).copy()
+    buf[:] = simple[::-1]
+    second = ser.loglike(buf, chi2_out=out)
+    assert second is out and np.array_equal(second[::-1], first)
+    assert np.array_equal(ser.loglike(simple[:8].copy()), first[:8])
+    assert np.array_equal(ser.loglike(buf, chi2_out=out)[::-1], first)
     cd, fd = ser.loglike_dev(dev(p), want_flux=True)
     assert np.array_equal(host(cd), chi.astype(np.float64), equal_nan=True)
     assert np.array_equal(host(fd), flux.astype(np.float64), equal_nan=True)
