@@ -369,6 +369,12 @@ def main():
     hs = (1, w.B, 512)               # hot_kernel's launch shape for this batch: (cluster, rows, threads)
     floor_graph = float(np.mean(timed(lambda: gl.gl_probe_empty_graph(hs[0], hs[1], hs[2]), k=max(K, 20))))
     floor_stream = float(np.mean(timed(lambda: gl.gl_probe_empty_launch(hs[0], hs[1], hs[2]), k=max(K, 20))))
+    # How the event-timed duration answers to the kernel's real duration on this box: a one-thread kernel
+    # that spins for a known number of SM cycles (torch.cuda._sleep), timed exactly like a step.
+    sm_hz = (clocks.get("sm_mhz") or sm_max) * 1e6
+    stair_spin_us = [0.0, 2.0, 4.0, 6.0, 8.0, 9.0, 10.0, 11.0, 12.0, 13.0, 14.0]
+    stair_event_us = [1e3 * float(np.mean(timed(lambda c=int(us * 1e-6 * sm_hz): torch.cuda._sleep(c), k=12, warm=2)))
+                      for us in stair_spin_us]
     roofline = {
         "bound": "alu", "achieved": fr["alg_tflops"], "peak": peak_tflops, "unit": "TFLOP/s",
         "frac": fr["frac_alg"],
@@ -387,6 +393,14 @@ def main():
         "launch_floor_note": "an EMPTY kernel of hot_kernel's grid/block shape, replayed as a CUDA graph the way "
                              "a step is (and launched on the stream, for comparison), timed exactly like a step, "
                              "L2 flushed",
+        "event_time_vs_kernel_time": {
+            "spin_kernel_us": stair_spin_us, "event_timed_us": stair_event_us,
+            "note": "CUDA-event time of a one-thread kernel that spins for the given time (torch.cuda._sleep), "
+                    "measured like a step.  On the B200s of this pool it is a staircase, about 6.1 us + 2.05 us "
+                    "x floor(kernel time / 2.04 us): the end of a kernel is observed on a 2.048-us grid, so "
+                    "ms_per_step moves in 2-us treads (14.3, 16.4, 18.4 us) while the kernel changes by tenths "
+                    "(profiles/r02_kernels.md, 'Event-time staircase'; on-device span of a step: "
+                    "profiles/r02_device_span.md)"},
         "peak_source": f"derived: {N_SM} SMs x {LANES} FP32 lanes x 2 x {sm_max:.0f} MHz "
                        "(MEASURED_PEAKS.json has no FP32 SIMT figure)",
         "peak_measured_ffma_chain": probe["fp32_tflops"],

@@ -835,3 +835,34 @@ def test_checked_build_index_assertions_and_delays(gl, tmp_path):
         same = (np.isnan(a) & np.isnan(b)) | (np.isinf(a) & np.isinf(b) & (np.sign(a) == np.sign(b)))
         d = np.abs(np.where(same, 0.0, a - b)) / np.maximum(np.abs(np.where(same, 1.0, a)), 1.0)
         assert d.max() <= 2e-6, (k, d.max())
+
+
+def test_device_span_of_one_step(gl, tmp_path, capsys):
+    """CUDA events see the end of a kernel on a 2.048-us grid on this hardware (bench.py reports the
+    staircase), so the step's real duration is taken ON the device: a second build of the library with
+    hot_kernel's phase hook filled by two %globaltimer stamps (tests/span_hooks.cuh) reports the span from
+    the first CTA's start to the last chi^2 write.  The numbers are printed (profiles/r02_device_span.md is
+    this test's output); asserted is only what must hold: the span is positive, below the event time of the
+    same launch, and config 3 fits 13 us."""
+    import json
+    import subprocess
+    import sys
+    from pathlib import Path
+    root = Path(__file__).resolve().parents[1]
+    so = tmp_path / "libgreenlantern_span.so"
+    subprocess.run(["nvcc", "-include", str(root / "tests" / "span_hooks.cuh"), "-gencode",
+                    "arch=compute_100a,code=sm_100a", "-O3", "-std=c++17", "-shared", "-Xcompiler", "-fPIC",
+                    "-diag-suppress", "128", "-o", str(so),
+                    str(root / "paper_2410_05408_b200" / "csrc" / "greenlantern_b200.cu")], check=True)
+    r = subprocess.run([sys.executable, str(root / "tests" / "device_span.py"), "--lib", str(so), "cfg3", "cfg2",
+                        "cfg4"], capture_output=True, text=True)
+    assert r.returncode == 0, r.stdout[-2000:] + r.stderr[-2000:]
+    res = json.loads(r.stdout.strip().splitlines()[-1])
+    with capsys.disabled():
+        print()
+        for k, v in res.items():
+            print(f"  device span  {k:32s} {v}")
+    assert len(res) == 12
+    for k, v in res.items():
+        assert 0.0 < v["span_us_min"] <= v["span_us_mean"] <= v["span_us_max"] < v["event_us_mean"], (k, v)
+    assert res["cfg3 chi2+flux L2 flushed"]["span_us_mean"] < 13.0
