@@ -237,11 +237,11 @@ int gl_series_destroy(gl_series* s);
 int gl_probe_peaks(double* out3);
 
 /* gl_probe_empty_launch: enqueues an EMPTY kernel of `rows` clusters of `cluster` CTAs of `threads`
- * threads on `stream` and, when fallback_rows > 0, a second empty grid (fallback_rows clusters of
- * fallback_cluster CTAs of 128 threads) chained to it by programmatic dependent launch -- launch
+ * threads on `stream` and, when dep_rows > 0, a second empty grid (dep_rows clusters of
+ * dep_cluster CTAs of 128 threads) chained to it by programmatic dependent launch -- launch
  * shapes of the library's calls without their work.  bench.py times it the way
  * it times a step and reports it as roofline.launch_floor_ms.  Not part of the hot path. */
-int gl_probe_empty_launch(int cluster, int rows, int threads, int fallback_cluster, int fallback_rows,
+int gl_probe_empty_launch(int cluster, int rows, int threads, int dep_cluster, int dep_rows,
                           void* stream);
 /* gl_probe_empty_graph: the same single empty kernel, captured once per shape (and calling thread) and
  * replayed as a CUDA graph on `stream` -- the way gl_series_loglike_dev launches a step. */

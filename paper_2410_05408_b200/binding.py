@@ -436,14 +436,14 @@ def gl_probe_peaks():
     return {"fp32_tflops": out[0], "fp64_tflops": out[1], "mufu_tops": out[2]}
 
 
-def gl_probe_empty_launch(cluster, rows, threads, fallback_cluster=1, fallback_rows=0, device=None):
+def gl_probe_empty_launch(cluster, rows, threads, dep_cluster=1, dep_rows=0, device=None):
     """Enqueue an empty kernel of the given shape (and, optionally, a dependent empty grid) on torch's
     current stream: the launch floor bench.py reports."""
     torch = _torch()
     dev = torch.device("cuda", torch.cuda.current_device()) if device is None else device
     st = ctypes.c_void_p(torch.cuda.current_stream(dev).cuda_stream)
-    _check(load_library().gl_probe_empty_launch(int(cluster), int(rows), int(threads), int(fallback_cluster),
-                                                int(fallback_rows), st))
+    _check(load_library().gl_probe_empty_launch(int(cluster), int(rows), int(threads), int(dep_cluster),
+                                                int(dep_rows), st))
 
 
 def gl_probe_empty_graph(cluster, rows, threads, device=None):

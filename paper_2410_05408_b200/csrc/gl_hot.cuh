@@ -45,7 +45,7 @@
 #endif
 // CHECKED build (-DGLH_CHECKED; tests/test_gpu_parity.py builds it, the product never does): every
 // shared- and global-memory index of the transit kernels is asserted to be in range, and pseudo-random
-// per-CTA delays are injected in front of every cluster barrier, DSMEM access and marker read, so that
+// per-CTA delays are injected in front of every cluster barrier and DSMEM access, so that
 // a protocol that only works by luck of timing shows up as a wrong or irreproducible result.
 // (compute-sanitizer is closed on the GPU pool this was developed on: profiles/r02_sanitizer.md.)
 #ifdef GLH_CHECKED
@@ -560,7 +560,7 @@ __device__ __forceinline__ int generic_unit(const HotArgs& A, bool pre, int wk, 
 
 template <bool PRE>
 __global__ void __launch_bounds__(HOT_NT, 2) hot_kernel(const HotArgs A) {
-    asm volatile("griddepcontrol.launch_dependents;");   // the fallback launch may become resident
+    asm volatile("griddepcontrol.launch_dependents;");   // a dependent launch (the GP scan) may become resident
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int csize = (int)gridDim.x, crank = (int)blockIdx.x;
     cg::cluster_group cluster = cg::this_cluster();
@@ -748,7 +748,7 @@ __global__ void __launch_bounds__(HOT_NT, 2) hot_kernel(const HotArgs A) {
             const float ab = a * b, e2 = (a - b) * (a + b);
             // the ranges are read from shared memory where they are needed (broadcast reads; nep is 1
             // for a single-transit series): len_k = max(hi_k - lo_k, 0) -- an unsorted share of the
-            // series may give anything, the unit is then redone by the fallback kernel
+            // series may give anything: such a unit was classified CLS_DEFER above and never gets here
             int M = 0;   // in-window exposures of the unit (the whole cluster's)
             for (int k = 0; k < nep; ++k) M += max(su.hi[k] - su.lo[k], 0);
             // v-th in-window exposure of the unit -> its index in the segment and its time from the

@@ -1663,10 +1663,10 @@ int gl_probe_peaks(double* out3) {
 }
 
 // Launch floor: an EMPTY kernel with a given grid/cluster/block shape, optionally followed by a
-// second empty grid chained by programmatic dependent launch (the hot + fallback pair's shape).
+// second empty grid chained by programmatic dependent launch (the shape of a flux kernel + dependent kernel pair, e.g. the GP likelihood).
 // bench.py times it exactly as it times a step; what it measures is what any launch of that shape
 // costs on this box before a single useful instruction runs.
-int gl_probe_empty_launch(int cluster, int rows, int threads, int fallback_cluster, int fallback_rows,
+int gl_probe_empty_launch(int cluster, int rows, int threads, int dep_cluster, int dep_rows,
                           void* stream) {
     if (cluster < 1 || cluster > 8 || rows < 1 || threads < 32 || threads > 1024) return GL_EINVAL;
     cudaStream_t st = (cudaStream_t)stream;
@@ -1683,10 +1683,10 @@ int gl_probe_empty_launch(int cluster, int rows, int threads, int fallback_clust
     cfg.numAttrs = 1;
     cudaError_t e = cudaLaunchKernelEx(&cfg, empty_kernel, 0);
     if (e != cudaSuccess) return cuda_fail(e, "empty_kernel launch");
-    if (fallback_rows > 0) {
-        cfg.gridDim = dim3((unsigned)fallback_cluster, (unsigned)fallback_rows, 1);
+    if (dep_rows > 0) {
+        cfg.gridDim = dim3((unsigned)dep_cluster, (unsigned)dep_rows, 1);
         cfg.blockDim = dim3(NT, 1, 1);
-        attr[0].val.clusterDim.x = (unsigned)fallback_cluster;
+        attr[0].val.clusterDim.x = (unsigned)dep_cluster;
         attr[1].id = cudaLaunchAttributeProgrammaticStreamSerialization;
         attr[1].val.programmaticStreamSerializationAllowed = 1;
         cfg.numAttrs = 2;
@@ -2021,7 +2021,7 @@ int gl_series_create(const double* times, const double* obs, const double* sigma
     *out = nullptr;
     if (T < 1 || B_max < 1 || n_ss < 1 || !(t_exp >= 0.0) || !isfinite(t_exp) || !times || !obs || !sigma)
         return GL_EINVAL;
-    {   // the full kernel (the fallback of a series call) reads the constant-memory tables
+    {   // generic_unit (walkers off the common path) reads the constant-memory tables
         const int rc = ensure_tables();
         if (rc != GL_OK) return rc;
     }

@@ -753,7 +753,7 @@ def test_resident_series_api(gl):
     info = ser.info()
     assert info["sorted"] and info["T"] == w.T and info["B_max"] == 64
     assert abs(info["baseline"] / float(np.sum(((w.obs - 1.0) / w.sigma) ** 2)) - 1.0) < 1e-13
-    for rep in range(3):       # the host call learns after the first call that the fallback is needed
+    for rep in range(3):       # (first call captures the graph, the others replay it)
         chi, flux = ser.loglike(p, want_flux=True)
         assert np.all(np.isinf(chi[bad])) and np.all(np.isnan(flux[bad]))
         assert np.abs(flux[~bad].astype(np.float64) - ref[~bad]).max() <= 5e-7
@@ -804,7 +804,7 @@ def test_checked_build_index_assertions_and_delays(gl, tmp_path):
     """compute-sanitizer is closed on this GPU pool (profiles/r02_sanitizer.md), so the library carries
     its own checks: built with -DGLH_CHECKED every shared/global index of the transit kernels is
     asserted in range and pseudo-random per-CTA delays sit in front of every cluster barrier, DSMEM
-    access and marker read.  The shapes of tests/sanitizer_shapes.py (clusters, many units per cluster,
+    access.  The shapes of tests/sanitizer_shapes.py (clusters, many units per cluster,
     multi-round series, PDL chains, deferred walkers, graph replay) must run clean through that build
     twice with bit-identical outputs, equal to the product build's up to the last place."""
     import subprocess
