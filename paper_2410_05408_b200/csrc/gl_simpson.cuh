@@ -32,9 +32,16 @@ template <> struct trig<double> {
 };
 
 // The three integrands of eqs. 21-23 at one (possibly snapped) node, times the Simpson weight w.
+// r^2 of a node, on which the snap decision r^2 > 1 hangs.  The integrand of eq. 23 is discontinuous across
+// the snap, so a node within rounding of the limb (a tangent outline) must be judged with the SAME arithmetic
+// by everyone who evaluates the definition: in fp64 plain IEEE products and sums in the written order, no
+// contraction into FMAs (fp32 is a different precision anyway: its nodes may flip).
+__device__ __forceinline__ float node_r2(float x, float y) { return x * x + y * y; }
+__device__ __forceinline__ double node_r2(double x, double y) { return __dadd_rn(__dmul_rn(x, x), __dmul_rn(y, y)); }
+
 template <typename T>
 __device__ __forceinline__ void add_node(T x, T y, T xp, T yp, T w, T* acc) {
-    T r2 = x * x + y * y;
+    T r2 = node_r2(x, y);
     if (r2 > T(1)) {
         // eqs. 16-19: snap radially onto the limb; cos(lambda) = x / r, sin(lambda) = y / r
         const T dlam = (x * yp - y * xp) / r2;
@@ -84,9 +91,23 @@ simpson_kernel(const double* __restrict__ geom, long long N, int n_int, T* __res
     const T inv_n = T(1) / T(n_int);
     // composite Simpson on the closed contour: node 0 = node n_int carries weight 1 + 1 = 2
     for (int k = lane; k < n_int; k += 32) {
-        T s, c;
-        trig<T>::sincos2pi(T(k) * inv_n, &s, &c);
-        const T x = x0 + dx * c, y = dy1 * c + dy2 * s;        // eqs. 7-8
+        T s, c, x, y;
+        if (sizeof(T) == 8) {
+            // fp64 (validation path): theta_k = k h with h = 2 pi / n as the definition writes it (at a tangent
+            // node the last bit of sin(theta_k) decides the snap: sin(pi) must be 1.2e-16, not sinpi(1) = 0),
+            // and eqs. 7-8 in plain IEEE operations in the written order (see node_r2)
+            const double h = 2.0 * 3.14159265358979323846 / (double)n_int;
+            double sd, cd;
+            sincos((double)k * h, &sd, &cd);
+            s = (T)sd;
+            c = (T)cd;
+            x = (T)__dadd_rn((double)x0, __dmul_rn((double)dx, cd));
+            y = (T)__dadd_rn(__dmul_rn((double)dy1, cd), __dmul_rn((double)dy2, sd));
+        } else {
+            trig<T>::sincos2pi(T(k) * inv_n, &s, &c);
+            x = x0 + dx * c;                                    // eqs. 7-8
+            y = dy1 * c + dy2 * s;
+        }
         const T xp = -dx * s, yp = dy2 * c - dy1 * s;           // eqs. 14-15
         add_node<T>(x, y, xp, yp, (k & 1) ? T(4) : T(2), acc);
     }
