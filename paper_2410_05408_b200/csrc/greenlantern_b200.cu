@@ -1115,30 +1115,24 @@ geometry_sorted_kernel(const double* __restrict__ geom, long long N, float* __re
 
 // Second launch of the fp32 bare-geometry call (programmatic dependent launch behind
 // geometry_sorted_kernel): the rows that kernel marked -- star centre possibly inside the outline's
-// evolute: up to four crossings, generic bracketed search (gl_core.cuh) -- gathered from EVO_ROWS rows of
-// the output into one list per CTA and evaluated with full warps.
-constexpr int EVO_NT = 256, EVO_ROWS = 2048;   // rows looked at per round of a CTA
+// evolute: up to four crossings, generic bracketed search (gl_core.cuh).  They are few (config 5: a few per
+// cent) and ~10x longer than any other row.  A CTA walks its share of the output in rounds of EVO_ROWS rows,
+// keeps appending the marked ones to one list (ballot + one shared counter update per warp) and evaluates the
+// list when the next round might overflow it or at the end.  Grid: EVO_CTAS_PER_SM CTAs per SM -- measured on
+// config 5 (1e6 rows): 1 per SM (135 rows per CTA, full warps) 117 us for the call, 2 per SM 96 us, 4 per SM
+// 90 us (round 2 before: 102 us): one evaluation is a ~50-us dependent chain, so warps in flight beat full
+// warps; lanes per instruction stay ~10 either way (the divergence is inside overlap_areas).
+constexpr int EVO_NT = 256, EVO_ROWS = 1024, EVO_CAP = 2048;   // rows looked at per round; list capacity
+constexpr int EVO_CTAS_PER_SM = 4;
 __global__ void __launch_bounds__(EVO_NT)
 geometry_evolute_kernel(const double* __restrict__ geom, long long N, float* out) {
-    __shared__ long long s_rows[EVO_ROWS];
+    __shared__ long long s_rows[EVO_CAP];
     __shared__ int s_n;
-    const int tid = threadIdx.x;
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    if (tid == 0) s_n = 0;
     asm volatile("griddepcontrol.wait;" ::: "memory");
-    // blocks of 32 rows, round-robin over the CTAs (see geometry_sorted_kernel); a CTA looks at EVO_ROWS
-    // rows per round, lists the marked ones and evaluates them
-    const long long nblocks = (N + 31) / 32;
-    for (long long b0 = blockIdx.x; b0 < nblocks; b0 += (long long)gridDim.x * (EVO_ROWS / 32)) {
-        __syncthreads();
-        if (tid == 0) s_n = 0;
-        __syncthreads();
-        for (int r = tid; r < EVO_ROWS; r += EVO_NT) {
-            const long long blk = b0 + (long long)(r >> 5) * gridDim.x;
-            const long long k = blk * 32 + (r & 31);
-            if (blk < nblocks && k < N && *reinterpret_cast<const volatile uint32_t*>(out + k) == GEO_MARK)
-                s_rows[atomicAdd(&s_n, 1)] = k;
-        }
-        __syncthreads();
-        const int n = s_n;
+    __syncthreads();
+    auto evaluate = [&](int n) {
         for (int j = tid; j < n; j += EVO_NT) {
             const long long k = s_rows[j];
             const double* g = geom + k * GL_NGEOM;
@@ -1154,7 +1148,34 @@ geometry_evolute_kernel(const double* __restrict__ geom, long long N, float* out
                              fmaf((float)(u1 + 2.0 * u2) * ipn, A[1], (float)u2 * ipn * A[2]));
             out[k] = 1.f - delta;
         }
+    };
+    // blocks of 32 rows, round-robin over the CTAs (see geometry_sorted_kernel); warp w of the CTA takes
+    // the CTA's blocks w, w + 8, ... of a round
+    const long long nblocks = (N + 31) / 32;
+    for (long long b0 = blockIdx.x; b0 < nblocks; b0 += (long long)gridDim.x * (EVO_ROWS / 32)) {
+        for (int r = warp; r < EVO_ROWS / 32; r += EVO_NT / 32) {
+            const long long blk = b0 + (long long)r * gridDim.x;
+            const long long k = blk * 32 + lane;
+            const bool marked = blk < nblocks && k < N &&
+                                *reinterpret_cast<const volatile uint32_t*>(out + k) == GEO_MARK;
+            const unsigned bal = __ballot_sync(0xffffffffu, marked);
+            if (bal) {   // (warp-uniform)
+                int base = 0;
+                if (lane == 0) base = atomicAdd(&s_n, __popc(bal));
+                base = __shfl_sync(0xffffffffu, base, 0);
+                if (marked) s_rows[base + __popc(bal & ((1u << lane) - 1u))] = k;
+            }
+        }
+        __syncthreads();
+        const int n = s_n;
+        if (n > EVO_CAP - EVO_ROWS) {   // the next round might not fit: evaluate what is listed (CTA-uniform)
+            evaluate(n);
+            __syncthreads();
+            if (tid == 0) s_n = 0;
+            __syncthreads();
+        }
     }
+    evaluate(s_n);
 }
 
 // ------------------------------------------------------------------------------------------
@@ -1529,8 +1550,8 @@ int gl_flux_geometry(const double* geom, long long N, void* flux_out, gl_dtype d
         if (e1 != cudaSuccess) return cuda_fail(e1, "geometry_sorted_kernel launch");
         ++tl_launches;
         cudaLaunchConfig_t cfg = {};
-        {   // as many CTAs as keep every SM busy, but no more than there are rounds of EVO_ROWS rows
-            const long long want = (N + EVO_ROWS - 1) / EVO_ROWS, room = (long long)sm_count() * 4;
+        {   // EVO_CTAS_PER_SM CTAs per SM, but no more than there are rounds of EVO_ROWS rows
+            const long long want = (N + EVO_ROWS - 1) / EVO_ROWS, room = (long long)sm_count() * EVO_CTAS_PER_SM;
             cfg.gridDim = dim3((unsigned)(want < room ? want : room), 1, 1);
         }
         cfg.blockDim = dim3(EVO_NT, 1, 1);
