@@ -226,102 +226,141 @@ template <typename T> GL_DEV void add_limb_arc(T xa, T ya, T xb, T yb, T* A) {
 //   t_a < t* and a local maximum t_b > t* of g).  Between consecutive critical points g is
 //   monotone, so each crossing is the single root of g in a known bracket: no quartic algebra.
 // ---------------------------------------------------------------------------------------------
-template <typename T, int NQ, bool FT = false>
-GL_DEV bool overlap_areas(T xc_in, T yc_in, T a, T b, const T* qphi, const T* qom, T* A) {
-    const T pi = num<T>::pi, half = T(0.5) * pi;
-    // quadrant boundaries pulled strictly inside their quadrant, so that a rounded boundary can
-    // never sit on the far side of a neighbouring critical point
-    const T q1hi = half * (T(1) - num<T>::nudge), q2lo = half * (T(1) + num<T>::nudge);
-    const T q2hi = pi * (T(1) - num<T>::nudge), q3lo = pi * (T(1) + num<T>::nudge);
-    const T q3hi = T(3) * half * (T(1) - num<T>::nudge);
+// The search is written in three stages so that a kernel can run each stage over a list of its own (the
+// bare-geometry kernel sorts its rows between them); overlap_areas() below runs them back to back.
+template <typename T> struct CritPoints {   // stage 1: the critical points of g and g there
+    T tfar, gfar, ta, tb, ga, gb;
+    bool evol;                              // the pair (ta, tb) exists
+};
+template <typename T> struct ArcPlan {      // stage 2: the arcs of the outline that lie inside the disc
+    T as[2], ae[2];
+    int narc;                               // 0: no overlap
+    bool limb;                              // the contour is closed along the limb
+};
+template <typename T> GL_DEV Outline<T> make_outline(T xc_in, T yc_in, T a, T b) {
     Outline<T> o;
     o.xc = gabs(xc_in);
     o.yc = gabs(yc_in);
     o.a = a;
     o.b = b;
     o.e2 = (a - b) * (a + b);
+    return o;
+}
+// Stage 1.  false: the outline cannot reach the disc.
+template <typename T, bool FT>
+GL_DEV bool critical_points(const Outline<T>& o, CritPoints<T>* cp) {
+    const T pi = num<T>::pi, half = T(0.5) * pi;
+    // quadrant boundaries pulled strictly inside their quadrant, so that a rounded boundary can
+    // never sit on the far side of a neighbouring critical point
+    const T q1hi = half * (T(1) - num<T>::nudge), q2lo = half * (T(1) + num<T>::nudge);
+    const T q2hi = pi * (T(1) - num<T>::nudge);
     const T r0sq = o.xc * o.xc + o.yc * o.yc;
-    if (r0sq >= (T(1) + a) * (T(1) + a)) return false;
-
-    const T Aa = a * o.xc, Bb = b * o.yc;
-    T g, hd;
-    T tfar = T(0);
-    if (Aa > T(0) || Bb > T(0)) tfar = solve_in<T, 1, FT>(o, T(0), q1hi, gatan2(Bb, Aa), false);
-    T gfar;
-    eval_g<T, FT>(o, tfar, &gfar, &hd);
-
-    bool evol = false;
-    T ta = T(0), tb = T(0), ga = T(0), gb = T(0);
+    if (r0sq >= (T(1) + o.a) * (T(1) + o.a)) return false;
+    const T Aa = o.a * o.xc, Bb = o.b * o.yc;
+    T hd;
+    cp->tfar = T(0);
+    if (Aa > T(0) || Bb > T(0)) cp->tfar = solve_in<T, 1, FT>(o, T(0), q1hi, gatan2(Bb, Aa), false);
+    eval_g<T, FT>(o, cp->tfar, &cp->gfar, &hd);
+    cp->evol = false;
+    cp->ta = cp->tb = cp->ga = cp->gb = T(0);
     if (Aa < o.e2 && Bb < o.e2) {
         const T cA = gcbrt(Aa), cB = gcbrt(Bb), cE = gcbrt(o.e2);
         if (cA * cA + cB * cB < cE * cE) {
-            evol = true;
+            cp->evol = true;
             const T tstar = gmin(gmax(pi - gatan2(cB, cA), q2lo), q2hi);
-            ta = solve_in<T, 1, FT>(o, q2lo, tstar, T(0.5) * (q2lo + tstar), true);
-            tb = solve_in<T, 1, FT>(o, tstar, q2hi, T(0.5) * (tstar + q2hi), false);
-            eval_g<T, FT>(o, ta, &ga, &hd);
-            eval_g<T, FT>(o, tb, &gb, &hd);
+            cp->ta = solve_in<T, 1, FT>(o, q2lo, tstar, T(0.5) * (q2lo + tstar), true);
+            cp->tb = solve_in<T, 1, FT>(o, tstar, q2hi, T(0.5) * (tstar + q2hi), false);
+            eval_g<T, FT>(o, cp->ta, &cp->ga, &hd);
+            eval_g<T, FT>(o, cp->tb, &cp->gb, &hd);
         }
     }
-
-    T as[2], ae[2];   // inside arcs [as, ae]
-    int narc = 1;
-    bool limb = true;
-    if (gfar <= T(0)) {
-        // the whole outline is inside the disc: open the contour at the point nearest the limb
-        limb = false;
-        as[0] = tfar;
-        ae[0] = tfar + T(2) * pi;
-        if (evol) {
-            narc = 2;
-            ae[0] = tb;
-            as[1] = tb;
-            ae[1] = tfar + T(2) * pi;
-        }
+    return true;
+}
+// Stage 2a: the whole outline is inside the disc (gfar <= 0): open the contour at the point nearest the limb.
+template <typename T> GL_DEV void plan_inside(const CritPoints<T>& cp, ArcPlan<T>* pl) {
+    const T pi = num<T>::pi;
+    pl->limb = false;
+    pl->narc = 1;
+    pl->as[0] = cp.tfar;
+    pl->ae[0] = cp.tfar + T(2) * pi;
+    if (cp.evol) {
+        pl->narc = 2;
+        pl->ae[0] = cp.tb;
+        pl->as[1] = cp.tb;
+        pl->ae[1] = cp.tfar + T(2) * pi;
+    }
+}
+// Stage 2b: gfar > 0: the nearest point and the crossings.  narc = 0: the outline misses the disc.
+template <typename T, bool FT>
+GL_DEV void plan_crossing(const Outline<T>& o, const CritPoints<T>& cp, ArcPlan<T>* pl) {
+    const T pi = num<T>::pi, half = T(0.5) * pi;
+    const T q3lo = pi * (T(1) + num<T>::nudge), q3hi = T(3) * half * (T(1) - num<T>::nudge);
+    const T Aa = o.a * o.xc, Bb = o.b * o.yc;
+    const T tfar = cp.tfar, gfar = cp.gfar, ta = cp.ta, tb = cp.tb, ga = cp.ga, gb = cp.gb;
+    T* as = pl->as;
+    T* ae = pl->ae;
+    pl->limb = true;
+    pl->narc = 0;
+    const T tnear = solve_in<T, 1, FT>(o, q3lo, q3hi, pi + gatan2(Bb, Aa), true);
+    T gnear, hd;
+    eval_g<T, FT>(o, tnear, &gnear, &hd);
+    if (gnear >= T(0)) return;
+    pl->narc = 1;
+    const T tend = tfar + T(2) * pi;
+    const T rexit = solve_in<T, 0, FT>(o, tnear, tend, cosine_guess(tnear, tend, gnear, gfar), true);
+    if (!cp.evol) {
+        as[0] = solve_in<T, 0, FT>(o, tfar, tnear, cosine_guess(tfar, tnear, gfar, gnear), false);
+        ae[0] = rexit;
+    } else if (ga < T(0) && gb > T(0)) {
+        pl->narc = 2;
+        as[0] = solve_in<T, 0, FT>(o, tfar, ta, cosine_guess(tfar, ta, gfar, ga), false);
+        ae[0] = solve_in<T, 0, FT>(o, ta, tb, cosine_guess(ta, tb, ga, gb), true);
+        as[1] = solve_in<T, 0, FT>(o, tb, tnear, cosine_guess(tb, tnear, gb, gnear), false);
+        ae[1] = rexit;
+    } else if (ga >= T(0)) {
+        as[0] = solve_in<T, 0, FT>(o, tb, tnear, cosine_guess(tb, tnear, gb, gnear), false);
+        ae[0] = rexit;
     } else {
-        const T tnear = solve_in<T, 1, FT>(o, q3lo, q3hi, pi + gatan2(Bb, Aa), true);
-        T gnear;
-        eval_g<T, FT>(o, tnear, &gnear, &hd);
-        if (gnear >= T(0)) return false;
-        const T tend = tfar + T(2) * pi;
-        const T rexit = solve_in<T, 0, FT>(o, tnear, tend, cosine_guess(tnear, tend, gnear, gfar), true);
-        if (!evol) {
-            as[0] = solve_in<T, 0, FT>(o, tfar, tnear, cosine_guess(tfar, tnear, gfar, gnear), false);
-            ae[0] = rexit;
-        } else if (ga < T(0) && gb > T(0)) {
-            narc = 2;
-            as[0] = solve_in<T, 0, FT>(o, tfar, ta, cosine_guess(tfar, ta, gfar, ga), false);
-            ae[0] = solve_in<T, 0, FT>(o, ta, tb, cosine_guess(ta, tb, ga, gb), true);
-            as[1] = solve_in<T, 0, FT>(o, tb, tnear, cosine_guess(tb, tnear, gb, gnear), false);
-            ae[1] = rexit;
-        } else if (ga >= T(0)) {
-            as[0] = solve_in<T, 0, FT>(o, tb, tnear, cosine_guess(tb, tnear, gb, gnear), false);
-            ae[0] = rexit;
-        } else {
-            // local maximum at t_b stays inside the disc: split there (near-singular integrand)
-            narc = 2;
-            as[0] = solve_in<T, 0, FT>(o, tfar, ta, cosine_guess(tfar, ta, gfar, ga), false);
-            ae[0] = tb;
-            as[1] = tb;
-            ae[1] = rexit;
-        }
+        // local maximum at t_b stays inside the disc: split there (near-singular integrand)
+        pl->narc = 2;
+        as[0] = solve_in<T, 0, FT>(o, tfar, ta, cosine_guess(tfar, ta, gfar, ga), false);
+        ae[0] = tb;
+        as[1] = tb;
+        ae[1] = rexit;
     }
-
+}
+// Stage 3: the boundary integrals along the planned arcs (and the limb arcs that close the contour).
+template <typename T, int NQ, bool FT>
+GL_DEV void integrate_plan(const Outline<T>& o, const ArcPlan<T>& pl, const T* qphi, const T* qom, T* A) {
     const ArcCoef<T> k = arc_coefficients(o);
     A[0] = A[1] = A[2] = T(0);
     T ss[2], cs[2], se[2], ce[2];
-    for (int i = 0; i < narc; ++i) {
-        gtrig<FT>(as[i], &ss[i], &cs[i]);
-        gtrig<FT>(ae[i], &se[i], &ce[i]);
-        add_outline_arc<T, NQ, FT>(o, k, as[i], ss[i], cs[i], ae[i], se[i], ce[i], qphi, qom, A);
+    for (int i = 0; i < pl.narc; ++i) {
+        gtrig<FT>(pl.as[i], &ss[i], &cs[i]);
+        gtrig<FT>(pl.ae[i], &se[i], &ce[i]);
+        add_outline_arc<T, NQ, FT>(o, k, pl.as[i], ss[i], cs[i], pl.ae[i], se[i], ce[i], qphi, qom, A);
     }
-    if (limb) {
-        for (int i = 0; i < narc; ++i) {
-            const int j = (i + 1 == narc) ? 0 : i + 1;
-            add_limb_arc(o.xc + a * ce[i], o.yc + b * se[i], o.xc + a * cs[j], o.yc + b * ss[j], A);
+    if (pl.limb) {
+        for (int i = 0; i < pl.narc; ++i) {
+            const int j = (i + 1 == pl.narc) ? 0 : i + 1;
+            add_limb_arc(o.xc + o.a * ce[i], o.yc + o.b * se[i], o.xc + o.a * cs[j], o.yc + o.b * ss[j], A);
         }
     }
-    (void)g;
+}
+
+template <typename T, int NQ, bool FT = false>
+GL_DEV bool overlap_areas(T xc_in, T yc_in, T a, T b, const T* qphi, const T* qom, T* A) {
+    const Outline<T> o = make_outline(xc_in, yc_in, a, b);
+    CritPoints<T> cp;
+    if (!critical_points<T, FT>(o, &cp)) return false;
+    ArcPlan<T> pl;
+    if (cp.gfar <= T(0)) {
+        plan_inside(cp, &pl);
+    } else {
+        plan_crossing<T, FT>(o, cp, &pl);
+        if (pl.narc == 0) return false;
+    }
+    integrate_plan<T, NQ, FT>(o, pl, qphi, qom, A);
     return true;
 }
 

@@ -1118,35 +1118,172 @@ geometry_sorted_kernel(const double* __restrict__ geom, long long N, float* __re
 // evolute: up to four crossings, generic bracketed search (gl_core.cuh).  They are few (config 5: a few per
 // cent) and ~10x longer than any other row.  A CTA walks its share of the output in rounds of EVO_ROWS rows,
 // keeps appending the marked ones to one list (ballot + one shared counter update per warp) and evaluates the
-// list when the next round might overflow it or at the end.  Grid: EVO_CTAS_PER_SM CTAs per SM -- measured on
-// config 5 (1e6 rows): 1 per SM (135 rows per CTA, full warps) 117 us for the call, 2 per SM 96 us, 4 per SM
-// 90 us (round 2 before: 102 us): one evaluation is a ~50-us dependent chain, so warps in flight beat full
-// warps; lanes per instruction stay ~10 either way (the divergence is inside overlap_areas).
-constexpr int EVO_NT = 256, EVO_ROWS = 1024, EVO_CAP = 2048;   // rows looked at per round; list capacity
+// list when the next round might overflow it or at the end.  Grid: EVO_CTAS_PER_SM CTAs per SM (what fits at
+// 55 registers and 40 KB of shared memory): one evaluation is a long dependent chain, so warps in flight count
+// for more than full lists -- config 5 (1e6 rows), the whole call: 2 per SM 72.9 us, 3 70.1, 4 68.1, 5 (a
+// second wave) 86.3.
+constexpr int EVO_NT = 256, EVO_ROWS = 256, EVO_CAP = 512;   // rows looked at per round; list capacity
 constexpr int EVO_CTAS_PER_SM = 4;
+// The evaluation itself is glc::overlap_areas cut at its stage boundaries (gl_core.cuh), with the rows
+// RE-LISTED between the stages, so that a warp runs one stage for 32 rows that all need it:
+//   E1  every listed row: critical points of g (3 root searches); outline wholly inside the disc -> its arcs
+//       are known; else the row goes on the crossing list
+//   E2  crossing list: nearest point, exit and entry crossings (2-5 root searches) -> arcs, or no overlap
+//   E3  arc list, one lane per ARC (a row has one or two): the three boundary integrals of the arc
+//   E4  every row with arcs: the arcs' sums in arc order, the limb arcs that close the contour, the flux
+// Every result lands in a slot fixed by its row (and arc number): the order in which rows enter a list
+// (atomics) changes nothing.  Measured on config 5: one lane per row through all of overlap_areas ran at 9.5 of
+// 32 lanes, 13.6 M warp instructions, 54 us; staged 16.5 lanes, 9.5 M, 34.6 us (the call: 89.9 -> 68.1 us).
+struct EvoRow {
+    glc::Outline<float> o;
+    float k0, k1, k2;
+};
+__device__ __forceinline__ EvoRow evo_row(const double* __restrict__ geom, long long k) {
+    const double* g = geom + k * GL_NGEOM;
+    const double d = g[0], Rp = g[1], fp = g[2], pa = g[3], u1 = g[4], u2 = g[5];
+    float s, c;
+    glh::angle_sincos(pa, &s, &c);   // (the same preparation as geometry_sorted_kernel)
+    const float a = (float)Rp, b = (float)(Rp * (1.0 - fp)), r0 = (float)d;
+    const float ipn = glh::rcp_nr((float)(kPi * (1.0 - u1 / 3.0 - u2 / 6.0)));
+    EvoRow r;
+    r.o = glc::make_outline(fabsf(r0 * c), fabsf(r0 * s), a, b);
+    r.k0 = (float)(1.0 - u1 - 2.0 * u2) * ipn;
+    r.k1 = (float)(u1 + 2.0 * u2) * ipn;
+    r.k2 = (float)u2 * ipn;
+    return r;
+}
 __global__ void __launch_bounds__(EVO_NT)
 geometry_evolute_kernel(const double* __restrict__ geom, long long N, float* out) {
     __shared__ long long s_rows[EVO_CAP];
-    __shared__ int s_n;
+    __shared__ float s_cp[6][EVO_CAP];            // tfar, gfar, ta, tb, ga, gb of a row
+    __shared__ unsigned char s_flag[EVO_CAP];     // bit 0: the pair (ta, tb) exists; bits 1-2: arcs; bit 3: limb
+    __shared__ unsigned short s_cross[EVO_CAP];   // E2's list (positions in s_rows)
+    __shared__ unsigned short s_arcs[2 * EVO_CAP];   // E3's list (arc slots: 2 * position + arc number)
+    __shared__ float s_as[2 * EVO_CAP], s_ae[2 * EVO_CAP], s_A[3][2 * EVO_CAP];   // per arc slot
+    __shared__ int s_n, s_ncross, s_narcs;
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     if (tid == 0) s_n = 0;
     asm volatile("griddepcontrol.wait;" ::: "memory");
     __syncthreads();
+    // warp-aggregated append to a shared list (the ballot is taken by all 32 lanes)
+    auto append = [&](bool mine, int* counter, unsigned short* list, int value) {
+        const unsigned bal = __ballot_sync(0xffffffffu, mine);
+        if (!bal) return;
+        int base = 0;
+        if (lane == 0) base = atomicAdd(counter, __popc(bal));
+        base = __shfl_sync(0xffffffffu, base, 0);
+        if (mine) list[base + __popc(bal & ((1u << lane) - 1u))] = (unsigned short)value;
+    };
+    auto push_arcs = [&](int j, const glc::ArcPlan<float>& pl) {   // (narc > 0)
+        s_flag[j] = (unsigned char)((s_flag[j] & 1u) | (pl.narc << 1) | (pl.limb ? 8u : 0u));
+        for (int i = 0; i < pl.narc; ++i) {
+            s_as[2 * j + i] = pl.as[i];
+            s_ae[2 * j + i] = pl.ae[i];
+        }
+    };
     auto evaluate = [&](int n) {
+        if (tid == 0) s_ncross = s_narcs = 0;
+        __syncthreads();
+        // ---- E1
+        for (int j0 = 0; j0 < n; j0 += EVO_NT) {   // (whole warps stay in the loop: the appends vote)
+            const int j = j0 + tid;
+            bool cross = false;
+            int narc = 0;
+            if (j < n) {
+                const EvoRow r = evo_row(geom, s_rows[j]);
+                glc::CritPoints<float> cp;
+                s_flag[j] = 0;
+                if (!glc::critical_points<float, true>(r.o, &cp)) {
+                    out[s_rows[j]] = 1.f;
+                } else {
+                    s_cp[0][j] = cp.tfar;
+                    s_cp[1][j] = cp.gfar;
+                    s_cp[2][j] = cp.ta;
+                    s_cp[3][j] = cp.tb;
+                    s_cp[4][j] = cp.ga;
+                    s_cp[5][j] = cp.gb;
+                    s_flag[j] = cp.evol ? 1 : 0;
+                    if (cp.gfar <= 0.f) {
+                        glc::ArcPlan<float> pl;
+                        glc::plan_inside(cp, &pl);
+                        push_arcs(j, pl);
+                        narc = pl.narc;
+                    } else {
+                        cross = true;
+                    }
+                }
+            }
+            append(cross, &s_ncross, s_cross, j);
+            append(narc >= 1, &s_narcs, s_arcs, 2 * j);
+            append(narc == 2, &s_narcs, s_arcs, 2 * j + 1);
+        }
+        __syncthreads();
+        // ---- E2
+        const int ncross = s_ncross;
+        for (int q0 = 0; q0 < ncross; q0 += EVO_NT) {
+            const int q = q0 + tid;
+            int narc = 0, j = 0;
+            if (q < ncross) {
+                j = s_cross[q];
+                const EvoRow r = evo_row(geom, s_rows[j]);
+                glc::CritPoints<float> cp;
+                cp.tfar = s_cp[0][j];
+                cp.gfar = s_cp[1][j];
+                cp.ta = s_cp[2][j];
+                cp.tb = s_cp[3][j];
+                cp.ga = s_cp[4][j];
+                cp.gb = s_cp[5][j];
+                cp.evol = (s_flag[j] & 1u) != 0;
+                glc::ArcPlan<float> pl;
+                glc::plan_crossing<float, true>(r.o, cp, &pl);
+                if (pl.narc == 0) out[s_rows[j]] = 1.f;
+                else push_arcs(j, pl);
+                narc = pl.narc;
+            }
+            append(narc >= 1, &s_narcs, s_arcs, 2 * j);
+            append(narc == 2, &s_narcs, s_arcs, 2 * j + 1);
+        }
+        __syncthreads();
+        // ---- E3
+        const int narcs = s_narcs;
+        for (int q = tid; q < narcs; q += EVO_NT) {
+            const int slot = s_arcs[q];
+            const EvoRow r = evo_row(geom, s_rows[slot >> 1]);
+            const glc::ArcCoef<float> kc = glc::arc_coefficients(r.o);
+            const float t1 = s_as[slot], t2 = s_ae[slot];
+            float s1, c1, s2, c2, A[3] = {0.f, 0.f, 0.f};
+            glc::gtrig<true>(t1, &s1, &c1);
+            glc::gtrig<true>(t2, &s2, &c2);
+            glc::add_outline_arc<float, 16, true>(r.o, kc, t1, s1, c1, t2, s2, c2, glf::c_gl_phi, glf::c_gl_om, A);
+            s_A[0][slot] = A[0];
+            s_A[1][slot] = A[1];
+            s_A[2][slot] = A[2];
+        }
+        __syncthreads();
+        // ---- E4
         for (int j = tid; j < n; j += EVO_NT) {
-            const long long k = s_rows[j];
-            const double* g = geom + k * GL_NGEOM;
-            const double d = g[0], Rp = g[1], fp = g[2], pa = g[3], u1 = g[4], u2 = g[5];
-            float s, c;
-            glh::angle_sincos(pa, &s, &c);   // (the same preparation as geometry_sorted_kernel)
-            const float a = (float)Rp, b = (float)(Rp * (1.0 - fp)), r0 = (float)d;
-            const float ipn = glh::rcp_nr((float)(kPi * (1.0 - u1 / 3.0 - u2 / 6.0)));
-            float A[3];
-            float delta = 0.f;
-            if (glc::overlap_areas<float, 16, true>(fabsf(r0 * c), fabsf(r0 * s), a, b, glf::c_gl_phi, glf::c_gl_om, A))
-                delta = fmaf((float)(1.0 - u1 - 2.0 * u2) * ipn, A[0],
-                             fmaf((float)(u1 + 2.0 * u2) * ipn, A[1], (float)u2 * ipn * A[2]));
-            out[k] = 1.f - delta;
+            const int narc = (s_flag[j] >> 1) & 3;
+            if (narc == 0) continue;
+            const EvoRow r = evo_row(geom, s_rows[j]);
+            float A[3] = {0.f, 0.f, 0.f};
+            for (int i = 0; i < narc; ++i) {
+                A[0] += s_A[0][2 * j + i];
+                A[1] += s_A[1][2 * j + i];
+                A[2] += s_A[2][2 * j + i];
+            }
+            if (s_flag[j] & 8u) {
+                float ss[2], cs[2], se[2], ce[2];
+                for (int i = 0; i < narc; ++i) {
+                    glc::gtrig<true>(s_as[2 * j + i], &ss[i], &cs[i]);
+                    glc::gtrig<true>(s_ae[2 * j + i], &se[i], &ce[i]);
+                }
+                for (int i = 0; i < narc; ++i) {
+                    const int i2 = (i + 1 == narc) ? 0 : i + 1;
+                    glc::add_limb_arc(r.o.xc + r.o.a * ce[i], r.o.yc + r.o.b * se[i], r.o.xc + r.o.a * cs[i2],
+                                      r.o.yc + r.o.b * ss[i2], A);
+                }
+            }
+            out[s_rows[j]] = 1.f - fmaf(r.k0, A[0], fmaf(r.k1, A[1], r.k2 * A[2]));
         }
     };
     // blocks of 32 rows, round-robin over the CTAs (see geometry_sorted_kernel); warp w of the CTA takes
