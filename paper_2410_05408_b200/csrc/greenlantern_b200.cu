@@ -480,6 +480,7 @@ __device__ __forceinline__ int glh::generic_unit(const glh::HotArgs& A, bool pre
     if (tid == 0) walker_prelude_orbit<float>(p, GL_NPARAMS, A.t_exp, &gw);
     if (tid == 32) walker_prelude_shape<float>(p, GL_NPARAMS, &gw);
     __syncthreads();
+    GLH_TL(11);
     const double* __restrict__ seg = A.times + t_lo;
     float* frow = A.flux ? A.flux + (size_t)wk * A.T + t_lo : nullptr;
     if (!gw.valid) {
@@ -551,6 +552,7 @@ __device__ __forceinline__ int glh::generic_unit(const glh::HotArgs& A, bool pre
         }
         if (in) s_li[before + __popc(bal & ((1u << lane) - 1u))] = i;
         __syncthreads();
+        GLH_TL(12);
         for (int g0 = 0; g0 < n_in; g0 += G) {   // (n_in is the CTA's: the barriers below are uniform)
             const int ng = min(G, n_in - g0);
             for (int q = tid; q < ng * S; q += glh::HOT_NT) {
@@ -558,12 +560,14 @@ __device__ __forceinline__ int glh::generic_unit(const glh::HotArgs& A, bool pre
                 s_d[q] = sample(seg[s_li[g0 + e]], j);
             }
             __syncthreads();
+            GLH_TL(13);
             for (int e = tid; e < ng; e += glh::HOT_NT) {
                 float sum = 0.f;
                 for (int j = 0; j < S; ++j) sum += s_d[e * S + j];
                 finish(s_li[g0 + e], sum * A.inv_ss);
             }
             __syncthreads();
+            GLH_TL(14);
         }
     }
     return glh::CLS_SIMPLE;
