@@ -207,41 +207,63 @@ __device__ __forceinline__ double largest_axis(const double* __restrict__ p, int
     return m;
 }
 
-template <typename R>
-__device__ void walker_prelude_orbit(const double* __restrict__ p, int nparams, double t_exp, Walker* w) {
-    const bool ok = walker_valid(p, nparams);
-    w->valid = ok ? 1 : 0;
-    if (!ok) return;
-    const double t0 = p[0], P = p[1], aR = p[2], b = p[3], e = p[4], om = p[5];
-    const double Rp = largest_axis(p, nparams);
+// The ORBIT half comes in three parts that write disjoint fields of the Walker and read only the parameter
+// row, so that three threads can run them side by side (generic_unit: a dozen fp64 libm calls in a row took
+// 4 us on one thread); walker_prelude_orbit runs them one after the other.
+//   basic  : validity, t0, 1/P, a/R*, e, omega, locked
+//   kepler : Kepler constants of the conjunction (R7)
+//   window : sin/cos omega, cos i, the transit window in phase, reach (+ what locked_axes needs)
+__device__ void walker_prelude_basic(const double* __restrict__ p, int nparams, Walker* w) {
+    w->valid = walker_valid(p, nparams) ? 1 : 0;
     w->locked = (nparams == GL_NPARAMS_EX && p[15] == 1.0) ? 1 : 0;
-    w->t0 = t0;
-    w->inv_P = 1.0 / P;
-    w->aR = aR;
-    w->e = e;
-    w->omega = om;
+    w->t0 = p[0];
+    w->inv_P = 1.0 / p[1];
+    w->aR = p[2];
+    w->e = p[4];
+    w->omega = p[5];
+}
+__device__ void walker_prelude_kepler(const double* __restrict__ p, Walker* w) {
+    const double e = p[4], om = p[5];
+    if (e == 0.0) {
+        w->Mc = w->Ec = w->sinEc = 0.0;
+        w->cosEc = 1.0;
+        w->sq1me2 = 1.0;
+        return;
+    }
+    // R7: conjunction at true anomaly pi/2 - omega
+    const double nuc = 0.5 * kPi - om;
+    const double s1 = sqrt(1.0 + e), s2 = sqrt(1.0 - e);
+    const double Ec = 2.0 * atan2(s2 * sin(0.5 * nuc), s1 * cos(0.5 * nuc));
+    sincos(Ec, &w->sinEc, &w->cosEc);
+    w->Ec = Ec;
+    w->Mc = Ec - e * w->sinEc;
+    w->sq1me2 = s1 * s2;
+}
+template <typename R>
+__device__ void walker_prelude_window(const double* __restrict__ p, int nparams, double t_exp, Walker* w) {
+    const double P = p[1], aR = p[2], b = p[3], e = p[4], om = p[5];
+    const double inv_P = 1.0 / P;
+    const double Rp = largest_axis(p, nparams);
     // the projected semi-major axis of an oblate spheroid is its equatorial radius: the window
     // does not have to wait for the SHAPE half
     const bool lowp = sizeof(R) == 4;
     const double reach = (1.0 + Rp) * (lowp ? 1.0 + 1e-5 : 1.0 + 1e-12);
     double hw = -1.0;   // < 0: never in transit
+    double cosi;
     if (e == 0.0) {
         // PAPER.md:85-87 eqs. 9-10: the centre is within `reach` of the star centre iff
         //   sin^2(phi) < [(reach/aR)^2 - cos^2 i] / sin^2 i  and cos(phi) > 0;
         // stored as a half-width in orbital phase, widened by half an exposure.
-        w->cosi = b / aR;
-        w->Mc = w->Ec = w->sinEc = 0.0;
-        w->cosEc = 1.0;
+        cosi = b / aR;
         w->sinw = 0.0;
         w->cosw = 1.0;
-        w->sq1me2 = 1.0;
-        const R ci2 = R(w->cosi) * R(w->cosi), q = R(reach) / R(aR);
+        const R ci2 = R(cosi) * R(cosi), q = R(reach) / R(aR);
         const R S2 = (q * q - ci2) / (R(1) - ci2);
         if (S2 > R(0))
             hw = (S2 >= R(1)) ? 0.25
                               : (double)(glc::gasin(glc::gsqrt(S2)) * R(0.15915494309189535)) *
                                     (lowp ? 1.0 + 1e-5 : 1.0);
-        if (hw >= 0.0) hw += 0.5 * t_exp * w->inv_P + (lowp ? 1e-9 : 1e-13);
+        if (hw >= 0.0) hw += 0.5 * t_exp * inv_P + (lowp ? 1e-9 : 1e-13);
         // exposures wholly inside |phase| < hard_phase keep the outline at least 0.01 inside the
         // limb (the cheap tiers of gl_fast32.cuh); the others (ingress, egress, grazing) are
         // listed FIRST so that the expensive geometries start early (scheduling only)
@@ -249,19 +271,14 @@ __device__ void walker_prelude_orbit(const double* __restrict__ p, int nparams, 
         const R S2h = (qh * qh - ci2) / (R(1) - ci2);
         double hp = 0.0;
         if (S2h > R(0) && S2h < R(1))
-            hp = (double)(glc::gasin(glc::gsqrt(S2h)) * R(0.15915494309189535)) - 0.5 * t_exp * w->inv_P;
+            hp = (double)(glc::gasin(glc::gsqrt(S2h)) * R(0.15915494309189535)) - 0.5 * t_exp * inv_P;
         w->hard_phase = hp > 0.0 ? hp : 0.0;
     } else {
-        // R7: conjunction at true anomaly pi/2 - omega; cos i from the impact parameter
+        // R7: cos i from the impact parameter
         const double nuc = 0.5 * kPi - om;
         const double s1 = sqrt(1.0 + e), s2 = sqrt(1.0 - e);
-        const double Ec = 2.0 * atan2(s2 * sin(0.5 * nuc), s1 * cos(0.5 * nuc));
-        sincos(Ec, &w->sinEc, &w->cosEc);
         sincos(om, &w->sinw, &w->cosw);
-        w->Ec = Ec;
-        w->Mc = Ec - e * w->sinEc;
-        w->sq1me2 = s1 * s2;
-        w->cosi = (b / aR) * (1.0 + e * w->sinw) / (1.0 - e * e);
+        cosi = (b / aR) * (1.0 + e * w->sinw) / (1.0 - e * e);
         // Transit window in phase, conservative.  With phi' = nu - nu_c the angle from conjunction,
         // the sky distance is >= r |sin phi'| >= aR (1-e) |sin phi'|, so in transit needs
         // |phi'| < phi_max = asin(reach / (aR (1-e))); the time to sweep phi_max is at most
@@ -279,20 +296,28 @@ __device__ void walker_prelude_orbit(const double* __restrict__ p, int nparams, 
             if (off < -kPi) off += kTwoPi;
             if (fabs(off) <= pmax) cmin = -1.0;
             const double slow = (1.0 + e * cmin) * (1.0 + e * cmin);
-            hw = pmax / kTwoPi * (1.0 - e * e) * s1 * s2 / slow * (1.0 + 1e-6) + 0.5 * t_exp * w->inv_P + 1e-9;
+            hw = pmax / kTwoPi * (1.0 - e * e) * s1 * s2 / slow * (1.0 + 1e-6) + 0.5 * t_exp * inv_P + 1e-9;
             if (hw > 0.5) hw = 0.5;
         }
         w->hard_phase = 0.0;
     }
+    w->cosi = cosi;
     w->half_win_phase = hw;
     w->reach = reach;
-    if (w->locked) {
+    if (nparams == GL_NPARAMS_EX && p[15] == 1.0) {
         // eq. 9: x0 = d cos(alpha) sin(beta)  =>  sin(beta) = cos i  (used by locked_axes)
-        w->sinb = w->cosi;
-        w->cosb = sqrt(fmax(1.0 - w->cosi * w->cosi, 0.0));
+        w->sinb = cosi;
+        w->cosb = sqrt(fmax(1.0 - cosi * cosi, 0.0));
         w->sinbf = (float)w->sinb;
         w->cosbf = (float)w->cosb;
     }
+}
+template <typename R>
+__device__ void walker_prelude_orbit(const double* __restrict__ p, int nparams, double t_exp, Walker* w) {
+    walker_prelude_basic(p, nparams, w);
+    if (!w->valid) return;
+    walker_prelude_kepler(p, w);
+    walker_prelude_window<R>(p, nparams, t_exp, w);
 }
 
 template <typename R>
@@ -477,8 +502,12 @@ __device__ __forceinline__ int glh::generic_unit(const glh::HotArgs& A, bool pre
     __shared__ Walker gw;
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const double* p = A.params + (size_t)wk * GL_NPARAMS;
-    if (tid == 0) walker_prelude_orbit<float>(p, GL_NPARAMS, A.t_exp, &gw);
+    // four threads of four warps, side by side (the parts write disjoint fields; on an invalid row the
+    // three that do not judge validity compute garbage that nobody reads)
+    if (tid == 0) walker_prelude_basic(p, GL_NPARAMS, &gw);
     if (tid == 32) walker_prelude_shape<float>(p, GL_NPARAMS, &gw);
+    if (tid == 64) walker_prelude_kepler(p, &gw);
+    if (tid == 96) walker_prelude_window<float>(p, GL_NPARAMS, A.t_exp, &gw);
     __syncthreads();
     GLH_TL(11);
     const double* __restrict__ seg = A.times + t_lo;
@@ -541,7 +570,9 @@ __device__ __forceinline__ int glh::generic_unit(const glh::HotArgs& A, bool pre
             if (!in && frow) frow[i] = 1.f;
         }
         const unsigned bal = __ballot_sync(0xffffffffu, in);
-        __syncthreads();   // the previous pass is done with s_li / s_d / s_cnt
+        // (the barrier also says that the previous pass is done with s_li / s_d / s_cnt; most passes of a
+        // K2-shaped series hold no in-window exposure at all and end here)
+        if (__syncthreads_count(in) == 0) continue;
         if (lane == 0) s_cnt[warp] = __popc(bal);
         __syncthreads();
         int before = 0, n_in = 0;
