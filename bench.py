@@ -457,6 +457,16 @@ def secondary_calls(gl, dev, d, w3, ser3, P3):
     calls["cfg3_gl_loglike_stateless"] = (
         lambda: gl.gl_loglike(P3, T3, w3.t_exp, w3.n_ss, O3, S3, dtype="f32", want_flux=True), w3.B * w3.T, "flux_evals")
     calls["cfg3_chi2_only"] = (lambda: ser3.loglike_dev(P3, chi2_out=chi2_only), w3.B * w3.T, "flux_evals")
+    # the same batch with every walker on an eccentric orbit (e = 0.2, omega uniform): off hot_kernel's common
+    # path, same single launch (generic_unit: Kepler's equation per sub-exposure)
+    pe = w3.params.copy()
+    pe[:, 4] = 0.2
+    pe[:, 5] = np.random.default_rng(wl.SEED_CFG3_WALKERS + 7).uniform(0.0, 2.0 * np.pi, w3.B)
+    P3e = d(pe)
+    chi2_e = torch.empty(w3.B, dtype=torch.float32, device=dev)
+    flux_e = torch.empty((w3.B, w3.T), dtype=torch.float32, device=dev)
+    calls["cfg3_all_walkers_eccentric_e0.2"] = (
+        lambda: ser3.loglike_dev(P3e, want_flux=True, chi2_out=chi2_e, flux_out=flux_e), w3.B * w3.T, "flux_evals")
     calls["cfg3_fp64"] = (
         lambda: gl.gl_loglike(P3, T3, w3.t_exp, w3.n_ss, O3, S3, dtype="f64", want_flux=True), w3.B * w3.T, "flux_evals")
     gp3 = d(np.tile([2e-4, 0.5, 1e-4], (w3.B, 1)))
