@@ -9,8 +9,10 @@ exposure mean, chi^2) over one batch: chi2[B] AND flux[B,T] for B walkers agains
 (gl_series_loglike_dev: the series was uploaded once, the parameter rows are resident in HBM).
 Default workload: config 3 of BASELINE.json (B=256 walkers x T=3900 x 15 sub-exposures, fp32), the
 configuration the metric's ">= 40 % of FP32 SIMT peak" is quoted on.  Prints ONE JSON line.
-`extra` carries the other workloads (cfg4, cfg5, cfg3 in fp64, one light curve of 1e5 exposures,
-the stateless gl_loglike call) timed the same way in the same run.
+`extra` carries the other workloads (cfg4, cfg5, cfg3 in fp64, cfg3 with every walker eccentric, the GP
+likelihood, the paper's snap + Simpson kernel, one light curve of 1e5 exposures, the stateless
+gl_loglike call) timed the same way in the same run; `roofline.event_time_vs_kernel_time` shows how the
+event timer of this hardware quantises a kernel's duration.
 `--gpus N` without a torchrun environment starts N ranks itself (torch.distributed.run on
 127.0.0.1); `--dry` exercises that plumbing on a CPU box with the gloo backend and no kernels.
 See DESIGN.md section 6 for what every key means and how the roofline numbers are formed.
@@ -42,7 +44,7 @@ N_SM, LANES = 148, 128
 # inside the disc (16 f_lin nodes x 60-70 flop + ~100), 1.4-1.6 kflop when it crosses the limb (root
 # isolation + polishing + atan2).  Mid-points; the mix is counted per workload from the sky distance.
 ALG_FLOP_INSIDE, ALG_FLOP_LIMB = 1050.0, 1500.0
-NCU_FILE = ROOT / "profiles" / "r02_ncu_constants.json"
+NCU_FILE = ROOT / "profiles" / "r02_ncu_constants.json.txt"
 
 
 def ncu_constants():
