@@ -581,6 +581,7 @@ __device__ __forceinline__ int glh::generic_unit(const glh::HotArgs& A, bool pre
             before += k < warp ? c : 0;
             n_in += c;
         }
+        GLH_ASSERT(before + __popc(bal) <= n_in && n_in <= glh::HOT_NT && n_in <= glh::CAP);
         if (in) s_li[before + __popc(bal & ((1u << lane) - 1u))] = i;
         __syncthreads();
         GLH_TL(12);
@@ -588,12 +589,14 @@ __device__ __forceinline__ int glh::generic_unit(const glh::HotArgs& A, bool pre
             const int ng = min(G, n_in - g0);
             for (int q = tid; q < ng * S; q += glh::HOT_NT) {
                 const int e = q / S, j = q - e * S;
+                GLH_ASSERT(q < glh::CAP && g0 + e < n_in && s_li[g0 + e] >= 0 && s_li[g0 + e] < nT);
                 s_d[q] = sample(seg[s_li[g0 + e]], j);
             }
             __syncthreads();
             GLH_TL(13);
             for (int e = tid; e < ng; e += glh::HOT_NT) {
                 float sum = 0.f;
+                GLH_ASSERT(e * S + S <= glh::CAP);
                 for (int j = 0; j < S; ++j) sum += s_d[e * S + j];
                 finish(s_li[g0 + e], sum * A.inv_ss);
             }
@@ -1201,12 +1204,14 @@ geometry_evolute_kernel(const double* __restrict__ geom, long long N, float* out
     asm volatile("griddepcontrol.wait;" ::: "memory");
     __syncthreads();
     // warp-aggregated append to a shared list (the ballot is taken by all 32 lanes)
-    auto append = [&](bool mine, int* counter, unsigned short* list, int value) {
+    auto append = [&](bool mine, int* counter, unsigned short* list, int capacity, int value) {
         const unsigned bal = __ballot_sync(0xffffffffu, mine);
         if (!bal) return;
         int base = 0;
         if (lane == 0) base = atomicAdd(counter, __popc(bal));
         base = __shfl_sync(0xffffffffu, base, 0);
+        GLH_ASSERT(base >= 0 && base + __popc(bal) <= capacity);
+        (void)capacity;
         if (mine) list[base + __popc(bal & ((1u << lane) - 1u))] = (unsigned short)value;
     };
     auto push_arcs = [&](int j, const glc::ArcPlan<float>& pl) {   // (narc > 0)
@@ -1248,9 +1253,9 @@ geometry_evolute_kernel(const double* __restrict__ geom, long long N, float* out
                     }
                 }
             }
-            append(cross, &s_ncross, s_cross, j);
-            append(narc >= 1, &s_narcs, s_arcs, 2 * j);
-            append(narc == 2, &s_narcs, s_arcs, 2 * j + 1);
+            append(cross, &s_ncross, s_cross, EVO_CAP, j);
+            append(narc >= 1, &s_narcs, s_arcs, 2 * EVO_CAP, 2 * j);
+            append(narc == 2, &s_narcs, s_arcs, 2 * EVO_CAP, 2 * j + 1);
         }
         __syncthreads();
         // ---- E2
@@ -1275,8 +1280,8 @@ geometry_evolute_kernel(const double* __restrict__ geom, long long N, float* out
                 else push_arcs(j, pl);
                 narc = pl.narc;
             }
-            append(narc >= 1, &s_narcs, s_arcs, 2 * j);
-            append(narc == 2, &s_narcs, s_arcs, 2 * j + 1);
+            append(narc >= 1, &s_narcs, s_arcs, 2 * EVO_CAP, 2 * j);
+            append(narc == 2, &s_narcs, s_arcs, 2 * EVO_CAP, 2 * j + 1);
         }
         __syncthreads();
         // ---- E3
@@ -1335,6 +1340,7 @@ geometry_evolute_kernel(const double* __restrict__ geom, long long N, float* out
                 int base = 0;
                 if (lane == 0) base = atomicAdd(&s_n, __popc(bal));
                 base = __shfl_sync(0xffffffffu, base, 0);
+                GLH_ASSERT(base >= 0 && base + __popc(bal) <= EVO_CAP);
                 if (marked) s_rows[base + __popc(bal & ((1u << lane) - 1u))] = k;
             }
         }
