@@ -25,12 +25,20 @@ template <> struct num<float> {
     // angle tolerance of the bracketed solves: an angle error eps moves the areas by O(eps^2) only
     // (gl_fast32.cuh header), so fp32 does not chase the last ulp
     static constexpr float tol = 2e-5f;
+    // ... and the CRITICAL POINTS of g need far less: they serve as brackets for the crossings, as places to
+    // open or split a contour (any point will do) and as the arguments of g(t_far), g(t_a), g(t_b), g(t_near),
+    // which are stationary there (an angle error eps moves them by O(eps^2) = 1e-6 of an O(a) quantity).
+    // Measured on config 5 (host build, 4e5 rows): iterations of a critical-point search 3.9 -> 2.4 on average,
+    // 95th percentile 12 -> 4 (the tail was bisection inside the tiny brackets of nearly symmetric outlines),
+    // max |flux error| per class unchanged (1.3e-7).
+    static constexpr float tol_h = 1e-3f;
     static constexpr float nudge = 2.5e-7f; // quadrant brackets are pulled strictly inside by this
     static constexpr int maxit = 40;
 };
 template <> struct num<double> {
     static constexpr double pi = 3.14159265358979323846;
     static constexpr double tol = 4e-16;
+    static constexpr double tol_h = 4e-16;
     static constexpr double nudge = 5e-16;
     static constexpr int maxit = 80;
 };
@@ -116,7 +124,7 @@ GL_DEV T solve_in(const Outline<T>& o, T lo, T hi, T t, bool rising) {
         if (!(tn > lo && tn < hi)) tn = T(0.5) * (lo + hi);
         const T d = tn - t;
         t = tn;
-        if (gabs(d) <= num<T>::tol * gmax(T(1), gabs(t))) break;
+        if (gabs(d) <= (WHICH == 1 ? num<T>::tol_h : num<T>::tol) * gmax(T(1), gabs(t))) break;
     }
     return t;
 }
