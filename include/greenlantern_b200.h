@@ -211,7 +211,9 @@ int gl_flux_geometry_host(const double* geom, long long N, void* flux_out, gl_dt
  * gl_series_loglike: params [B, GL_NPARAMS] fp64 HOST (any memory), B <= B_max; chi2_out [B] float
  *   HOST; flux_out_or_null [B, T] float HOST.  Synchronous: returns when the outputs are written.
  *   The kernel reads the parameter rows from, and writes chi^2 to, pinned host memory directly (no
- *   copy engine on the path); flux, when asked for, comes back by one device-to-host copy.  Same
+ *   copy engine on the path); a chi^2-only call waits on a completion word in pinned memory that the
+ *   kernel's last CTA sets (no stream synchronise; after 2 s without it the stream is synchronised
+ *   and its error, if any, returned); flux, when asked for, comes back by one device-to-host copy.  Same
  *   values as gl_loglike(GL_F32) up to the rounding of S (kept in fp64 here, narrowed there).
  * gl_series_loglike_dev: params, chi2_out, flux_out_or_null are DEVICE pointers; work is enqueued on
  *   `stream` without synchronising (the series buffers are only read, so several streams may use
