@@ -9,7 +9,8 @@ exposure mean, chi^2) over one batch: chi2[B] AND flux[B,T] for B walkers agains
 (gl_series_loglike_dev: the series was uploaded once, the parameter rows are resident in HBM).
 Default workload: config 3 of BASELINE.json (B=256 walkers x T=3900 x 15 sub-exposures, fp32), the
 configuration the metric's ">= 40 % of FP32 SIMT peak" is quoted on.  Prints ONE JSON line.
-`extra` carries the other workloads (cfg4, cfg5, cfg3 in fp64, cfg3 with every walker eccentric, the GP
+`extra` carries the other workloads (cfg4, cfg5, cfg3 in fp64, cfg3 with every walker eccentric, cfg3's series
+with 4096 walkers, the GP
 likelihood, the paper's snap + Simpson kernel, one light curve of 1e5 exposures, the stateless
 gl_loglike call) timed the same way in the same run; `roofline.event_time_vs_kernel_time` shows how the
 event timer of this hardware quantises a kernel's duration.
@@ -471,6 +472,15 @@ def secondary_calls(gl, dev, d, w3, ser3, P3):
         lambda: ser3.loglike_dev(P3e, want_flux=True, chi2_out=chi2_e, flux_out=flux_e), w3.B * w3.T, "flux_evals")
     calls["cfg3_fp64"] = (
         lambda: gl.gl_loglike(P3, T3, w3.t_exp, w3.n_ss, O3, S3, dtype="f64", want_flux=True), w3.B * w3.T, "flux_evals")
+    # the same series with 16x the walkers (sixteen waves of CTAs): what the kernel sustains once the launch is
+    # not one walker's dependent chain any more (context for roofline.frac; not BASELINE.json's configuration)
+    Bbig = 16 * w3.B
+    serb = gl.GlSeries(w3.times, w3.obs, w3.sigma, w3.t_exp, w3.n_ss, Bbig, device=dev)
+    Pb = d(wl.draw_walkers(Bbig, wl.SEED_CFG3_WALKERS + 99))
+    chi2_b = torch.empty(Bbig, dtype=torch.float32, device=dev)
+    flux_b = torch.empty((Bbig, w3.T), dtype=torch.float32, device=dev)
+    calls["cfg3_shape_B4096"] = (
+        lambda: serb.loglike_dev(Pb, want_flux=True, chi2_out=chi2_b, flux_out=flux_b), Bbig * w3.T, "flux_evals")
     gp3 = d(np.tile([2e-4, 0.5, 1e-4], (w3.B, 1)))
     calls["cfg3_gp_loglike"] = (
         lambda: gl.gl_gp_loglike(P3, T3, w3.t_exp, w3.n_ss, O3, S3, gp3, dtype="f32"), w3.B * w3.T, "flux_evals")
@@ -492,7 +502,7 @@ def secondary_calls(gl, dev, d, w3, ser3, P3):
     p1 = d(wl.CFG2_ROW[None, :])
     f1 = torch.empty((1, T1), dtype=torch.float32, device=dev)
     calls["single_lightcurve_T1e5"] = (lambda: gl.gl_lightcurve(p1, t1, 0.0, 1, dtype="f32", out=f1), T1, "flux_evals")
-    return calls, {"w4": w4, "ser4": ser4}
+    return calls, {"w4": w4, "ser4": ser4, "serb": serb, "Pb_rows": Bbig}
 
 
 def extra_workloads(gl, dev, d, timed, fractions, peak_tflops, probe, ncu, w3, ser3, P3):
@@ -514,6 +524,17 @@ def extra_workloads(gl, dev, d, timed, fractions, peak_tflops, probe, ncu, w3, s
     n_in, n_limb = in_transit_mix(w4)
     ex["cfg4"].update({"B": w4.B, "T": w4.T, "n_ss": w4.n_ss, "in_transit_subsamples": n_in,
                        "of_which_limb_crossing": n_limb, **fractions("cfg4", n_in, n_limb, ex["cfg4"]["ms"])})
+    # (the walkers of the large batch are drawn like config 3's: the in-transit mix per walker is the same)
+    n_in3, n_limb3 = in_transit_mix(w3)
+    scale = keep["Pb_rows"] / w3.B
+    ex["cfg3_shape_B4096"].update({"B": keep["Pb_rows"], "note": "in-transit counts scaled from config 3's walkers",
+                                   **fractions("cfg3", int(n_in3 * scale), int(n_limb3 * scale),
+                                               ex["cfg3_shape_B4096"]["ms"])})
+    if "executed_flop_ncu" in ex["cfg3_shape_B4096"]:      # the capture is of the 256-walker launch: scale it
+        exf3 = ex["cfg3_shape_B4096"]["executed_flop_ncu"] * scale
+        ex["cfg3_shape_B4096"]["executed_flop_ncu"] = exf3
+        ex["cfg3_shape_B4096"]["frac_executed"] = exf3 / (ex["cfg3_shape_B4096"]["ms"] * 1e-3) / 1e12 / peak_tflops
+    keep["serb"].close()
     ex["cfg5"]["active_lanes_per_instruction_ncu"] = ncu.get("active_lanes", {}).get("cfg5")
     ex["single_lightcurve_T1e5"].update({
         "us_per_flux_sample": ex["single_lightcurve_T1e5"]["ms"] * 1e3 / 100_000,
