@@ -561,6 +561,7 @@ __device__ __forceinline__ int generic_unit(const HotArgs& A, bool pre, int wk, 
 template <bool PRE>
 __global__ void __launch_bounds__(HOT_NT, 2) hot_kernel(const HotArgs A) {
     asm volatile("griddepcontrol.launch_dependents;");   // a dependent launch (the GP scan) may become resident
+    GLH_TL(15);
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int csize = (int)gridDim.x, crank = (int)blockIdx.x;
     cg::cluster_group cluster = cg::this_cluster();
@@ -577,7 +578,6 @@ __global__ void __launch_bounds__(HOT_NT, 2) hot_kernel(const HotArgs A) {
     __shared__ int s_li[CAP];              // ... index in the segment of in-window exposure e
     __shared__ float2 s_ow[CAP];           // ... its (obs - 1, 1/sigma)
     __shared__ glf::TrapNode s_trap[16];
-    if (tid < 16) s_trap[tid] = glf::TrapNode{c_trap16[tid].x, c_trap16[tid].y};
 
     const int S = A.n_ss;
     const float inv_ss = A.inv_ss, doff = A.doff, off0 = A.off0;
@@ -681,6 +681,13 @@ __global__ void __launch_bounds__(HOT_NT, 2) hot_kernel(const HotArgs A) {
             const long long ci = (long long)tid * stride;
             GLH_ASSERT(ci >= 0 && (ci < nT || ci >= nT));
             s_coarse[tid] = ci < nT ? seg[ci] : __longlong_as_double(0x7ff0000000000000LL);
+        }
+        // the node table of the fixed-angle rules, from constant memory: filled HERE by the last warp, behind
+        // the first loads of the unit, and not in front of the kernel's first barrier -- after an L2 flush the
+        // constant-cache miss sat on the entry path of every CTA (entry to first unit: 2.0 us flushed, 1.1 warm)
+        if (kun == 0 && tid >= HOT_NT - 16) {
+            const int k = tid - (HOT_NT - 16);
+            s_trap[k] = glf::TrapNode{c_trap16[k].x, c_trap16[k].y};
         }
         int unsorted = 0;
         if (!A.sorted_known) {   // (every CTA of a cluster looks at ALL pairs: the verdict must be the cluster's)
