@@ -1010,7 +1010,10 @@ geometry_sorted_kernel(const double* __restrict__ geom, long long N, float* __re
     __shared__ int s_count[4], s_start[5], s_count2[3], s_start2[4];
     const int tid = threadIdx.x;
     asm volatile("griddepcontrol.launch_dependents;");   // geometry_evolute_kernel may become resident
-    if (tid < 16) s_trap[tid] = glf::TrapNode{glh::c_trap16[tid].x, glh::c_trap16[tid].y};
+    // node table of the fixed-angle rules (constant memory): the loads are issued now by the last 16 threads, the
+    // values stored behind stage 1 -- nobody waits for the constant cache in front of the kernel's first barrier
+    float2 trap_mine = make_float2(0.f, 0.f);
+    if (tid >= GEO_NT - 16) trap_mine = glh::c_trap16[tid - (GEO_NT - 16)];
     if (tid < 4) s_count[tid] = 0;
     if (tid < 3) s_count2[tid] = 0;
     __syncthreads();
@@ -1059,6 +1062,7 @@ geometry_sorted_kernel(const double* __restrict__ geom, long long N, float* __re
         s_par[6][loc] = (float)u2 * ipn;
         slot[q] = atomicAdd(&s_count[4 - path[q]], 1);   // list 0 = path 4 (the long one first)
     }
+    if (tid >= GEO_NT - 16) s_trap[tid - (GEO_NT - 16)] = glf::TrapNode{trap_mine.x, trap_mine.y};
     __syncthreads();
     if (tid == 0) {
         int run = 0;
@@ -1201,6 +1205,13 @@ geometry_evolute_kernel(const double* __restrict__ geom, long long N, float* out
     __shared__ int s_n, s_ncross, s_narcs;
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     if (tid == 0) s_n = 0;
+    // the quadrature table (constant memory) is copied while this grid still waits for the first kernel: E3
+    // finds it in shared memory instead of missing the constant cache on its critical path
+    __shared__ float s_gl[16];
+    if (tid < 8) {
+        s_gl[tid] = glf::c_gl_phi[tid];
+        s_gl[8 + tid] = glf::c_gl_om[tid];
+    }
     asm volatile("griddepcontrol.wait;" ::: "memory");
     __syncthreads();
     // warp-aggregated append to a shared list (the ballot is taken by all 32 lanes)
@@ -1294,7 +1305,7 @@ geometry_evolute_kernel(const double* __restrict__ geom, long long N, float* out
             float s1, c1, s2, c2, A[3] = {0.f, 0.f, 0.f};
             glc::gtrig<true>(t1, &s1, &c1);
             glc::gtrig<true>(t2, &s2, &c2);
-            glc::add_outline_arc<float, 16, true>(r.o, kc, t1, s1, c1, t2, s2, c2, glf::c_gl_phi, glf::c_gl_om, A);
+            glc::add_outline_arc<float, 16, true>(r.o, kc, t1, s1, c1, t2, s2, c2, s_gl, s_gl + 8, A);
             s_A[0][slot] = A[0];
             s_A[1][slot] = A[1];
             s_A[2][slot] = A[2];
