@@ -656,7 +656,9 @@ __global__ void __launch_bounds__(HOT_NT, 2) hot_kernel(const HotArgs A) {
     __shared__ unsigned s_defer[MAXDEFER_WORDS];
     const unsigned nunits = (unsigned)A.B * (unsigned)A.nseg;
     {
-        const unsigned mine = blockIdx.y < nunits ? (nunits - blockIdx.y + gridDim.y - 1) / gridDim.y : 0u;
+        // (one unit per CTA row unless the batch exceeds the grid: no division then)
+        const unsigned mine = blockIdx.y >= nunits ? 0u
+                              : (nunits <= gridDim.y ? 1u : (nunits - blockIdx.y + gridDim.y - 1) / gridDim.y);
         GLH_ASSERT((mine + 31) / 32 <= MAXDEFER_WORDS);
         for (unsigned i = tid; i < (mine + 31) / 32; i += HOT_NT) s_defer[i] = 0u;   // (barrier: top of the loop)
     }
@@ -758,7 +760,8 @@ __global__ void __launch_bounds__(HOT_NT, 2) hot_kernel(const HotArgs A) {
             // for a single-transit series): len_k = max(hi_k - lo_k, 0) -- an unsorted share of the
             // series may give anything: such a unit was classified CLS_DEFER above and never gets here
             int M = 0;   // in-window exposures of the unit (the whole cluster's)
-            for (int k = 0; k < nep; ++k) M += max(su.hi[k] - su.lo[k], 0);
+#pragma unroll 1
+            for (int k = 0; k < nep; ++k) M += max(su.hi[k] - su.lo[k], 0);   // (nep is 1 for a single-transit series)
             // v-th in-window exposure of the unit -> its index in the segment and its time from the
             // centre of its transit, (float)(t - t_c): the fp64 phase reduction is gone
             auto entry = [&](int v, int* idx) {
@@ -808,11 +811,14 @@ __global__ void __launch_bounds__(HOT_NT, 2) hot_kernel(const HotArgs A) {
                 const int head = (int)((4u - (((uintptr_t)frow >> 2) & 3u)) & 3u);
                 if (ft < head && ft < nT && !inwin(ft)) frow[ft] = 1.f;
                 const int nchunk = nT > head ? (nT - head) >> 2 : 0;
+                // (one transit in the series is the common case: its range sits in registers, not in a loop
+                // over shared memory per 16-byte chunk)
+                const int lo0 = nep > 0 ? su.lo[0] : 0, hi0 = nep > 0 ? su.hi[0] : 0;
                 for (int c = ft; c < nchunk; c += nft) {
                     const int i0 = head + 4 * c;
-                    bool hit = false;
+                    bool hit = (i0 + 3 >= lo0 && i0 < hi0);
 #pragma unroll 1
-                    for (int k = 0; k < nep; ++k) hit = hit || (i0 + 3 >= su.lo[k] && i0 < su.hi[k]);
+                    for (int k = 1; k < nep; ++k) hit = hit || (i0 + 3 >= su.lo[k] && i0 < su.hi[k]);
                     if (!hit) {
                         GLH_ASSERT(i0 >= 0 && i0 + 3 < nT && (((uintptr_t)(frow + i0)) & 15u) == 0);
                         *reinterpret_cast<float4*>(frow + i0) = make_float4(1.f, 1.f, 1.f, 1.f);
